@@ -1,0 +1,483 @@
+"""Pins for the oracle: what the paper and the mathematics fix (CPU only, no CUDA).
+
+Each test is chosen so that a plausible mistake in oracle/kbmod_oracle.c (a dropped term, a wrong
+sign or index, a transposed operand, P instead of P^2, a wrong percentile rank) fails it.
+Citations are PAPER.md lines; R-numbers are DESIGN.md readings.
+"""
+import math
+import os
+
+import numpy as np
+import pytest
+from scipy import signal, special
+
+from oracle import oracle as O
+from paper_2109_03296_b200 import synth
+from tests import brute
+
+GOLDEN = os.path.join(os.path.dirname(__file__), "golden", "paper_constants.txt")
+
+
+def golden():
+    out = {}
+    for line in open(GOLDEN):
+        line = line.split("#")[0].split()
+        if len(line) == 2:
+            out[line[0]] = float(line[1])
+    return out
+
+
+def P(**kw):
+    return O.Params(**kw)
+
+
+# ------------------------------------------------------------------ sigma-G constant (Eq. 1-5)
+def test_coefficient_closed_form_matches_paper_constant():
+    """L117: C_25,75 ~ 0.7413; Eq. 4 (with the sqrt(2) of Eq. 3, R12): C = 1/(sqrt2 (erfinv(.5) - erfinv(-.5)))."""
+    g = golden()
+    c = 1.0 / (math.sqrt(2.0) * (special.erfinv(2 * 0.75 - 1) - special.erfinv(2 * 0.25 - 1)))
+    assert abs(c - g["sigmag_coeff_25_75"]) < 5e-5
+    assert abs(1.0 / (special.erfinv(0.5) - special.erfinv(-0.5)) - 1.0484) < 1e-3  # the garbled Eq. 4 without sqrt2
+    assert O.Params().coeff == pytest.approx(g["sigmag_coeff_25_75"])
+    assert (O.Params().pct_lo, O.Params().pct_hi, O.Params().n_sigma, O.Params().K) == (
+        g["sigmag_pct_lo"], g["sigmag_pct_hi"], g["sigmag_n_sigma"], g["results_per_pixel"])
+
+
+def test_percentile_ranks_match_sorted_reference():
+    """R10 nearest rank: the q-th percentile of n points is sorted(x)[ceil(q n/100) - 1]."""
+    for n in range(1, 65):
+        for q in (25.0, 50.0, 75.0, 10.0, 90.0):
+            r = O.pct_rank(q, n)
+            # smallest index whose cumulative fraction (r+1)/n reaches q/100
+            ref = next(i for i in range(n) if (i + 1) * 100.0 >= q * n)
+            assert r == ref, (n, q, r, ref)
+    assert [O.pct_rank(q, 26) for q in (25, 50, 75)] == [6, 12, 19]
+
+
+def test_kept_set_matches_sorted_reference():
+    """The kept set is {|f - median| <= 2 * 0.7413 * (P75 - P25)} with percentiles from sorted()."""
+    rng = np.random.default_rng(5)
+    for T in (1, 2, 3, 4, 5, 6, 10, 26, 50, 64):
+        n_lc = 300
+        phi = rng.uniform(0.5, 2.0, (n_lc, T)).astype(np.float32)
+        psi = (rng.standard_normal((n_lc, T)) * np.sqrt(phi)).astype(np.float32)
+        psi[rng.random((n_lc, T)) < 0.1] *= 8.0
+        phi[rng.random((n_lc, T)) < 0.15] = 0.0  # invalid epochs
+        for filter_on in (0, 1):
+            out = O.sigmag_filter(psi, phi, P(filter_on=filter_on))
+            for i in range(n_lc):
+                val = [t for t in range(T) if phi[i, t] > 0]
+                if not val:
+                    assert out["n_kept"][i] == 0 and out["lh"][i] == -np.inf
+                    continue
+                f = {t: (np.float32(psi[i, t]) / np.sqrt(np.float32(phi[i, t])) if filter_on
+                         else np.float32(psi[i, t]) / np.float32(phi[i, t])) for t in val}
+                s = sorted(f.values())
+                n = len(s)
+                p25, p50, p75 = (s[math.ceil(q * n / 100) - 1] for q in (25, 50, 75))
+                w = np.float32(2.0) * (np.float32(0.7413) * np.float32(p75 - p25))
+                keep = [t for t in val if p50 - w <= f[t] <= p50 + w]
+                bits = sum(1 << t for t in keep)
+                assert int(out["kept"][i]) == bits, (T, i)
+                sp = sum(float(psi[i, t]) for t in keep)
+                sf = sum(float(phi[i, t]) for t in keep)
+                assert out["lh"][i] == pytest.approx(sp / math.sqrt(sf), rel=1e-12, abs=1e-12)
+                assert out["flux"][i] == pytest.approx(sp / sf, rel=1e-12, abs=1e-12)
+
+
+def test_small_n_and_constant_lightcurve():
+    """R11/R13: inclusive bounds; n = 1, 2 keep everything; sigma_G = 0 keeps points equal to the median."""
+    one = O.sigmag_filter(np.array([[3.0, 0, 0]], np.float32), np.array([[2.0, 0, 0]], np.float32), P())
+    assert one["n_kept"][0] == 1 and one["lh"][0] == pytest.approx(3 / math.sqrt(2))
+    two = O.sigmag_filter(np.array([[1.0, 100.0]], np.float32), np.array([[1.0, 1.0]], np.float32), P())
+    assert two["n_kept"][0] == 2  # ranks(25,50,75 | n=2) = 0,0,1: window = 1 +- 1.48*99 -> keeps 100 too
+    const = O.sigmag_filter(np.full((1, 7), 5.0, np.float32), np.ones((1, 7), np.float32), P())
+    assert const["n_kept"][0] == 7
+    c2 = np.full((1, 7), 5.0, np.float32)
+    c2[0, 3] = 5.5  # sigma_G = 0 -> the odd one out is dropped
+    out = O.sigmag_filter(c2, np.ones((1, 7), np.float32), P())
+    assert out["n_kept"][0] == 6 and int(out["kept"][0]) == 0b1110111
+
+
+def test_two_point_window_value():
+    """n = 2: P25 = P50 = s[0], P75 = s[1]; window half-width 2*0.7413*(s1-s0) = 1.4826 (s1-s0) > s1-s0."""
+    two = O.sigmag_filter(np.array([[1.0, 100.0]], np.float32), np.array([[1.0, 1.0]], np.float32), P())
+    assert int(two["kept"][0]) == 0b11
+
+
+def test_sigma_g_estimates_gaussian_sigma():
+    """L117: sigma_G ~ sigma of the underlying Gaussian, so a 2 sigma_G clip keeps ~95.45 % of pure noise.
+    A wrong coefficient (1.0484 -> 99.5 %, 1.0 -> 99.3 %, 0.5 -> 82 %) fails."""
+    rng = np.random.default_rng(11)
+    T, n = 64, 20000
+    psi = rng.standard_normal((n, T)).astype(np.float32)
+    out = O.sigmag_filter(psi, np.ones((n, T), np.float32), P())
+    frac = out["n_kept"].sum() / (n * T)
+    assert abs(frac - math.erf(2 / math.sqrt(2))) < 0.012, frac
+
+
+def test_outlier_epoch_is_dropped_and_score_returns_to_noise():
+    """Section 3.1: one +30 sigma epoch in Gaussian noise is always clipped; L' falls back to ~N(0, 1.1)."""
+    rng = np.random.default_rng(12)
+    T, n = 26, 4000
+    psi = rng.standard_normal((n, T)).astype(np.float32)
+    psi[:, 7] += 30.0
+    phi = np.ones((n, T), np.float32)
+    raw = O.sigmag_filter(psi, phi, P(sigmag_enable=0))
+    out = O.sigmag_filter(psi, phi, P())
+    assert np.all((out["kept"] >> np.uint64(7)) & np.uint64(1) == 0)
+    assert raw["lh"].mean() == pytest.approx(30 / math.sqrt(T), abs=0.1)
+    assert abs(out["lh"].mean()) < 0.1 and 0.9 < out["lh"].std() < 1.3
+
+
+def test_lightcurve_shift_scale_equivariance():
+    """Kept set is invariant under f -> a f + b (a > 0) with exactly representable a, b."""
+    rng = np.random.default_rng(13)
+    psi = np.round(rng.standard_normal((500, 26)) * 64).astype(np.float32) / 64
+    phi = np.ones_like(psi)
+    k0 = O.sigmag_filter(psi, phi, P())["kept"]
+    k1 = O.sigmag_filter(psi * 4 + 32, phi, P())["kept"]
+    assert np.array_equal(k0, k1)
+
+
+# ------------------------------------------------------------------ O1 psi/phi
+def _point_source_stack(T, H, W, psf, F, var, starts):
+    img = np.zeros((T, H, W), np.float32)
+    r = psf.shape[0] // 2
+    for t, (x, y) in enumerate(starts):
+        img[t, y - r:y + r + 1, x - r:x + r + 1] += (F * psf).astype(np.float32)
+    return img, np.full((T, H, W), var, np.float32), np.zeros((T, H, W), np.uint8)
+
+
+def test_prep_closed_form_flux_and_snr():
+    """R1: isolated noiseless source of flux F, constant variance v: Psi/Phi = F and Psi/sqrt(Phi) =
+    F sqrt(sum P^2 / v) at the centre.  With P instead of P^2 in Phi the flux would be F sum(P^2)."""
+    psf = synth.gaussian_psf(1.0).astype(np.float64)
+    F, v = 100.0, 4.0
+    img, var, mask = _point_source_stack(1, 31, 33, psf, F, v, [(16, 14)])
+    psi, phi, valid, _ = O.prepare_psi_phi(img, var, mask, psf)
+    assert psi[0, 14, 16] / phi[0, 14, 16] == pytest.approx(F, rel=1e-6)
+    sp2 = float((psf.astype(np.float32).astype(np.float64) ** 2).sum())
+    assert psi[0, 14, 16] / math.sqrt(phi[0, 14, 16]) == pytest.approx(F * math.sqrt(sp2 / v), rel=1e-6)
+    assert np.unravel_index(np.argmax(psi[0]), psi[0].shape) == (14, 16)
+    assert valid.all()
+
+
+def test_prep_equals_library_correlation_without_mask():
+    """No mask, constant variance: Psi = correlate2d(I, P)/v, Phi = correlate2d(1, P^2)/v with zero fill."""
+    rng = np.random.default_rng(3)
+    T, H, W = 2, 19, 23
+    img = rng.standard_normal((T, H, W)).astype(np.float32)
+    k = rng.random((5, 5)).astype(np.float32)  # asymmetric: a flipped kernel (convolution) fails this
+    v = 2.0
+    psi, phi, _, _ = O.prepare_psi_phi(img, np.full_like(img, v), None, k)
+    for t in range(T):
+        ref = signal.correlate2d(img[t].astype(np.float64), k.astype(np.float64), mode="same") / v
+        assert np.allclose(psi[t], ref, rtol=1e-12, atol=1e-12)
+        ref2 = signal.correlate2d(np.ones((H, W)), k.astype(np.float64) ** 2, mode="same") / v
+        assert np.allclose(phi[t], ref2, rtol=1e-12)
+
+
+def test_prep_asymmetric_kernel_peak_location():
+    """R2 correlation: an image equal to P centred at c has its Psi maximum at c."""
+    k = np.zeros((5, 5), np.float32)
+    k[0, 4], k[2, 2], k[4, 1] = 0.5, 0.3, 0.2
+    img = np.zeros((1, 21, 21), np.float32)
+    img[0, 8:13, 9:14] = k  # centred at (y, x) = (10, 11)
+    psi, _, _, _ = O.prepare_psi_phi(img, np.ones_like(img), None, k)
+    assert np.unravel_index(np.argmax(psi[0]), (21, 21)) == (10, 11)
+
+
+def test_prep_masked_neighbours_keep_flux_and_canvas_embedding():
+    """R3: masking neighbour taps of a noiseless isolated source leaves Psi/Phi = F; a masked centre is
+    invalid; embedding in a larger fully masked canvas changes nothing (mask == off-image)."""
+    psf = synth.gaussian_psf(1.5).astype(np.float64)
+    F = 50.0
+    img, var, mask = _point_source_stack(1, 41, 41, psf, F, 1.0, [(20, 20)])
+    rng = np.random.default_rng(4)
+    mask[0] = (rng.random((41, 41)) < 0.3).astype(np.uint8)
+    mask[0, 20, 20] = 0
+    mask[0, 5, 5] = 1
+    psi, phi, valid, _ = O.prepare_psi_phi(img, var, mask, psf)
+    assert psi[0, 20, 20] / phi[0, 20, 20] == pytest.approx(F, rel=1e-6)
+    assert valid[0, 5, 5] == 0 and psi[0, 5, 5] == 0 and phi[0, 5, 5] == 0
+    assert np.array_equal(valid[0], 1 - mask[0])
+    # var <= 0 and non-finite pixels behave like masked ones (R19)
+    var2, img2 = var.copy(), img.copy()
+    var2[0][mask[0] == 1] = 0.0
+    img2[0, 7, 7], mask2 = np.nan, np.zeros_like(mask)
+    mask3 = mask.copy(); mask3[0, 7, 7] = 1
+    a = O.prepare_psi_phi(img2, var2, mask2, psf)
+    b = O.prepare_psi_phi(img, var, mask3, psf)
+    assert np.array_equal(a[0], b[0]) and np.array_equal(a[1], b[1]) and np.array_equal(a[2], b[2])
+    # canvas embedding
+    big = np.zeros((1, 61, 71), np.float32); bv = np.ones_like(big); bm = np.ones((1, 61, 71), np.uint8)
+    big[0, 10:51, 15:56], bm[0, 10:51, 15:56] = img[0], mask[0]
+    c = O.prepare_psi_phi(big, bv, bm, psf)
+    assert np.array_equal(c[0][0, 10:51, 15:56], psi[0]) and np.array_equal(c[1][0, 10:51, 15:56], phi[0])
+
+
+def test_prep_per_epoch_psf():
+    rng = np.random.default_rng(6)
+    img = rng.standard_normal((3, 12, 13)).astype(np.float32)
+    var = rng.uniform(0.5, 2, (3, 12, 13)).astype(np.float32)
+    ks = rng.random((3, 3, 3)).astype(np.float32)
+    allp = O.prepare_psi_phi(img, var, None, ks)
+    for t in range(3):
+        one = O.prepare_psi_phi(img[t:t + 1], var[t:t + 1], None, ks[t])
+        assert np.array_equal(allp[0][t], one[0][0]) and np.array_equal(allp[1][t], one[1][0])
+
+
+# ------------------------------------------------------------------ O2 displacements
+def test_round_half_up_and_translation():
+    """R5: d = floor(v dt + 1/2): +2.5 -> 3, -2.5 -> -2; config 1's vy = 5 at t = 0.5 d lands on 33 from 30."""
+    times = np.array([0.0, 0.5, 1.0])
+    dx, dy = O.displacements(times, np.array([5.0, -5.0, 20.0], np.float32), np.array([5.0, -5.0, 5.0], np.float32))
+    assert dx.tolist() == [[0, 3, 5], [0, -2, -5], [0, 10, 20]]
+    assert dy[2].tolist() == [0, 3, 5]
+    # time zero point is irrelevant (R18) and epochs need not start at 0
+    dx2, _ = O.displacements(times + 57000.25, np.array([5.0, -5.0, 20.0], np.float32), np.zeros(3, np.float32))
+    assert np.array_equal(dx, dx2)
+    rng = np.random.default_rng(7)
+    t = np.sort(rng.random(9) * 4); v = (rng.standard_normal(200) * 300).astype(np.float32)
+    dx, _ = O.displacements(t, v, v)
+    assert np.array_equal(dx, brute.round_half_up(v.astype(np.float64)[:, None] * (t - t[0])[None, :]))
+
+
+# ------------------------------------------------------------------ search: closed form, zero, brute force
+def _closed_form_case(T=5, H=40, W=48, F=100.0, var=1.0, sigma=1.0):
+    psf = synth.gaussian_psf(sigma)
+    times = np.arange(T, dtype=np.float64) * 0.5
+    vx, vy = synth.velocity_grid(8, 8, -math.pi / 4, math.pi / 4, 0.0, 16.0)
+    vx = np.concatenate([vx, [8.0, 4.0]]).astype(np.float32)  # integer displacements at dt = 0.5 k
+    vy = np.concatenate([vy, [4.0, -2.0]]).astype(np.float32)
+    true_v = len(vx) - 2
+    starts = [(10 + int(round(8.0 * t)), 12 + int(round(4.0 * t))) for t in times]
+    img, v, m = _point_source_stack(T, H, W, psf.astype(np.float64), F, var, starts)
+    return img, v, m, psf, times, vx, vy, true_v
+
+
+def test_search_recovers_point_source_with_closed_form_score():
+    """Pin 1 (north_star): noiseless constant-variance stack, one point source at a known velocity is the top
+    trajectory with L = F sqrt(T sum P^2 / v), flux = F, n_kept = T, and nothing scores higher (Cauchy-Schwarz)."""
+    F, var, T = 100.0, 1.0, 5
+    img, v, m, psf, times, vx, vy, true_v = _closed_form_case(T=T, F=F, var=var)
+    psi, phi, _, _ = O.prepare_psi_phi(img, v, m, psf)
+    pp = O.interleave(psi, phi)
+    lh, flux, vel, nobs = O.search(pp, times, vx, vy, P(K=1))
+    sp2 = float((psf.astype(np.float64) ** 2).sum())
+    L_true = F * math.sqrt(T * sp2 / var)
+    assert L_true == pytest.approx(63.119, abs=2e-3)  # sigma = 1, F = 100, v = 1, T = 5
+    best = np.unravel_index(np.argmax(lh[..., 0]), lh.shape[:2])
+    assert best == (12, 10)
+    assert vel[12, 10, 0] == true_v
+    assert lh[12, 10, 0] == pytest.approx(L_true, rel=1e-6)
+    assert flux[12, 10, 0] == pytest.approx(F, rel=1e-6)
+    assert nobs[12, 10, 0] == T
+    assert lh.max() <= L_true * (1 + 1e-9)
+
+
+def test_all_zero_psi_gives_zero_scores_not_sentinel():
+    """Pin 2: img = 0 -> L' = 0 and flux' = 0 for every trajectory; K results per pixel, lowest vel_idx first."""
+    T, H, W = 4, 9, 11
+    pp = O.interleave(np.zeros((T, H, W)), np.ones((T, H, W)))
+    vx, vy = np.array([0, 1, -1], np.float32), np.array([0, 1, 2], np.float32)
+    lh, flux, vel, nobs = O.search(pp, np.arange(T, dtype=float), vx, vy, P(K=2))
+    assert np.all(lh == 0) and np.all(flux == 0)
+    assert np.all(vel[..., 0] == 0) and np.all(vel[..., 1] == 1)
+    assert nobs[0, 0, 0] == T
+
+
+@pytest.mark.parametrize("seed,T,H,W,filter_on,min_obs", [(0, 4, 12, 16, 0, 1), (1, 5, 16, 13, 1, 2), (2, 7, 9, 10, 0, 4)])
+def test_search_equals_numpy_brute_force(seed, T, H, W, filter_on, min_obs):
+    """Pin 3: per-velocity shifted-image numpy formulation == per-trajectory oracle (same sets, same doubles)."""
+    st = synth.random_stack(seed, T, H, W, mask_frac=0.1, t_span=2.0)
+    psi, phi, valid, _ = O.prepare_psi_phi(st.img, st.var, st.mask, st.psf)
+    pp = O.interleave(psi, phi)
+    rng = np.random.default_rng(seed)
+    vx = (rng.uniform(-6, 6, 14)).astype(np.float32); vy = (rng.uniform(-6, 6, 14)).astype(np.float32)
+    vx[3], vy[3] = vx[2], vy[2]  # exact duplicate -> tie broken by lower index (R15)
+    K = 3
+    p = P(K=K, filter_on=filter_on, min_obs=min_obs, min_lh=-np.inf)
+    lh, flux, vel, nobs = O.search(pp, st.times, vx, vy, p)
+    L, F, NK, KEPT = brute.all_scores(pp[..., 0], pp[..., 1], st.times, vx, vy, filter_on=filter_on, min_obs=min_obs)
+    blh, bfl, bvi, bno = brute.topk(L, F, NK, K)
+    assert np.array_equal(vel, bvi)
+    assert np.array_equal(nobs, bno)
+    assert np.allclose(lh, blh, rtol=1e-12, atol=1e-12, equal_nan=True)
+    assert np.allclose(flux, bfl, rtol=1e-12, atol=1e-12)
+    # with a threshold
+    p2 = P(K=K, filter_on=filter_on, min_obs=min_obs, min_lh=1.0)
+    lh2, _, vel2, _ = O.search(pp, st.times, vx, vy, p2)
+    blh2, _, bvi2, _ = brute.topk(L, F, NK, K, min_lh=1.0)
+    assert np.array_equal(vel2, bvi2) and np.allclose(lh2, blh2, rtol=1e-12, equal_nan=True)
+    # single-trajectory variant agrees with the brute force kept masks
+    yy, xx = np.mgrid[0:H, 0:W]
+    for v in (0, 5, 13):
+        ev = O.eval_trajectories(pp, st.times, xx.ravel(), yy.ravel(), np.full(H * W, vx[v]), np.full(H * W, vy[v]), p)
+        assert np.array_equal(ev["kept"].reshape(H, W), KEPT[v])
+        ok = ~np.isnan(L[v])
+        assert np.allclose(ev["lh"].reshape(H, W)[ok], L[v][ok], rtol=1e-12, atol=1e-12)
+        assert np.all(ev["lh"].reshape(H, W)[~ok] == -np.inf)
+
+
+def test_search_without_filter_is_plain_sum():
+    """sigma-G off: L = sum psi / sqrt(sum phi) over on-image valid epochs (L79)."""
+    st = synth.random_stack(9, 5, 10, 12, mask_frac=0.0)
+    psi, phi, _, _ = O.prepare_psi_phi(st.img, st.var, None, st.psf)
+    pp = O.interleave(psi, phi)
+    vx, vy = np.array([2.0], np.float32), np.array([-1.0], np.float32)
+    lh, flux, vel, nobs = O.search(pp, st.times, vx, vy, P(K=1, sigmag_enable=0))
+    dt = st.times - st.times[0]
+    for (y, x) in [(0, 0), (5, 5), (9, 11), (3, 10)]:
+        sp = sf = 0.0; n = 0
+        for t in range(5):
+            xx, yy = x + int(math.floor(2.0 * dt[t] + .5)), y + int(math.floor(-1.0 * dt[t] + .5))
+            if 0 <= xx < 12 and 0 <= yy < 10:
+                sp += float(pp[t, yy, xx, 0]); sf += float(pp[t, yy, xx, 1]); n += 1
+        assert lh[y, x, 0] == pytest.approx(sp / math.sqrt(sf), rel=1e-12)
+        assert nobs[y, x, 0] == n
+
+
+# ------------------------------------------------------------------ invariants (pin 5)
+def _noise_case(seed=21, T=6, H=14, W=15):
+    st = synth.random_stack(seed, T, H, W, mask_frac=0.08, t_span=1.5)
+    rng = np.random.default_rng(seed)
+    vx = rng.uniform(-5, 5, 10).astype(np.float32); vy = rng.uniform(-5, 5, 10).astype(np.float32)
+    return st, vx, vy
+
+
+def test_invariance_scaling():
+    """(I, var) -> (c I, c^2 var), c a power of two: L' unchanged, flux' x c, same kept sets."""
+    st, vx, vy = _noise_case()
+    a = O.prepare_psi_phi(st.img, st.var, st.mask, st.psf)
+    b = O.prepare_psi_phi(st.img * 4, st.var * 16, st.mask, st.psf)
+    ra = O.search(O.interleave(a[0], a[1]), st.times, vx, vy, P(K=2))
+    rb = O.search(O.interleave(b[0], b[1]), st.times, vx, vy, P(K=2))
+    assert np.array_equal(ra[2], rb[2]) and np.array_equal(ra[3], rb[3])
+    assert np.allclose(ra[0], rb[0], rtol=1e-6) and np.allclose(ra[1] * 4, rb[1], rtol=1e-6)
+
+
+def test_invariance_translation_and_canvas_embedding():
+    """Embedding the psi/phi stack in a larger invalid canvas == the off-image rule; results translate."""
+    st, vx, vy = _noise_case(22)
+    psi, phi, _, _ = O.prepare_psi_phi(st.img, st.var, st.mask, st.psf)
+    pp = O.interleave(psi, phi)
+    T, H, W, _ = pp.shape
+    big = np.zeros((T, H + 30, W + 30, 2), np.float32)
+    big[:, 12:12 + H, 17:17 + W] = pp
+    ra = O.search(pp, st.times, vx, vy, P(K=2, min_obs=2))
+    rb = O.search(big, st.times, vx, vy, P(K=2, min_obs=2))
+    for a, b in zip(ra, rb):
+        assert np.array_equal(a, b[12:12 + H, 17:17 + W], equal_nan=True)
+
+
+def test_invariance_epoch_permutation_and_masked_epoch_equals_deleted_epoch():
+    st, vx, vy = _noise_case(23, T=7)
+    psi, phi, _, _ = O.prepare_psi_phi(st.img, st.var, st.mask, st.psf)
+    pp = O.interleave(psi, phi)
+    perm = np.array([0, 4, 2, 6, 1, 5, 3])  # epoch 0 stays the time origin
+    ra = O.search(pp, st.times, vx, vy, P(K=2))
+    rb = O.search(pp[perm], st.times[perm], vx, vy, P(K=2))
+    assert np.array_equal(ra[2], rb[2]) and np.array_equal(ra[3], rb[3])
+    assert np.allclose(ra[0], rb[0], rtol=1e-12) and np.allclose(ra[1], rb[1], rtol=1e-12)
+    # epoch 3 fully invalid == epoch 3 deleted (R8)
+    gone = pp.copy(); gone[3] = 0
+    keep = [0, 1, 2, 4, 5, 6]
+    rc = O.search(gone, st.times, vx, vy, P(K=2))
+    rd = O.search(pp[keep], st.times[keep], vx, vy, P(K=2))
+    assert np.array_equal(rc[2], rd[2]) and np.array_equal(rc[3], rd[3]) and np.array_equal(rc[0], rd[0])
+
+
+def test_filter_choice_irrelevant_for_constant_variance():
+    """R9: with constant phi, filtering flux or likelihood keeps the same set."""
+    rng = np.random.default_rng(24)
+    psi = rng.standard_normal((400, 26)).astype(np.float32); psi[:, 3] += 9
+    phi = np.full_like(psi, 4.0)  # sqrt(4) = 2 exact
+    a = O.sigmag_filter(psi, phi, P(filter_on=0)); b = O.sigmag_filter(psi, phi, P(filter_on=1))
+    assert np.array_equal(a["kept"], b["kept"])
+
+
+def test_min_obs_and_threshold():
+    T, H, W = 5, 6, 20
+    pp = O.interleave(np.ones((T, H, W)), np.ones((T, H, W)))
+    vx, vy = np.array([4.0], np.float32), np.array([0.0], np.float32)
+    lh, _, vel, nobs = O.search(pp, np.arange(T, dtype=float), vx, vy, P(K=1, min_obs=3))
+    assert nobs[0, 3, 0] == 5 and nobs[0, 11, 0] == 3 and vel[0, 12, 0] == -1 and lh[0, 12, 0] == -np.inf
+    lh, _, vel, _ = O.search(pp, np.arange(T, dtype=float), vx, vy, P(K=1, min_lh=2.0))
+    assert vel[0, 3, 0] == 0 and lh[0, 3, 0] == pytest.approx(math.sqrt(5))
+    assert vel[0, 11, 0] == -1  # sqrt(3) < 2
+
+
+def test_inline_filter_protects_valid_trajectory():
+    """Pin 6 / L137: an artefact trajectory (one huge epoch) and a fainter genuine mover share a start pixel;
+    K = 1 returns the mover with the in-line filter on and the artefact with it off."""
+    T, H, W = 10, 30, 60
+    psi = np.zeros((T, H, W)); phi = np.ones((T, H, W))
+    times = np.arange(T, dtype=float)
+    for t in range(T):
+        psi[t, 10, 5 + 3 * t] = 4.0          # mover: v = (3, 0), nu = 4 per epoch -> L = 12.6
+    psi[6, 10 + 6, 5] = 60.0                 # artefact on the track of v = (0, 1): L = 60/sqrt(10) = 19
+    vx, vy = np.array([0.0, 3.0], np.float32), np.array([1.0, 0.0], np.float32)
+    pp = O.interleave(psi, phi)
+    on = O.search(pp, times, vx, vy, P(K=1, min_lh=10.0))
+    off = O.search(pp, times, vx, vy, P(K=1, min_lh=10.0, sigmag_enable=0))
+    assert off[2][10, 5, 0] == 0 and off[0][10, 5, 0] == pytest.approx(64 / math.sqrt(10))
+    assert on[2][10, 5, 0] == 1 and on[0][10, 5, 0] == pytest.approx(40 / math.sqrt(10))
+
+
+# ------------------------------------------------------------------ O7 coadd
+def test_coadd_zero_velocity_equals_numpy_crops():
+    """R17: v = 0, no mask: stamps are numpy mean / median of plain crops (even and odd T)."""
+    rng = np.random.default_rng(30)
+    for T in (4, 5):
+        img = rng.standard_normal((T, 40, 44)).astype(np.float32)
+        x0, y0 = np.array([20, 25], np.int32), np.array([15, 22], np.int32)
+        z = np.zeros(2, np.float32)
+        mean, med = O.coadd_stamps(img, None, np.arange(T, dtype=float), x0, y0, z, z, 3)
+        for i in range(2):
+            crop = img[:, y0[i] - 3:y0[i] + 4, x0[i] - 3:x0[i] + 4].astype(np.float64)
+            assert np.allclose(mean[i], crop.mean(0), rtol=1e-12) and np.array_equal(med[i], np.median(crop, 0))
+
+
+def test_coadd_moving_masked_offimage_against_python_loops():
+    rng = np.random.default_rng(31)
+    T, H, W, r = 6, 24, 26, 2
+    img = rng.standard_normal((T, H, W)).astype(np.float32)
+    mask = (rng.random((T, H, W)) < 0.2).astype(np.uint8)
+    img[2, 5, 5] = np.inf
+    times = np.sort(rng.random(T)) * 2
+    x0, y0 = np.array([1, 12, 24], np.int32), np.array([2, 10, 22], np.int32)
+    vx, vy = np.array([3.3, -4.1, 2.5], np.float32), np.array([-2.5, 2.5, 6.0], np.float32)
+    em = np.array([0b111111, 0b101101, 0b111111], np.uint64)
+    mean, med = O.coadd_stamps(img, mask, times, x0, y0, vx, vy, r, em)
+    for i in range(3):
+        for v in range(-r, r + 1):
+            for u in range(-r, r + 1):
+                vals = []
+                for t in range(T):
+                    if not (int(em[i]) >> t) & 1:
+                        continue
+                    dt = times[t] - times[0]
+                    x = int(x0[i]) + int(math.floor(float(vx[i]) * dt + 0.5)) + u
+                    y = int(y0[i]) + int(math.floor(float(vy[i]) * dt + 0.5)) + v
+                    if 0 <= x < W and 0 <= y < H and mask[t, y, x] == 0 and np.isfinite(img[t, y, x]):
+                        vals.append(float(img[t, y, x]))
+                em_, ed_ = (np.mean(vals), np.median(vals)) if vals else (0.0, 0.0)
+                assert mean[i, v + r, u + r] == pytest.approx(em_, rel=1e-12, abs=1e-15)
+                assert med[i, v + r, u + r] == pytest.approx(ed_, rel=1e-12, abs=1e-15)
+
+
+# ------------------------------------------------------------------ config 1 recovery (BASELINE.json configs[0])
+def test_config1_recovers_injected_mover_within_paper_window():
+    """configs[0]: the top result lies within 5 px / 5 px/day of the injected (20,30) @ (20,5) px/day (L177)."""
+    g = golden()
+    st = synth.config1_tiny()
+    vx, vy = synth.config1_grid()
+    psi, phi, _, _ = O.prepare_psi_phi(st.img, st.var, st.mask, st.psf)
+    lh, flux, vel, nobs = O.search(O.interleave(psi, phi), st.times, vx, vy, P(K=1, min_obs=3))
+    y, x = np.unravel_index(np.argmax(lh[..., 0]), lh.shape[:2])
+    v = vel[y, x, 0]
+    assert abs(x - 20) <= g["recovery_window_px"] and abs(y - 30) <= g["recovery_window_px"]
+    assert math.hypot(vx[v] - 20, vy[v] - 5) <= g["recovery_window_px_per_day"]
+    assert 35 < lh[y, x, 0] < 70
