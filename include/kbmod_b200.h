@@ -1,0 +1,183 @@
+/*
+ * kbmod_b200.h -- C ABI of libkbmod_b200.so: the data-parallel hot path of the KBMOD
+ * shift-and-stack moving-object search as extended by Smotherman et al. (arXiv 2109.03296),
+ * hand-written CUDA for sm_100a (NVIDIA B200).
+ *
+ * Citations are "PAPER.md:L<line>" (/root/reference/PAPER.md, the text of the paper) plus the
+ * section / equation the line falls in.  Readings of points the paper leaves open are the
+ * R-numbers of DESIGN.md.
+ *
+ * Conventions (all entry points)
+ *   - extern "C", plain pointers and sizes.  `d_` = DEVICE pointer (current CUDA device),
+ *     `h_` = HOST pointer.  Host arrays are consumed before the call returns.
+ *   - The library never allocates or frees device memory: every device buffer (inputs,
+ *     outputs, workspace) is caller-owned.  (The *_host convenience call takes a caller-owned
+ *     device arena for the same reason.)
+ *   - All kernels are enqueued on `stream` (a cudaStream_t passed as void*; NULL = the legacy
+ *     default stream).  Calls return without synchronising unless stated.
+ *   - Layouts are C-contiguous with x fastest: stacks are [T][H][W]; the psi/phi stack is
+ *     [T][H][W][2] float (psi, phi interleaved, i.e. a CUDA float2 per pixel).
+ *   - Every function returns an int status: KBMOD_OK (0) or a negative error code;
+ *     kbmod_last_error() gives a thread-local message for the last failure.
+ *   - Limits: T <= 64 epochs, K <= 32 results per pixel, PSF side k odd and <= 31,
+ *     stamp radius <= 15, T*H*W < 2^31 pixels per stack.  Outside -> KBMOD_ERR_UNSUPPORTED.
+ *   - There is no CPU fallback: without a CUDA device every compute entry point fails with
+ *     KBMOD_ERR_CUDA.
+ */
+#ifndef KBMOD_B200_H
+#define KBMOD_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define KBMOD_OK 0
+#define KBMOD_ERR_INVALID_ARG (-1) /* null pointer, non-positive size, inconsistent arguments      */
+#define KBMOD_ERR_UNSUPPORTED (-2) /* a documented limit is exceeded (see above)                   */
+#define KBMOD_ERR_WORKSPACE (-3)   /* workspace_bytes < kbmod_search_workspace_bytes(...)          */
+#define KBMOD_ERR_CUDA (-4)        /* a CUDA runtime / driver call failed (message has the detail) */
+
+#define KBMOD_MAX_T 64
+#define KBMOD_MAX_K 32
+#define KBMOD_MAX_PSF 31
+#define KBMOD_MAX_STAMP_RADIUS 15
+
+/* Which search kernel kbmod_search runs.  Both give the same results. */
+#define KBMOD_ALGO_AUTO 0   /* pruned when min_lh is finite and sigma-G is on, else direct       */
+#define KBMOD_ALGO_DIRECT 1 /* every trajectory gets the full sigma-G evaluation                 */
+#define KBMOD_ALGO_PRUNED 2 /* exact upper bound from shared-memory tiles first, full evaluation
+                               only for trajectories whose bound reaches the threshold           */
+
+/* sigma-G filter + selection parameters.  kbmod_default_params() fills the paper's values. */
+typedef struct {
+    int sigmag_enable; /* 1: apply the in-line sigma-G lightcurve filter (s3.2)   */
+    float pct_lo;      /* 25  lower percentile  (s3.1)                                  */
+    float pct_hi;      /* 75  upper percentile                                        */
+    float sigmag_coeff;/* 0.7413  sigma_G = coeff * (P_hi - P_lo)  (Eq. 5)              */
+    float n_sigma;     /* 2   keep points within +- n_sigma * sigma_G of the median    */
+    int filter_on;     /* 0: filter the flux lightcurve psi/phi; 1: the likelihood lightcurve
+                          psi/sqrt(phi)  ("likelihood and/or flux values"; reading R9)   */
+    float min_lh;      /* keep a trajectory iff its recomputed likelihood L' >= min_lh
+                          (10); -INFINITY keeps everything                              */
+    int min_obs;       /* minimum number of valid epochs BEFORE filtering (reading R8)  */
+    int K;             /* results kept per start pixel (8)                              */
+    int algo;          /* KBMOD_ALGO_*                                                                 */
+} kbmod_search_params;
+
+/* Fills *p with the paper's operating point: sigma-G on, 25/75, 0.7413, n=2, flux lightcurve,
+ * min_lh=10, min_obs=1, K=8, algo=AUTO. */
+void kbmod_default_params(kbmod_search_params* p);
+
+/* ---------------------------------------------------------------------------------------------
+ * (a1) psi/phi preparation.  PAPER.md:L79 (s3): "KBMOD generates images of likelihood (Psi_i)
+ * and variance (Phi_i) ... as described in Whidden et al. (2019)"; masks and variance planes are
+ * part of the input.  Reading R1-R4:
+ *     w(x,y)   = 1/var(x,y) if the pixel is on-image, mask==0, var>0, img and var finite; else 0
+ *     Psi(x,y) = sum_{j,i} P[j][i] * img(x+i-r, y+j-r) * w(x+i-r, y+j-r)        (correlation)
+ *     Phi(x,y) = sum_{j,i} P[j][i]^2 * w(x+i-r, y+j-r),        r = k/2
+ * An output pixel whose own centre pixel has w == 0 is invalid and is written as (0, 0).
+ *   d_img, d_var  [T][H][W] float32          d_mask  [T][H][W] uint8, non-zero = bad; may be NULL
+ *   h_psf         [n_psf][k][k] float32 on the HOST; n_psf is 1 (shared) or T (per epoch); k odd
+ *   d_psiphi      out, [T][H][W][2] float32
+ * float32 arithmetic (FMA accumulation); agrees with the double-precision definition to
+ * 1e-5 * sum|P I w| (psi) and 1e-5 * Phi (phi). */
+int kbmod_prepare_psi_phi(const float* d_img, const float* d_var, const uint8_t* d_mask, int T, int H, int W,
+                          const float* h_psf, int n_psf, int k, float* d_psiphi, void* stream);
+
+/* ---------------------------------------------------------------------------------------------
+ * (a2) displacement table, host only (no GPU needed).  PAPER.md:L79-L81: the images are
+ * "shifted along a potential asteroid trajectory" by "pointer arithmetic"; reading R5/R18:
+ *     dx[v][t] = floor( (double)vx[v] * (times[t]-times[0]) + 0.5 )     (round half up)
+ * multiply and add separately rounded in IEEE double.  The position of trajectory (x0,y0,v) at
+ * epoch t is (x0+dx[v][t], y0+dy[v][t]).   h_dx, h_dy: out, [n_vel][T] int32. */
+int kbmod_displacements(const double* h_times, int T, const float* h_vx, const float* h_vy, int n_vel,
+                        int32_t* h_dx, int32_t* h_dy);
+
+/* ---------------------------------------------------------------------------------------------
+ * (a3)-(a5) the search: gather + in-line sigma-G + per-pixel top-K.
+ * PAPER.md:L79 (Psi_coadd = sum Psi_i, Phi_coadd = sum Phi_i, nu = Psi_coadd/sqrt(Phi_coadd)),
+ * L81, L93-L117 (s3.1, Eq. 1-5), L123, L127-L137 (s3.2).  For every start pixel (x0,y0) in
+ * [0,W)x[0,H) and every velocity v in [0,n_vel):
+ *   1. gather (psi_t, phi_t) at (x0+dx[v][t], y0+dy[v][t]); a sample is valid iff on-image and
+ *      phi_t > 0; n = number of valid samples; if n < max(1,min_obs) the trajectory has no result;
+ *   2. if sigmag_enable: f_t = psi_t/phi_t (filter_on=0) or psi_t/sqrt(phi_t) (filter_on=1) in
+ *      IEEE float32; s = ascending sort of the n valid f; P_q = s[ceil(q*n/100)-1] (nearest rank,
+ *      clamped to [0,n-1]; R10); sigma_G = coeff*(P_hi-P_lo); kept = { t valid :
+ *      P_50 - n_sigma*sigma_G <= f_t <= P_50 + n_sigma*sigma_G } (one pass, inclusive bounds,
+ *      each float32 operation separately rounded; R11-R13).  Else kept = valid;
+ *   3. L' = sum_kept psi / sqrt(sum_kept phi), flux' = sum_kept psi / sum_kept phi (float32);
+ *      the trajectory is dropped if !(L' >= min_lh);
+ *   4. per start pixel keep the K survivors with the largest L' (ties: lower velocity index),
+ *      sorted descending.
+ * Outputs, each [H][W][K]: d_lh (L'), d_flux (flux'), d_vel_idx, d_n_obs (= |kept|).  Unfilled
+ * slots hold lh=-INFINITY, flux=0, vel_idx=-1, n_obs=0.
+ *   d_psiphi   [T][H][W][2] float32 (kbmod_prepare_psi_phi's output; not modified)
+ *   h_times    [T] double, days, any zero point, any order (R18)
+ *   h_vx, h_vy [n_vel] float32, px/day
+ *   d_workspace caller-owned scratch of at least kbmod_search_workspace_bytes(...) bytes,
+ *               256-byte aligned; contents undefined on entry and exit.
+ * kbmod_search does host-side planning (the displacement table and the velocity grouping), copies
+ * small tables to the workspace with cudaMemcpyAsync on `stream`, and enqueues the kernels. */
+size_t kbmod_search_workspace_bytes(int T, int H, int W, int n_vel, const kbmod_search_params* p);
+int kbmod_search(const float* d_psiphi, int T, int H, int W, const double* h_times, const float* h_vx,
+                 const float* h_vy, int n_vel, const kbmod_search_params* p, float* d_lh, float* d_flux,
+                 int32_t* d_vel_idx, int32_t* d_n_obs, void* d_workspace, size_t workspace_bytes, void* stream);
+
+/* Counters of the last kbmod_search on this thread (read after synchronising the stream).
+ * h_out[0] = trajectories fully evaluated (sigma-G run), h_out[1] = trajectories nominally
+ * searched (H*W*n_vel), h_out[2] = kernels launched by the call, h_out[3] = algo actually used. */
+int kbmod_search_stats(const void* d_workspace, unsigned long long* h_out);
+
+/* ---------------------------------------------------------------------------------------------
+ * (a6) coadded stamps.  PAPER.md:L141 (s3.3): stamps are coadded by "computing the median pixel
+ * value for each pixel along the trajectory"; mean/sum is the earlier variant; 21x21 (L145, L175);
+ * reading R17.  For trajectory i and stamp offset (u,v) in [-radius,radius]^2 the samples are
+ * img_t(x0+dx_t+u, y0+dy_t+v) over epochs t that are selected (bit t of d_epoch_mask[i], all
+ * epochs when d_epoch_mask is NULL), on-image, unmasked and finite.  mean = sum/count;
+ * median = middle of the sort (mean of the two middles for an even count); count 0 -> 0.
+ *   d_x0,d_y0 [n_traj] int32; d_vx,d_vy [n_traj] float32 (px/day); displacements as in (a2)
+ *   d_mean, d_median  out, [n_traj][2r+1][2r+1] float32 (v rows, u columns); either may be NULL */
+int kbmod_coadd_stamps(const float* d_img, const uint8_t* d_mask, int T, int H, int W, const double* h_times,
+                       const int32_t* d_x0, const int32_t* d_y0, const float* d_vx, const float* d_vy,
+                       const uint64_t* d_epoch_mask, int n_traj, int radius, float* d_mean, float* d_median,
+                       void* stream);
+
+/* ---------------------------------------------------------------------------------------------
+ * Single-trajectory variant (s4.1: "computes the likelihoods along a single
+ * trajectory then runs the ... quantile-based filtering").  Steps 1-3 of kbmod_search for an
+ * explicit list of trajectories; min_lh and K are ignored.
+ *   d_psi_lc, d_phi_lc  out [n_traj][T] float32 (0 where invalid); may be NULL
+ *   d_valid, d_kept     out [n_traj] uint64, bit t = epoch t valid / kept; may be NULL
+ *   d_lh, d_flux        out [n_traj] float32; n < max(1,min_obs): lh=-INFINITY, flux=0, kept=0 */
+int kbmod_eval_trajectories(const float* d_psiphi, int T, int H, int W, const double* h_times,
+                            const int32_t* d_x0, const int32_t* d_y0, const float* d_vx, const float* d_vy,
+                            int n_traj, const kbmod_search_params* p, float* d_psi_lc, float* d_phi_lc,
+                            uint64_t* d_valid, uint64_t* d_kept, float* d_lh, float* d_flux, void* stream);
+
+/* sigma-G on given lightcurves (the paper's post-filter; BASELINE configs[4]).
+ * Epoch t of lightcurve i is valid iff d_phi_lc[i][t] > 0.  Steps 2-3 of kbmod_search. */
+int kbmod_sigmag_filter(const float* d_psi_lc, const float* d_phi_lc, int n_lc, int T,
+                        const kbmod_search_params* p, uint64_t* d_kept, float* d_lh, float* d_flux, void* stream);
+
+/* ---------------------------------------------------------------------------------------------
+ * Whole path from HOST buffers (what bench.py's end-to-end number times): H2D copies of the
+ * image / variance / mask stacks, kbmod_prepare_psi_phi, kbmod_search, D2H copies of the four
+ * result arrays, then synchronises `stream`.  h_mask may be NULL.  Host buffers should be pinned
+ * for the copies to run at full PCIe speed (pageable memory works, slower).
+ *   d_arena  caller-owned device scratch of at least kbmod_pipeline_host_arena_bytes(...) bytes */
+size_t kbmod_pipeline_host_arena_bytes(int T, int H, int W, int n_vel, const kbmod_search_params* p);
+int kbmod_pipeline_host(const float* h_img, const float* h_var, const uint8_t* h_mask, int T, int H, int W,
+                        const float* h_psf, int n_psf, int k, const double* h_times, const float* h_vx,
+                        const float* h_vy, int n_vel, const kbmod_search_params* p, float* h_lh, float* h_flux,
+                        int32_t* h_vel_idx, int32_t* h_n_obs, void* d_arena, size_t arena_bytes, void* stream);
+
+const char* kbmod_last_error(void); /* thread-local, never NULL */
+int kbmod_version(void);            /* 10000*major + 100*minor + patch */
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* KBMOD_B200_H */

@@ -1,0 +1,117 @@
+// Single-trajectory variant (s4.1) and the sigma-G post-filter on given lightcurves
+// (s3.1; BASELINE configs[4]).  One thread per trajectory / lightcurve; the filter is
+// the same device function the search kernels use (common.cuh: kb_score_lightcurve).
+#include "common.cuh"
+
+namespace {
+
+constexpr int LC_THREADS = 128;
+
+template <int TP>
+__global__ void __launch_bounds__(LC_THREADS)
+eval_trajectories_kernel(const float2* __restrict__ psiphi, int T, int H, int W, const __grid_constant__ DevTimes times,
+                         const int32_t* __restrict__ x0s, const int32_t* __restrict__ y0s,
+                         const float* __restrict__ vxs, const float* __restrict__ vys, int n_traj,
+                         const __grid_constant__ DevParams P, float* __restrict__ psi_lc, float* __restrict__ phi_lc,
+                         unsigned long long* __restrict__ valid_out, unsigned long long* __restrict__ kept_out,
+                         float* __restrict__ lh_out, float* __restrict__ flux_out) {
+    extern __shared__ float scratch_all[];
+    float* scratch = scratch_all + threadIdx.x;
+    const int i = blockIdx.x * LC_THREADS + threadIdx.x;
+    if (i >= n_traj) return;
+    const int x0 = x0s[i], y0 = y0s[i];
+    const float vx = vxs[i], vy = vys[i];
+    const size_t plane = (size_t)H * W;
+    float psi[TP], phi[TP];
+    unsigned long long valid = 0ull;
+#pragma unroll
+    for (int t = 0; t < TP; ++t) {
+        psi[t] = 0.0f;
+        phi[t] = 0.0f;
+        if (t < T) {
+            const int x = x0 + kb_displacement(vx, times.dt[t]);
+            const int y = y0 + kb_displacement(vy, times.dt[t]);
+            if (x >= 0 && x < W && y >= 0 && y < H) {
+                const float2 s = __ldg(psiphi + t * plane + (size_t)y * W + x);
+                if (s.y > 0.0f) {
+                    psi[t] = s.x;
+                    phi[t] = s.y;
+                    valid |= 1ull << t;
+                }
+            }
+        }
+    }
+    float lh, flux;
+    unsigned long long kept;
+    kb_score_lightcurve<TP>(psi, phi, P, scratch, LC_THREADS, lh, flux, kept);
+    if (psi_lc)
+#pragma unroll
+        for (int t = 0; t < TP; ++t)
+            if (t < T) psi_lc[(size_t)i * T + t] = psi[t];
+    if (phi_lc)
+#pragma unroll
+        for (int t = 0; t < TP; ++t)
+            if (t < T) phi_lc[(size_t)i * T + t] = phi[t];
+    if (valid_out) valid_out[i] = valid;
+    if (kept_out) kept_out[i] = kept;
+    if (lh_out) lh_out[i] = lh;
+    if (flux_out) flux_out[i] = flux;
+}
+
+template <int TP>
+__global__ void __launch_bounds__(LC_THREADS)
+sigmag_filter_kernel(const float* __restrict__ psi_lc, const float* __restrict__ phi_lc, int n_lc, int T,
+                     const __grid_constant__ DevParams P, unsigned long long* __restrict__ kept_out,
+                     float* __restrict__ lh_out, float* __restrict__ flux_out) {
+    extern __shared__ float scratch_all[];
+    float* scratch = scratch_all + threadIdx.x;
+    const int i = blockIdx.x * LC_THREADS + threadIdx.x;
+    if (i >= n_lc) return;
+    float psi[TP], phi[TP];
+#pragma unroll
+    for (int t = 0; t < TP; ++t) {
+        float a = 0.0f, b = 0.0f;
+        if (t < T) {
+            a = __ldg(psi_lc + (size_t)i * T + t);
+            b = __ldg(phi_lc + (size_t)i * T + t);
+        }
+        const bool ok = b > 0.0f;
+        psi[t] = ok ? a : 0.0f;
+        phi[t] = ok ? b : 0.0f;
+    }
+    float lh, flux;
+    unsigned long long kept;
+    kb_score_lightcurve<TP>(psi, phi, P, scratch, LC_THREADS, lh, flux, kept);
+    if (kept_out) kept_out[i] = kept;
+    if (lh_out) lh_out[i] = lh;
+    if (flux_out) flux_out[i] = flux;
+}
+
+}  // namespace
+
+int kb_launch_eval_trajectories(const float* d_psiphi, int T, int TPv, int H, int W, const DevTimes& times,
+                                const int32_t* d_x0, const int32_t* d_y0, const float* d_vx, const float* d_vy,
+                                int n_traj, const DevParams& P, float* d_psi_lc, float* d_phi_lc,
+                                unsigned long long* d_valid, unsigned long long* d_kept, float* d_lh, float* d_flux,
+                                cudaStream_t st) {
+    const int grid = (n_traj + LC_THREADS - 1) / LC_THREADS;
+    KB_DISPATCH_TP(TPv, {
+        const size_t smem = (size_t)TP * LC_THREADS * sizeof(float);
+        eval_trajectories_kernel<TP><<<grid, LC_THREADS, smem, st>>>(reinterpret_cast<const float2*>(d_psiphi), T, H, W,
+                                                                     times, d_x0, d_y0, d_vx, d_vy, n_traj, P, d_psi_lc,
+                                                                     d_phi_lc, d_valid, d_kept, d_lh, d_flux);
+    });
+    KB_CUDA(cudaGetLastError());
+    return KBMOD_OK;
+}
+
+int kb_launch_sigmag_filter(const float* d_psi_lc, const float* d_phi_lc, int n_lc, int T, int TPv, const DevParams& P,
+                            unsigned long long* d_kept, float* d_lh, float* d_flux, cudaStream_t st) {
+    const int grid = (n_lc + LC_THREADS - 1) / LC_THREADS;
+    KB_DISPATCH_TP(TPv, {
+        const size_t smem = (size_t)TP * LC_THREADS * sizeof(float);
+        sigmag_filter_kernel<TP><<<grid, LC_THREADS, smem, st>>>(d_psi_lc, d_phi_lc, n_lc, T, P, d_kept, d_lh, d_flux);
+    });
+    KB_CUDA(cudaGetLastError());
+    return KBMOD_OK;
+}

@@ -1,0 +1,111 @@
+// (a1) psi/phi preparation -- PAPER.md:L79 (s3), readings R1-R4 (see include/kbmod_b200.h).
+//   Psi = P (*) (I w),  Phi = P^2 (*) w,  w = 1/var on good pixels and 0 elsewhere (correlation).
+// One launch per epoch; the epoch's PSF travels in the kernel parameter bank (<= 31*31 floats).
+//
+// Kernel shape: a block computes a PREP_TX x PREP_TY tile of outputs.  The (I w, w) pairs of the
+// tile plus its PSF halo are staged once in shared memory (coalesced reads of img / var / mask:
+// 9 B per pixel, the algorithmic minimum, plus the halo overlap), then every thread produces
+// PREP_R vertically adjacent outputs, sliding a register window down each kernel column so that
+// one shared-memory read feeds up to PREP_R multiply-adds per plane.
+#include "common.cuh"
+
+namespace {
+
+constexpr int PREP_TX = 32;          // outputs per block in x  (one warp-row)
+constexpr int PREP_R = 8;            // outputs per thread in y
+constexpr int PREP_WARPS = 8;        // warps per block
+constexpr int PREP_TY = PREP_R * PREP_WARPS;
+
+struct PsfParam {
+    float p[KBMOD_MAX_PSF * KBMOD_MAX_PSF];
+};
+
+template <int KS>  // KS = compile-time PSF side, or 0 for a run-time side
+__global__ void __launch_bounds__(PREP_TX* PREP_WARPS)
+prep_kernel(const float* __restrict__ img, const float* __restrict__ var, const uint8_t* __restrict__ mask, int H,
+            int W, int k_rt, const __grid_constant__ PsfParam psf, float2* __restrict__ out) {
+    const int k = KS ? KS : k_rt;
+    const int r = k / 2;
+    extern __shared__ float2 tile[];  // [(PREP_TY + k - 1)][pitch]
+    const int pitch = PREP_TX + k - 1;
+    const int rows = PREP_TY + k - 1;
+    const int x_org = blockIdx.x * PREP_TX - r;
+    const int y_org = blockIdx.y * PREP_TY - r;
+    const int tid = threadIdx.y * PREP_TX + threadIdx.x;
+
+    for (int idx = tid; idx < rows * pitch; idx += PREP_TX * PREP_WARPS) {
+        const int ty = idx / pitch, tx = idx - ty * pitch;
+        const int x = x_org + tx, y = y_org + ty;
+        float2 v = make_float2(0.0f, 0.0f);
+        if (x >= 0 && x < W && y >= 0 && y < H) {
+            const size_t q = (size_t)y * W + x;
+            const float I = __ldg(img + q), V = __ldg(var + q);
+            const bool bad = (mask && __ldg(mask + q) != 0) || !(V > 0.0f) || !isfinite(V) || !isfinite(I);
+            if (!bad) {
+                const float w = 1.0f / V;
+                v = make_float2(I * w, w);
+            }
+        }
+        tile[idx] = v;
+    }
+    __syncthreads();
+
+    float ps[PREP_R], ph[PREP_R];
+#pragma unroll
+    for (int a = 0; a < PREP_R; ++a) ps[a] = ph[a] = 0.0f;
+    const int ly = threadIdx.y * PREP_R;  // first output row of this thread inside the tile
+    const int lx = threadIdx.x;
+
+    // out(ly+a) = sum_j sum_i P[j][i] * tile[ly+a+j][lx+i].  For a fixed column i walk jj = a + j
+    // down the column: each value read once, used by every output row a with 0 <= jj-a < k.
+#pragma unroll 1
+    for (int i = 0; i < k; ++i) {
+        const float2* col = tile + (size_t)ly * pitch + lx + i;
+#pragma unroll 1
+        for (int jj = 0; jj < k + PREP_R - 1; ++jj) {
+            const float2 v = col[jj * pitch];
+#pragma unroll
+            for (int a = 0; a < PREP_R; ++a) {
+                const int j = jj - a;
+                if (j >= 0 && j < k) {
+                    const float p = psf.p[j * k + i];
+                    ps[a] = fmaf(p, v.x, ps[a]);
+                    ph[a] = fmaf(p * p, v.y, ph[a]);
+                }
+            }
+        }
+    }
+
+    const int x = blockIdx.x * PREP_TX + lx;
+    if (x < W) {
+#pragma unroll
+        for (int a = 0; a < PREP_R; ++a) {
+            const int y = blockIdx.y * PREP_TY + ly + a;
+            if (y < H) {
+                const float wc = tile[(size_t)(ly + a + r) * pitch + lx + r].y;
+                out[(size_t)y * W + x] = (wc > 0.0f) ? make_float2(ps[a], ph[a]) : make_float2(0.0f, 0.0f);
+            }
+        }
+    }
+}
+
+}  // namespace
+
+int kb_launch_prep(const float* d_img, const float* d_var, const uint8_t* d_mask, int T, int H, int W,
+                   const float* h_psf, int n_psf, int k, float* d_psiphi, cudaStream_t st) {
+    const dim3 block(PREP_TX, PREP_WARPS);
+    const dim3 grid((W + PREP_TX - 1) / PREP_TX, (H + PREP_TY - 1) / PREP_TY);
+    const size_t smem = (size_t)(PREP_TY + k - 1) * (PREP_TX + k - 1) * sizeof(float2);
+    const size_t plane = (size_t)H * W;
+    PsfParam psf;
+    for (int t = 0; t < T; ++t) {
+        const float* src = h_psf + (n_psf > 1 ? (size_t)t * k * k : 0);
+        for (int i = 0; i < k * k; ++i) psf.p[i] = src[i];
+        for (int i = k * k; i < KBMOD_MAX_PSF * KBMOD_MAX_PSF; ++i) psf.p[i] = 0.0f;
+        prep_kernel<0><<<grid, block, smem, st>>>(d_img + t * plane, d_var + t * plane,
+                                                  d_mask ? d_mask + t * plane : nullptr, H, W, k, psf,
+                                                  reinterpret_cast<float2*>(d_psiphi) + t * plane);
+    }
+    KB_CUDA(cudaGetLastError());
+    return KBMOD_OK;
+}

@@ -1,0 +1,91 @@
+"""CPU-side checks of the boundary: the C-ABI library loads, exports every symbol include/kbmod_b200.h
+declares, and its host-only logic (displacement table, argument validation, workspace sizing) is right.
+No compute entry point is called here (no GPU)."""
+import ctypes as C
+import os
+import re
+
+import numpy as np
+import pytest
+
+from paper_2109_03296_b200 import binding, synth
+from paper_2109_03296_b200 import build as kb_build
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def lib():
+    kb_build.build()
+    return binding.lib()
+
+
+def declared_functions():
+    src = open(os.path.join(ROOT, "include", "kbmod_b200.h")).read()
+    src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
+    return sorted(set(re.findall(r"\b(kbmod_[a-z_]+)\s*\(", src)))
+
+
+def test_exports_every_declared_symbol(lib):
+    names = declared_functions()
+    assert len(names) >= 13
+    for n in names:
+        assert hasattr(lib, n), f"{n} declared in include/kbmod_b200.h but not exported"
+    assert set(binding.EXPORTS) == set(names)
+    for n in names:  # the Python binding carries the same names
+        assert hasattr(binding, n) or n == "kbmod_last_error"
+    assert binding.kbmod_version() >= 100
+
+
+def test_default_params_are_the_papers(lib):
+    p = binding.kbmod_default_params()
+    assert (p.sigmag_enable, p.pct_lo, p.pct_hi, p.n_sigma, p.min_lh, p.K) == (1, 25.0, 75.0, 2.0, 10.0, 8)
+    assert abs(p.sigmag_coeff - 0.7413) < 1e-7
+
+
+@pytest.mark.parametrize("cfg", ["c1", "c2", "c3", "c4", "half"])
+def test_displacement_table_bit_exact(lib, oracle, cfg):
+    """(a2) is integer work: the library's table equals the oracle's, entry by entry (reading R5)."""
+    if cfg == "c1":
+        t, (vx, vy) = np.array([0, .5, 1, 1.5, 2.]), synth.config1_grid()
+    elif cfg == "c2":
+        t, (vx, vy) = synth.config2_medium(size=16, n_movers=0).times, synth.config2_grid()
+    elif cfg == "c3":
+        t, (vx, vy) = synth.night_times((7, 6, 7, 6)), synth.config3_grid()
+    elif cfg == "c4":
+        t, (vx, vy) = synth.night_times((9, 8, 8, 9, 8, 8)), synth.config4_grid()
+    else:  # exact halves, negative and positive; times with a non-zero zero point, unsorted
+        t = np.array([10.0, 10.5, 9.5, 11.0])
+        vx = np.array([5, -5, 3, -3, 2.5, 0], np.float32)
+        vy = np.array([-1, 1, -7, 7, 0, 1e-8], np.float32)
+    dx, dy = binding.kbmod_displacements(t, vx, vy)
+    ox, oy = oracle.displacements(t, vx, vy)
+    assert np.array_equal(dx, ox) and np.array_equal(dy, oy)
+    if cfg == "half":
+        assert dx[0].tolist() == [0, 3, -2, 5] and dx[1].tolist() == [0, -2, 3, -5]  # round half up
+
+
+def test_workspace_and_validation_without_gpu(lib):
+    sp = binding.SearchParams(K=8)
+    n1 = binding.kbmod_search_workspace_bytes(26, 4096, 2048, 8192, sp)
+    n2 = binding.kbmod_search_workspace_bytes(26, 4096, 2048, 16384, sp)
+    assert 0 < n1 < n2 and n1 % 256 == 0
+    assert binding.kbmod_search_workspace_bytes(65, 10, 10, 1, sp) == 0  # T > 64 unsupported
+    cp = sp.c()
+    # argument validation happens before any CUDA call, so it is testable here
+    rc = lib.kbmod_search(None, 5, 8, 8, None, None, None, 0, C.byref(cp), None, None, None, None, None,
+                          C.c_size_t(0), None)
+    assert rc == -1 and b"NULL" in lib.kbmod_last_error()
+    rc = lib.kbmod_displacements(None, 1, None, None, 0, None, None)
+    assert rc == -1
+    one = (C.c_float * 4)()
+    rc = lib.kbmod_prepare_psi_phi(one, one, None, 1, 2, 2, one, 1, 2, one, None)
+    assert rc == -1 and b"odd" in lib.kbmod_last_error()
+    rc = lib.kbmod_prepare_psi_phi(one, one, None, 65, 2, 2, one, 1, 1, one, None)
+    assert rc == -2
+
+
+def test_binding_refuses_cpu_tensors(lib):
+    import torch
+    with pytest.raises(TypeError):
+        binding.kbmod_prepare_psi_phi(torch.zeros(1, 4, 4), torch.ones(1, 4, 4), None, np.ones((1, 1), np.float32))

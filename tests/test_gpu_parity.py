@@ -1,0 +1,252 @@
+"""GPU parity tests proper: the CUDA path (through the C ABI) against the oracle, element by element,
+on the same seeded inputs.  Sizes span several tiles and a ragged tail; protocol in tests/parity.py."""
+import math
+
+import numpy as np
+import pytest
+
+from paper_2109_03296_b200 import synth
+from tests import parity
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def kb():
+    import torch
+    import paper_2109_03296_b200 as kb_
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device (there is no CPU fallback)"
+    kb_.binding.lib()
+    return kb_
+
+
+def _cuda(a):
+    import torch
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def _prep(kb, st, psf=None):
+    out = kb.kbmod_prepare_psi_phi(_cuda(st.img), _cuda(st.var), _cuda(st.mask) if st.mask is not None else None,
+                                   st.psf if psf is None else psf)
+    return out
+
+
+def _search_and_compare(kb, O, psiphi_d, times, vx, vy, sp, pixels=None):
+    T, H, W, _ = psiphi_d.shape
+    out = kb.kbmod_search(psiphi_d, times, vx, vy, sp)
+    g = [o.cpu().numpy() for o in out]
+    psiphi = psiphi_d.cpu().numpy()
+    if pixels is None:
+        yy, xx = np.mgrid[0:H, 0:W]
+        px, py = xx.reshape(-1).astype(np.int32), yy.reshape(-1).astype(np.int32)
+    else:
+        px, py = pixels
+    op = parity.oracle_params(O, sp)
+    ora = O.search_pixels(psiphi, times, vx, vy, px, py, op)
+    gsel = [a[py, px] for a in g]
+    return parity.compare_topk(O, psiphi, times, vx, vy, op, px, py, gsel, ora)
+
+
+# ------------------------------------------------------------------------------------------- prep
+@pytest.mark.parametrize("seed,T,H,W,sigma", [(11, 3, 37, 70, 1.0), (12, 2, 130, 65, 1.8), (13, 1, 9, 5, 1.5)])
+def test_prep_random(kb, oracle, seed, T, H, W, sigma):
+    st = synth.random_stack(seed, T, H, W, psf_sigma=sigma, mask_frac=0.08)
+    st.var[0, 0, 0] = 0.0  # var <= 0 and non-finite pixels are bad pixels (reading R19)
+    st.img[0, min(3, H - 1), min(4, W - 1)] = np.nan
+    st.var[0, min(5, H - 1), 1] = np.inf
+    g = _prep(kb, st).cpu().numpy()
+    assert parity.check_prep(oracle, st, g) > 0
+
+
+def test_prep_per_epoch_asymmetric_psf(kb, oracle):
+    st = synth.random_stack(14, 3, 40, 50, mask_frac=0.03)
+    rng = np.random.default_rng(5)
+    psf = rng.random((3, 5, 5)).astype(np.float32)  # asymmetric: tells correlation from convolution (R2)
+    g = _prep(kb, st, psf).cpu().numpy()
+    parity.check_prep(oracle, st, g, psf)
+
+
+def test_prep_no_mask_and_max_psf(kb, oracle):
+    st = synth.random_stack(15, 1, 50, 80, mask_frac=0.0)
+    st.mask = None
+    psf = synth.gaussian_psf(5.0)  # 31 x 31, the largest supported
+    assert psf.shape == (31, 31)
+    g = _prep(kb, st, psf).cpu().numpy()
+    parity.check_prep(oracle, st, g, psf)
+
+
+def test_prep_config1(kb, oracle):
+    st = synth.config1_tiny()
+    parity.check_prep(oracle, st, _prep(kb, st).cpu().numpy())
+
+
+# ------------------------------------------------------------------------------------------- search
+def test_search_config1_tiny(kb, oracle):
+    """BASELINE configs[0]: every pixel, K=1, sigma-G on; the injected mover is recovered (L177 window)."""
+    st = synth.config1_tiny()
+    vx, vy = synth.config1_grid()
+    d = _prep(kb, st)
+    for min_lh in (-np.inf, 10.0):
+        sp = kb.SearchParams(K=1, min_obs=3, min_lh=min_lh, algo=kb.ALGO_DIRECT)
+        r = _search_and_compare(kb, oracle, d, st.times, vx, vy, sp)
+        assert r["n_pix"] == 64 * 64
+    lh, flux, vel, nobs = [o.cpu().numpy() for o in kb.kbmod_search(d, st.times, vx, vy, sp)]
+    y, x = np.unravel_index(np.argmax(lh[..., 0]), lh.shape[:2])
+    v = vel[y, x, 0]
+    assert abs(x - 20) <= 5 and abs(y - 30) <= 5 and abs(vx[v] - 20) <= 5 and abs(vy[v] - 5) <= 5
+    assert 35 < lh[y, x, 0] < 70
+
+
+@pytest.mark.parametrize("seed,T,H,W,K,sig,fon,min_lh,min_obs", [
+    (21, 7, 45, 70, 4, 1, 0, -np.inf, 1),
+    (22, 10, 33, 37, 8, 1, 1, -np.inf, 4),
+    (23, 5, 20, 100, 3, 0, 0, -np.inf, 2),
+    (24, 12, 40, 40, 2, 1, 0, 1.5, 6),
+    (25, 26, 24, 40, 8, 1, 0, -np.inf, 13),
+    (26, 1, 10, 10, 2, 1, 0, -np.inf, 1),
+    (27, 3, 17, 19, 32, 1, 0, -np.inf, 1),
+])
+def test_search_random(kb, oracle, seed, T, H, W, K, sig, fon, min_lh, min_obs):
+    st = synth.random_stack(seed, T, H, W, mask_frac=0.06, t_span=1.5)
+    rng = np.random.default_rng(seed)
+    nv = 40
+    vx = rng.uniform(-25, 25, nv).astype(np.float32)
+    vy = rng.uniform(-25, 25, nv).astype(np.float32)
+    vx[0] = vy[0] = 0.0
+    vx[1], vy[1] = 1e4, 0.0  # leaves the chip after the first epoch
+    d = _prep(kb, st)
+    sp = kb.SearchParams(sigmag_enable=sig, filter_on=fon, min_lh=min_lh, min_obs=min_obs, K=K, algo=kb.ALGO_DIRECT)
+    r = _search_and_compare(kb, oracle, d, st.times, vx, vy, sp)
+    assert r["n_entries"] > 0
+
+
+def test_search_all_zero_psi(kb, oracle):
+    """All-zero psi gives L' = 0 and flux' = 0 (a legal score, not the sentinel) -- SURVEY 8c pin 2."""
+    import torch
+    T, H, W = 4, 12, 16
+    d = torch.zeros((T, H, W, 2), device="cuda")
+    d[..., 1] = 0.5
+    vx, vy = np.array([0, 1, 2], np.float32), np.array([0, 0, 1], np.float32)
+    sp = kb.SearchParams(K=2, min_lh=-np.inf, algo=kb.ALGO_DIRECT)
+    lh, flux, vel, nobs = [o.cpu().numpy() for o in kb.kbmod_search(d, np.arange(T) * 0.5, vx, vy, sp)]
+    assert np.all(lh == 0) and np.all(flux == 0) and np.all(vel[..., 0] == 0) and np.all(vel[..., 1] == 1)
+
+
+def test_search_empty_velocity_list(kb):
+    import torch
+    d = torch.ones((2, 8, 8, 2), device="cuda")
+    sp = kb.SearchParams(K=3, algo=kb.ALGO_DIRECT)
+    lh, flux, vel, nobs = kb.kbmod_search(d, np.array([0.0, 1.0]), np.zeros(0, np.float32), np.zeros(0, np.float32), sp)
+    assert torch.all(torch.isneginf(lh)) and torch.all(vel == -1) and torch.all(nobs == 0) and torch.all(flux == 0)
+
+
+def test_search_config2_medium(kb, oracle):
+    """BASELINE configs[1] at full size on the GPU (512x512, T=10, 2048 velocities, K=8, 1% mask);
+    the oracle checks 3000 random pixels, the four borders' corners and every injected mover start."""
+    st = synth.config2_medium()
+    vx, vy = synth.config2_grid()
+    d = _prep(kb, st)
+    rng = np.random.default_rng(7)
+    px = rng.integers(0, 512, 3000).astype(np.int32)
+    py = rng.integers(0, 512, 3000).astype(np.int32)
+    mx = np.array([int(m["x0"]) for m in st.movers] + [0, 511, 0, 511], np.int32)
+    my = np.array([int(m["y0"]) for m in st.movers] + [0, 0, 511, 511], np.int32)
+    px, py = np.concatenate([px, mx]), np.concatenate([py, my])
+    sp = kb.SearchParams(K=8, min_obs=5, min_lh=-np.inf, algo=kb.ALGO_DIRECT)
+    r = _search_and_compare(kb, oracle, d, st.times, vx, vy, sp, pixels=(px, py))
+    assert r["n_entries"] == len(px) * 8
+    sp = kb.SearchParams(K=8, min_obs=5, min_lh=10.0, algo=kb.ALGO_DIRECT)
+    _search_and_compare(kb, oracle, d, st.times, vx, vy, sp, pixels=(px, py))
+
+
+# ------------------------------------------------------------------------------------------- lightcurves
+def _random_trajectories(rng, n, H, W, vmax):
+    return (rng.integers(0, W, n).astype(np.int32), rng.integers(0, H, n).astype(np.int32),
+            rng.uniform(-vmax, vmax, n).astype(np.float32), rng.uniform(-vmax, vmax, n).astype(np.float32))
+
+
+@pytest.mark.parametrize("T,fon,min_obs", [(5, 0, 1), (10, 1, 3), (26, 0, 13), (50, 0, 1), (64, 0, 20), (3, 0, 1)])
+def test_eval_trajectories(kb, oracle, T, fon, min_obs):
+    st = synth.random_stack(30 + T, T, 60, 75, mask_frac=0.1, t_span=3.0)
+    d = _prep(kb, st)
+    psiphi = d.cpu().numpy()
+    rng = np.random.default_rng(T)
+    x0, y0, vx, vy = _random_trajectories(rng, 5000, 60, 75, 12.0)
+    sp = kb.SearchParams(filter_on=fon, min_obs=min_obs, K=1)
+    g = {k: v.cpu().numpy() for k, v in
+         kb.kbmod_eval_trajectories(d, st.times, _cuda(x0), _cuda(y0), _cuda(vx), _cuda(vy), sp).items()}
+    o = oracle.eval_trajectories(psiphi, st.times, x0, y0, vx, vy, parity.oracle_params(oracle, sp))
+    assert np.array_equal(g["valid"].view(np.uint64), o["valid"])      # positions + validity: bit-exact
+    assert np.array_equal(g["psi_lc"], o["psi_lc"]) and np.array_equal(g["phi_lc"], o["phi_lc"])
+    assert np.array_equal(g["kept"].view(np.uint64), o["kept"])        # float32 decisions: bit-exact
+    tl, tf = parity.score_tolerances(o, T)
+    has = o["n_kept"] > 0
+    assert has.sum() > 1000
+    assert np.all(np.abs(g["lh"][has] - o["lh"][has]) <= tl[has])
+    assert np.all(np.abs(g["flux"][has] - o["flux"][has]) <= tf[has])
+    assert np.all(np.isneginf(g["lh"][~has])) and np.all(g["flux"][~has] == 0)
+
+
+@pytest.mark.parametrize("T", [4, 9, 26, 50])
+def test_sigmag_filter_with_outliers(kb, oracle, T):
+    """BASELINE configs[4]: rerun sigma-G on lightcurves with 20% of epochs replaced by 10-sigma outliers."""
+    rng = np.random.default_rng(40 + T)
+    n = 20000
+    phi = rng.uniform(0.5, 2.0, (n, T)).astype(np.float32)
+    psi = (rng.standard_normal((n, T)) * np.sqrt(phi)).astype(np.float32)
+    phi[rng.random((n, T)) < 0.1] = 0.0  # invalid epochs
+    psi, hit = synth.outlier_lightcurves(T, psi, phi, 0.2, 10.0)
+    sp = kb.SearchParams(K=1, min_obs=2)
+    g = {k: v.cpu().numpy() for k, v in kb.kbmod_sigmag_filter(_cuda(psi), _cuda(phi), sp).items()}
+    o = oracle.sigmag_filter(psi, phi, parity.oracle_params(oracle, sp))
+    assert np.array_equal(g["kept"].view(np.uint64), o["kept"])
+    has = o["n_kept"] > 0
+    o2 = dict(o, psi_lc=psi, phi_lc=phi)
+    tl, tf = parity.score_tolerances(o2, T)
+    assert np.all(np.abs(g["lh"][has] - o["lh"][has]) <= tl[has])
+    assert np.all(np.abs(g["flux"][has] - o["flux"][has]) <= tf[has])
+
+
+# ------------------------------------------------------------------------------------------- coadd
+@pytest.mark.parametrize("T,radius,use_sel,use_mask", [(5, 10, False, True), (26, 10, True, True), (10, 3, True, False),
+                                                      (50, 15, False, True), (1, 0, False, True), (64, 2, True, True)])
+def test_coadd_stamps(kb, oracle, T, radius, use_sel, use_mask):
+    import torch
+    H, W = 70, 90
+    st = synth.random_stack(50 + T, T, H, W, mask_frac=0.1, t_span=2.0)
+    st.img[0, 5, 5] = np.inf
+    rng = np.random.default_rng(T)
+    n = 300
+    x0, y0, vx, vy = _random_trajectories(rng, n, H, W, 15.0)
+    x0[:4], y0[:4] = [0, W - 1, 0, W - 1], [0, 0, H - 1, H - 1]  # stamps hanging over the corners
+    sel = rng.integers(0, 2 ** min(T, 62), n, dtype=np.int64) if use_sel else None
+    mask = st.mask if use_mask else None
+    gm, gd = kb.kbmod_coadd_stamps(_cuda(st.img), _cuda(mask) if use_mask else None, st.times, _cuda(x0), _cuda(y0),
+                                   _cuda(vx), _cuda(vy), radius, _cuda(sel) if use_sel else None)
+    om, od = oracle.coadd_stamps(st.img, mask, st.times, x0, y0, vx, vy, radius,
+                                 sel.view(np.uint64) if use_sel else None)
+    gm, gd = gm.cpu().numpy(), gd.cpu().numpy()
+    assert np.array_equal(gd, od.astype(np.float32))  # a median is one sample or the mean of two: exact in float32
+    assert np.all(np.abs(gm - om) <= 1e-5 * np.abs(om) + 1e-5)
+
+
+# ------------------------------------------------------------------------------------------- errors
+def test_error_codes(kb):
+    import torch
+    d = torch.zeros((2, 8, 8, 2), device="cuda")
+    t = np.array([0.0, 1.0])
+    v = np.zeros(1, np.float32)
+    with pytest.raises(kb.KbmodError) as e:
+        kb.kbmod_search(d, t, v, v, kb.SearchParams(K=33))
+    assert e.value.code == -2
+    with pytest.raises(kb.KbmodError) as e:
+        kb.kbmod_search(d, t, v, v, kb.SearchParams(K=0))
+    assert e.value.code == -1
+    with pytest.raises(kb.KbmodError) as e:
+        kb.kbmod_search(d, t, v, v, kb.SearchParams(K=1), workspace=torch.empty(256, dtype=torch.uint8, device="cuda")[:0])
+    assert e.value.code in (-1, -3)
+    with pytest.raises(kb.KbmodError) as e:
+        kb.kbmod_prepare_psi_phi(d[..., 0].contiguous(), d[..., 0].contiguous(), None, np.ones((4, 4), np.float32))
+    assert e.value.code == -1
+    with pytest.raises(TypeError):
+        kb.kbmod_search(d.cpu(), t, v, v, kb.SearchParams(K=1))  # no CPU fallback
