@@ -1,0 +1,375 @@
+#!/usr/bin/env python3
+"""bench.py -- trajectory-epoch evaluations per second of the whole hot path on synthetic DECam-shaped
+stacks (BASELINE.json `metric`), one JSON line on stdout (rank 0).
+
+A "step" is one pass of every SURVEY.md section-8(a) row over one stack: kbmod_prepare_psi_phi (a1),
+kbmod_search = displacement table + gather + in-line sigma-G + per-pixel top-K (a2-a5), and
+kbmod_coadd_stamps on a candidate list (a6).  N = 1 runs BASELINE configs[2] (2048x4096x26, 128x64
+velocities, K=8, sigma-G on, min_lh = 10 = the paper's operating point).  N > 1: one
+independent CCD stack per rank (replicas: 2580 independent per-CCD searches),
+no data-path collective, "scaling": "weak".
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload c3|c2|c1|c4]
+                  [--min-lh X] [--algo auto|direct|pruned]
+`--impl reference` times the oracle (oracle/, plain C, double) on the host cores on a bounded sample
+of the same workload; it is the only leg besides `cpu_baseline` that executes anything under oracle/.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import math
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+from paper_2109_03296_b200 import synth  # noqa: E402  (input generators only: no method arithmetic)
+
+METRIC = "trajectory_epoch_evals_per_s"
+UNIT = "evals/s"
+
+
+def load_peaks():
+    """Measured peaks written by the driver; else the fallback B200_PROFILING.md states."""
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return dict(hbm_gbs=float(d["hbm_gbs"]), sm_max_mhz=float(d.get("sm_max_mhz", 1965.0)), source="measured")
+    return dict(hbm_gbs=6650.0, sm_max_mhz=1965.0, source="fallback")
+
+
+def make_workload(name: str, seed_shift: int = 0):
+    """Returns (stack, vx, vy, params-dict, description).  Recipes: DESIGN.md 'synthetic inputs'."""
+    if name == "c3":
+        st = synth.config3_decam(seed=2 + seed_shift)
+        vx, vy = synth.config3_grid()
+        return st, vx, vy, dict(K=8, min_obs=13), "configs[2] DECam-shaped 2048x4096x26, 128x64 velocities, K=8"
+    if name == "c4":
+        st = synth.config4_heavy(seed=3 + seed_shift)
+        vx, vy = synth.config4_grid()
+        return st, vx, vy, dict(K=16, min_obs=25), "configs[3] heavy 2048x4096x50, 256x128 velocities, K=16"
+    if name == "c2":
+        st = synth.config2_medium(seed=1 + seed_shift)
+        vx, vy = synth.config2_grid()
+        return st, vx, vy, dict(K=8, min_obs=5), "configs[1] 512x512x10, 64x32 velocities, K=8"
+    if name == "c1":
+        st = synth.config1_tiny(seed=0 + seed_shift)
+        vx, vy = synth.config1_grid()
+        return st, vx, vy, dict(K=1, min_obs=3), "configs[0] tiny 64x64x5, 16x16 velocities, K=1"
+    raise SystemExit(f"unknown workload {name}")
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md recipe)."""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.proc, self.lines = index, None, []
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                          "-lms", "100", "-i", str(self.index)], stdout=subprocess.PIPE, text=True)
+            threading.Thread(target=lambda: self.lines.extend(self.proc.stdout), daemon=True).start()
+        except OSError:
+            self.proc = None
+
+    def stop(self):
+        if self.proc is None:
+            return dict(sm_mhz=None, sm_max_mhz=None, reasons=["nvidia-smi unavailable"])
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+        sm, mx, reasons = [], [], set()
+        for ln in self.lines:
+            f = [x.strip() for x in ln.split(",")]
+            if len(f) < 9:
+                continue
+            try:
+                sm.append(float(f[1])); mx.append(float(f[2]))
+            except ValueError:
+                continue
+            for name, val in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), f[5:9]):
+                if val.lower().startswith("active"):
+                    reasons.add(name)
+        busy = [s for s in sm if s > 0]
+        return dict(sm_mhz=float(np.median(busy)) if busy else None, sm_max_mhz=max(mx) if mx else None,
+                    reasons=sorted(reasons), samples=len(sm))
+
+
+# ----------------------------------------------------------------------------------------- oracle legs
+class OracleSample:
+    """The oracle (as it stands) on a bounded sample of the workload.  O1 runs once on a crop tall
+    enough that most displaced epochs stay on it (real values: movers, masks, artefacts); what is
+    timed is the search (O2-O6) on random start pixels of that crop, where the time goes."""
+
+    def __init__(self, st, vx, vy, pd, min_lh):
+        from oracle import oracle as O
+        self.O, self.vx, self.vy, self.times = O, vx, vy, st.times
+        T, H, W = st.img.shape
+        self.T, self.ch, self.cw = T, min(H, 2048), min(W, 1024)
+        ch, cw = self.ch, self.cw
+        t0 = time.time()
+        psi, phi, _, _ = O.prepare_psi_phi(st.img[:, :ch, :cw], st.var[:, :ch, :cw], st.mask[:, :ch, :cw], st.psf)
+        self.t_prep = time.time() - t0
+        self.psiphi = O.interleave(psi, phi)
+        self.p = O.Params(K=pd["K"], min_obs=pd["min_obs"], min_lh=min_lh)
+        self.rng = np.random.default_rng(123)
+        self.rate = None
+
+    def _run(self, n):
+        px = self.rng.integers(0, self.cw, n).astype(np.int32)
+        py = self.rng.integers(0, self.ch, n).astype(np.int32)
+        t0 = time.time()
+        self.O.search_pixels(self.psiphi, self.times, self.vx, self.vy, px, py, self.p)
+        return max(time.time() - t0, 1e-6)
+
+    def step(self, target_s):
+        """One bounded sample of about target_s seconds.  Returns (evals/s, cores, description, seconds)."""
+        if self.rate is None:
+            self.rate = 256 / self._run(256)  # pixels per second, probe
+        n = int(min(max(256, self.rate * target_s), self.ch * self.cw))
+        dt = self._run(n)
+        self.rate = n / dt
+        evals = float(n) * len(self.vx) * self.T
+        desc = (f"oracle search (O2-O6) on {n} random start pixels of a {self.cw}x{self.ch} crop x all {len(self.vx)} "
+                f"velocities x {self.T} epochs = {evals:.3g} evals in {dt:.1f} s (O1 on the crop, {self.t_prep:.1f} s, "
+                f"not counted)")
+        return evals / dt, self.O.num_threads(), desc, dt
+
+
+def run_reference(args):
+    """--impl reference: the oracle, as it stands, on the host cores; rank 0 only."""
+    if int(os.environ.get("RANK", "0")) != 0:
+        return
+    peaks = load_peaks()
+    st, vx, vy, pd, desc = make_workload(args.workload)
+    T, H, W = st.img.shape
+    per_step = max(2.0, min(20.0, 150.0 / max(1, args.steps + args.warmup)))
+    rates, times_s = [], []
+    cores, sample = 0, ""
+    smp = OracleSample(st, vx, vy, pd, args.min_lh)
+    for i in range(args.warmup + args.steps):
+        r, cores, sample, dt = smp.step(per_step)
+        if i >= args.warmup:
+            rates.append(r); times_s.append(dt)
+    value = float(np.mean(rates))
+    line = dict(impl="reference", metric=METRIC, value=value, unit=UNIT, n_gpus=args.gpus, steps=args.steps,
+                warmup=args.warmup, ms_per_step=1e3 * float(np.mean(times_s)), higher_is_better=True, scaling="weak",
+                vs_baseline=None, dtype="f64", data="synthetic",
+                config=dict(workload=desc, min_lh=args.min_lh, sigma_g="on", note="each step = a bounded sample"),
+                cpu_baseline=dict(value=value, unit=UNIT, cores=cores, kind="oracle", sample=sample),
+                e2e=dict(value=value, unit=UNIT, h2d_bytes_per_step=0, d2h_bytes_per_step=0), gpu_launches=0,
+                peaks_source=peaks["source"])
+    print(json.dumps(line), flush=True)
+
+
+# ----------------------------------------------------------------------------------------- GPU arm
+# Algorithmic work per unit for the roofline.
+#   direct kernel  : bound "alu" -- every trajectory runs the compare-exchange network; the algorithmic
+#                    lane-operations per trajectory are 2*CE(T) min/max + per epoch 1 gather, 1 divide,
+#                    2 window compares, 2 adds, 1 count = 2*CE(T) + 7*T; peak = 148 SMs x 128 lanes x f_max.
+#   pruned kernel  : bound "smem" -- 8 B (one float2 of the bound planes) per trajectory-epoch evaluation
+#                    read from shared memory; peak = 148 SMs x 128 B/clk x f_max.
+CE_COUNT = {4: 5, 5: 9, 8: 19, 10: 32, 12: 42, 16: 63, 20: 103, 24: 132, 26: 147, 28: 162, 32: 191, 40: 305,
+            48: 384, 50: 403, 56: 464, 64: 543}
+N_SM = 148
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    import paper_2109_03296_b200 as kb
+
+    rank, world = int(os.environ.get("RANK", "0")), int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    kb.binding.lib()
+    peaks = load_peaks()
+    dev = torch.device("cuda", local)
+
+    st, vx, vy, pd, desc = make_workload(args.workload, seed_shift=100 * rank)  # one CCD stack per rank
+    T, H, W = st.img.shape
+    algo = dict(auto=kb.ALGO_AUTO, direct=kb.ALGO_DIRECT, pruned=kb.ALGO_PRUNED)[args.algo]
+    sp = kb.SearchParams(K=pd["K"], min_obs=pd["min_obs"], min_lh=args.min_lh, algo=algo)
+    n_vel = len(vx)
+    evals = float(H) * W * n_vel * T
+
+    # inputs resident in HBM before the timed region
+    img, var, mask = (torch.from_numpy(a).to(dev) for a in (st.img, st.var, st.mask))
+    psiphi = torch.empty((T, H, W, 2), dtype=torch.float32, device=dev)
+    out = tuple(torch.empty((H, W, sp.K), dtype=dt, device=dev)
+                for dt in (torch.float32, torch.float32, torch.int32, torch.int32))
+    ws = torch.empty(max(256, kb.kbmod_search_workspace_bytes(T, H, W, n_vel, sp)), dtype=torch.uint8, device=dev)
+    n_cand = min(100_000, H * W)  # (a6) candidate list: configs[4]'s recipe
+    cx0, cy0, cvx, cvy = (torch.from_numpy(a).to(dev) for a in synth.config5_trajectories(4 + rank, H, W, n_cand))
+
+    ev = lambda: torch.cuda.Event(enable_timing=True)
+    seg = {"prep": [], "search": [], "coadd": []}
+
+    def step(record):
+        e = [ev() for _ in range(4)]
+        e[0].record()
+        kb.kbmod_prepare_psi_phi(img, var, mask, st.psf, out=psiphi)
+        e[1].record()
+        kb.kbmod_search(psiphi, st.times, vx, vy, sp, out=out, workspace=ws)
+        e[2].record()
+        kb.kbmod_coadd_stamps(img, mask, st.times, cx0, cy0, cvx, cvy, 10)
+        e[3].record()
+        if record:
+            record.append(e)
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(args.warmup):
+        step(None)
+    barrier()
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    recs = []
+    t_beg, t_end = ev(), ev()
+    t_beg.record()
+    for _ in range(args.steps):
+        step(recs)
+    t_end.record()
+    barrier()
+    clocks = sampler.stop() if rank == 0 else None
+    total_ms = t_beg.elapsed_time(t_end)
+    for e in recs:
+        seg["prep"].append(e[0].elapsed_time(e[1])); seg["search"].append(e[1].elapsed_time(e[2]))
+        seg["coadd"].append(e[2].elapsed_time(e[3]))
+    stats = kb.kbmod_search_stats(ws)  # [evaluated, nominal, launches, algo]
+    return dict(torch=torch, dist=dist, kb=kb, rank=rank, world=world, dev=dev, st=st, vx=vx, vy=vy, pd=pd, sp=sp,
+                desc=desc, evals=evals, total_ms=total_ms, seg=seg, stats=stats, clocks=clocks, peaks=peaks,
+                n_cand=n_cand, out=out)
+
+
+def run_e2e(R, steps):
+    """Same metric end to end through the C-ABI call with HOST buffers (kbmod_pipeline_host): every step
+    copies the image/variance/mask stacks from pinned host memory, runs prep + search, and reads the four
+    result arrays back.  Timed on the device with events around the call (the call itself synchronises)."""
+    torch, kb, st, sp = R["torch"], R["kb"], R["st"], R["sp"]
+    T, H, W = st.img.shape
+    h_in = [torch.from_numpy(a).pin_memory() for a in (st.img, st.var, st.mask)]
+    h_out = [torch.empty((H, W, sp.K), dtype=dt).pin_memory()
+             for dt in (torch.float32, torch.float32, torch.int32, torch.int32)]
+    arena = torch.empty(kb.kbmod_pipeline_host_arena_bytes(T, H, W, len(R["vx"]), sp), dtype=torch.uint8, device=R["dev"])
+    h2d = sum(a.numel() * a.element_size() for a in h_in)
+    d2h = sum(a.numel() * a.element_size() for a in h_out)
+    kb.kbmod_pipeline_host(*h_in, st.psf, st.times, R["vx"], R["vy"], sp, h_out, arena)  # warm-up
+    b, e = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    b.record()
+    for _ in range(steps):
+        kb.kbmod_pipeline_host(*h_in, st.psf, st.times, R["vx"], R["vy"], sp, h_out, arena)
+    e.record()
+    torch.cuda.synchronize()
+    ms = b.elapsed_time(e) / steps
+    # the host result must be the device result of the resident-input run (same inputs)
+    same = bool(torch.equal(h_out[2], R["out"][2].cpu()))
+    del arena
+    return ms, h2d, d2h, same
+
+
+def report(R, args):
+    torch, dist, kb = R["torch"], R["dist"], R["kb"]
+    rank, world = R["rank"], R["world"]
+    # max over ranks of the device time of the timed region
+    tmax = torch.tensor([R["total_ms"]], dtype=torch.float64, device=R["dev"])
+    if world > 1:
+        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
+    total_ms = float(tmax.item())
+    e2e_steps = max(1, min(args.steps, 3))
+    e2e_ms, h2d, d2h, same = run_e2e(R, e2e_steps)
+    emax = torch.tensor([e2e_ms], dtype=torch.float64, device=R["dev"])
+    if world > 1:
+        dist.all_reduce(emax, op=dist.ReduceOp.MAX)
+    if rank != 0:
+        return
+    ms_per_step = total_ms / args.steps
+    value = world * R["evals"] / (ms_per_step * 1e-3)
+    st, sp, peaks = R["st"], R["sp"], R["peaks"]
+    T, H, W = st.img.shape
+    n_vel = len(R["vx"])
+    search_ms = float(np.mean(R["seg"]["search"]))
+    evaluated, nominal, launches, algo_used = R["stats"]
+    f_max = peaks["sm_max_mhz"] * 1e6
+    tp = min(k for k in CE_COUNT if k >= T)
+    if algo_used == kb.ALGO_DIRECT:
+        ops = float(H) * W * n_vel * (2 * CE_COUNT[tp] + 7 * T)
+        roof = dict(bound="alu", achieved=ops / (search_ms * 1e-3) / 1e12, peak=N_SM * 128 * f_max / 1e12,
+                    unit="Tlane-op/s", kernel="search_direct_kernel",
+                    peak_source="derived: 148 SMs x 128 FP32/ALU lanes x sm_max_mhz (DESIGN.md)")
+    else:
+        byts = R["evals"] * 8.0
+        roof = dict(bound="smem", achieved=byts / (search_ms * 1e-3) / 1e9, peak=N_SM * 128 * f_max / 1e9,
+                    unit="GB/s", kernel="search_pruned_kernel",
+                    peak_source="derived: 148 SMs x 128 B/clk shared-memory bandwidth x sm_max_mhz (DESIGN.md)")
+    roof["frac"] = roof["achieved"] / roof["peak"]
+    roof["traffic"] = None
+    roof["kernel_ms"] = search_ms
+    cpu = None
+    if not args.no_cpu_baseline:
+        smp = OracleSample(st, R["vx"], R["vy"], R["pd"], args.min_lh)
+        r, cores, sample, _ = smp.step(12.0)
+        cpu = dict(value=r, unit=UNIT, cores=cores, kind="oracle", sample=sample)
+    line = dict(metric=METRIC, value=value, unit=UNIT, n_gpus=world, steps=args.steps, warmup=args.warmup,
+                ms_per_step=ms_per_step, higher_is_better=True, scaling="weak", vs_baseline=None, dtype="f32",
+                data="synthetic",
+                config=dict(workload=R["desc"], min_lh=args.min_lh, min_obs=sp.min_obs, sigma_g="on",
+                            algo={1: "direct", 2: "pruned"}.get(algo_used, "?"), coadd_candidates=R["n_cand"],
+                            l2="inputs larger than L2 (psi/phi stack %.2f GB)" % (T * H * W * 8 / 1e9),
+                            multi_gpu="one independent CCD stack per rank, no collective" if world > 1 else "single GPU"),
+                segments_ms={k: float(np.mean(v)) for k, v in R["seg"].items()},
+                evaluated_fraction=evaluated / max(1, nominal),
+                roofline=roof, cpu_baseline=cpu,
+                e2e=dict(value=world * R["evals"] / (float(emax.item()) * 1e-3), unit=UNIT, h2d_bytes_per_step=h2d,
+                         d2h_bytes_per_step=d2h, ms_per_step=float(emax.item()), steps=e2e_steps,
+                         matches_resident_run=same, api="kbmod_pipeline_host (prep + search; host buffers pinned)"),
+                gpu_launches=args.steps * (T + int(launches) + 1), clocks=R["clocks"], peaks_source=peaks["source"])
+    print(json.dumps(line), flush=True)
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=3)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="c3", choices=["c1", "c2", "c3", "c4"])
+    ap.add_argument("--min-lh", type=float, default=10.0, dest="min_lh")
+    ap.add_argument("--algo", default="auto", choices=["auto", "direct", "pruned"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+        return
+    R = run_ours(args)
+    report(R, args)
+    if R["world"] > 1:
+        R["dist"].destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -9,7 +9,7 @@
 namespace {
 
 template <int TP>
-__global__ void coadd_kernel(const float* __restrict__ img, const uint8_t* __restrict__ mask, int T, int H, int W,
+__global__ void __launch_bounds__(448) coadd_kernel(const float* __restrict__ img, const uint8_t* __restrict__ mask, int T, int H, int W,
                              const __grid_constant__ DevTimes times, const int32_t* __restrict__ x0s,
                              const int32_t* __restrict__ y0s, const float* __restrict__ vxs,
                              const float* __restrict__ vys, const unsigned long long* __restrict__ epoch_mask,
@@ -23,11 +23,10 @@ __global__ void coadd_kernel(const float* __restrict__ img, const uint8_t* __res
         sdy[threadIdx.x] = kb_displacement(vys[i], times.dt[threadIdx.x]);
     }
     __syncthreads();
-    const int p = threadIdx.x;
-    if (p >= S * S) return;
-    const int v = p / S - radius, u = p % S - radius;
     const unsigned long long sel = epoch_mask ? epoch_mask[i] : ~0ull;
     const size_t plane = (size_t)H * W;
+    for (int p = threadIdx.x; p < S * S; p += blockDim.x) {
+    const int v = p / S - radius, u = p % S - radius;
 
     float vals[TP];
     float sum = 0.0f;
@@ -74,6 +73,7 @@ __global__ void coadd_kernel(const float* __restrict__ img, const uint8_t* __res
     const size_t o = (size_t)i * S * S + p;
     if (mean_out) mean_out[o] = mean;
     if (median_out) median_out[o] = med;
+    }
 }
 
 }  // namespace
@@ -83,8 +83,9 @@ int kb_launch_coadd(const float* d_img, const uint8_t* d_mask, int T, int TPv, i
                     const unsigned long long* d_epoch_mask, int n_traj, int radius, float* d_mean, float* d_median,
                     cudaStream_t st) {
     const int S = 2 * radius + 1;
-    int threads = ((S * S + 31) / 32) * 32;
-    if (threads < 64) threads = 64;  // the first T threads compute the displacements
+    int threads = ((S * S + 31) / 32) * 32;  // one stamp pixel per thread up to 21x21, a loop above that
+    if (threads < 64) threads = 64;          // the first T threads compute the displacements
+    if (threads > 448) threads = 256;
     KB_DISPATCH_TP(TPv, {
         coadd_kernel<TP><<<n_traj, threads, 0, st>>>(d_img, d_mask, T, H, W, times, d_x0, d_y0, d_vx, d_vy,
                                                         d_epoch_mask, radius, d_mean, d_median);
