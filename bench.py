@@ -232,7 +232,7 @@ def run_ours(args):
         e[2].record()
         kb.kbmod_coadd_stamps(img, mask, st.times, cx0, cy0, cvx, cvy, 10)
         e[3].record()
-        if record:
+        if record is not None:
             record.append(e)
 
     def barrier():

@@ -131,13 +131,12 @@ extern "C" int kbmod_prepare_psi_phi(const float* d_img, const float* d_var, con
 // workspace layout of kbmod_search (all offsets 256-byte aligned)
 struct SearchPlan {
     int TP;
-    size_t off_stats, off_tab, total;
+    size_t off_stats, off_tab, off_pruned, pruned_bytes, total;
 };
 
 static size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
 
 static int plan_search(int T, int H, int W, int n_vel, const kbmod_search_params* p, SearchPlan* pl) {
-    (void)H; (void)W; (void)p;
     pl->TP = kb_padded_T(T);
     KB_REQUIRE(pl->TP > 0, KBMOD_ERR_UNSUPPORTED, "T = %d unsupported", T);
     size_t o = 0;
@@ -145,6 +144,11 @@ static int plan_search(int T, int H, int W, int n_vel, const kbmod_search_params
     o = align256(o + 8 * sizeof(unsigned long long));
     pl->off_tab = o;
     o = align256(o + (size_t)n_vel * pl->TP * sizeof(DispEntry));
+    pl->off_pruned = o;
+    // the pruned path's bound planes and key lists; not needed when the caller forces the direct kernel
+    const int K = (p->K >= 1 && p->K <= KBMOD_MAX_K) ? p->K : 1;
+    pl->pruned_bytes = (p->algo == KBMOD_ALGO_DIRECT) ? 0 : kb_pruned_workspace_bytes(T, H, W, n_vel, K);
+    o = align256(o + pl->pruned_bytes);
     pl->total = o;
     return KBMOD_OK;
 }
@@ -182,13 +186,17 @@ extern "C" int kbmod_search(const float* d_psiphi, int T, int H, int W, const do
     const int TP = pl.TP;
     const size_t plane = (size_t)H * W;
     std::vector<DispEntry> tab((size_t)n_vel * TP);
+    std::vector<int32_t> hdx((size_t)n_vel * T), hdy((size_t)n_vel * T);
+    KB_REQUIRE(W <= 32767 && H <= 32767, KBMOD_ERR_UNSUPPORTED, "W, H = %d, %d exceed 32767", W, H);
     for (int v = 0; v < n_vel; ++v)
         for (int t = 0; t < TP; ++t) {
             DispEntry e;
             if (t < T) {
                 const double dt = h_times[t] - h_times[0];
                 const int32_t dx = displacement(h_vx[v], dt), dy = displacement(h_vy[v], dt);
-                // |d| beyond the image size can never land on-image: clamp so it fits int16 / int32
+                hdx[(size_t)v * T + t] = dx;
+                hdy[(size_t)v * T + t] = dy;
+                // |d| beyond the image size can never land on-image: flag it so the entry fits int16 / int32
                 const bool off_image = dx <= -W || dx >= W || dy <= -H || dy >= H;
                 e.dx = off_image ? (int16_t)-32768 : (int16_t)dx;
                 e.dy = off_image ? (int16_t)0 : (int16_t)dy;
@@ -200,16 +208,37 @@ extern "C" int kbmod_search(const float* d_psiphi, int T, int H, int W, const do
             }
             tab[(size_t)v * TP + t] = e;
         }
-    KB_REQUIRE(W <= 32767 && H <= 32767, KBMOD_ERR_UNSUPPORTED, "W, H = %d, %d exceed 32767", W, H);
-    unsigned long long stats[8] = {(unsigned long long)plane * n_vel, (unsigned long long)plane * n_vel, 1,
-                                   KBMOD_ALGO_DIRECT, 0, 0, 0, 0};
+
+    // which kernel: the pruned one needs a finite threshold to prune against and a velocity list whose
+    // groups can be staged
+    int algo = p->algo;
+    if (algo != KBMOD_ALGO_DIRECT && n_vel > 0) {
+        double ps[2] = {0, 0};
+        rc = kb_launch_search_pruned(nullptr, T, TP, H, W, nullptr, hdx.data(), hdy.data(), n_vel, p, P, nullptr, nullptr,
+                                     nullptr, nullptr, nullptr, 0, nullptr, st, /*plan_only=*/1, ps, nullptr);
+        if (algo == KBMOD_ALGO_AUTO) {
+            const bool ok = rc == KBMOD_OK && isfinite(p->min_lh) && p->min_lh >= 3.0f && ps[0] <= 0.10 && ps[1] <= 4.0;
+            algo = ok ? KBMOD_ALGO_PRUNED : KBMOD_ALGO_DIRECT;
+        } else if (rc) {
+            return rc;
+        }
+    } else {
+        algo = KBMOD_ALGO_DIRECT;
+    }
+    unsigned long long stats[8] = {0, (unsigned long long)plane * n_vel, 1, (unsigned long long)algo, 0, 0, 0, 0};
+    if (algo == KBMOD_ALGO_DIRECT) stats[0] = stats[1];
+    else stats[2] = 3;
     // pageable source: cudaMemcpyAsync stages it before returning, so the vectors may go out of scope
     KB_CUDA(cudaMemcpyAsync(ws + pl.off_stats, stats, sizeof(stats), cudaMemcpyHostToDevice, st));
     if (n_vel > 0)
         KB_CUDA(cudaMemcpyAsync(ws + pl.off_tab, tab.data(), tab.size() * sizeof(DispEntry), cudaMemcpyHostToDevice,
                                 st));
-    return kb_launch_search_direct(d_psiphi, T, TP, H, W, (const DispEntry*)(ws + pl.off_tab), n_vel, P, d_lh, d_flux,
-                                   d_vel_idx, d_n_obs, st);
+    const DispEntry* d_tab = (const DispEntry*)(ws + pl.off_tab);
+    if (algo == KBMOD_ALGO_DIRECT)
+        return kb_launch_search_direct(d_psiphi, T, TP, H, W, d_tab, n_vel, P, d_lh, d_flux, d_vel_idx, d_n_obs, st);
+    return kb_launch_search_pruned(d_psiphi, T, TP, H, W, d_tab, hdx.data(), hdy.data(), n_vel, p, P, d_lh, d_flux,
+                                   d_vel_idx, d_n_obs, ws + pl.off_pruned, pl.pruned_bytes,
+                                   (unsigned long long*)(ws + pl.off_stats), st, 0, nullptr, nullptr);
 }
 
 extern "C" int kbmod_search_stats(const void* d_workspace, unsigned long long* h_out) {

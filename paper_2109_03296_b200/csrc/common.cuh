@@ -161,3 +161,12 @@ int kb_launch_coadd(const float* d_img, const uint8_t* d_mask, int T, int TP, in
                     const int32_t* d_x0, const int32_t* d_y0, const float* d_vx, const float* d_vy,
                     const unsigned long long* d_epoch_mask, int n_traj, int radius, float* d_mean, float* d_median,
                     cudaStream_t st);
+
+// pruned search (search_pruned.cu).  h_dx, h_dy: [n_vel][T] displacement table (a2).  plan_only: run the host
+// planner only and fill plan_stats = {fraction of velocity groups that cannot be staged, staged bytes per evaluation}.
+size_t kb_pruned_workspace_bytes(int T, int H, int W, int n_vel, int K);
+int kb_launch_search_pruned(const float* d_psiphi, int T, int TP, int H, int W, const DispEntry* d_tab,
+                            const int32_t* h_dx, const int32_t* h_dy, int n_vel, const kbmod_search_params* p,
+                            const DevParams& P, float* d_lh, float* d_flux, int32_t* d_vel, int32_t* d_nobs,
+                            void* d_ws, size_t ws_bytes, unsigned long long* d_stats, cudaStream_t st, int plan_only,
+                            double* plan_stats, int* n_launches);

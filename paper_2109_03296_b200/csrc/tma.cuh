@@ -1,0 +1,52 @@
+// Minimal inline-PTX wrappers for the sm_100a asynchronous-copy machinery the pruned search uses:
+// mbarrier (init / expect_tx / try_wait.parity), the 3-D TMA tile load (cp.async.bulk.tensor ->
+// SASS UTMALDG) and the generic->async proxy fence.  Host side: cuTensorMapEncodeTiled resolved at
+// run time through cudaGetDriverEntryPoint (no link-time dependency on libcuda).
+#pragma once
+#include <cuda.h>
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+__device__ __forceinline__ uint32_t kb_smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void kb_mbar_init(uint64_t* bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(kb_smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void kb_fence_barrier_init() {
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+}
+__device__ __forceinline__ void kb_mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(kb_smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void kb_mbar_wait(uint64_t* bar, uint32_t parity) {
+    asm volatile(
+        "{\n\t"
+        ".reg .pred p;\n\t"
+        "KB_WAIT_%=:\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
+        "@p bra KB_DONE_%=;\n\t"
+        "bra KB_WAIT_%=;\n\t"
+        "KB_DONE_%=:\n\t"
+        "}" ::"r"(kb_smem_u32(bar)), "r"(parity) : "memory");
+}
+// generic-proxy writes to shared memory (st.shared) must be ordered before async-proxy (TMA) writes
+__device__ __forceinline__ void kb_fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+
+// 3-D tile load: box (boxDim of the map) at element coordinates (x, y, z) -> dense smem block; signed
+// coordinates; out-of-bounds elements are zero-filled (this IS the off-image rule of the search).
+__device__ __forceinline__ void kb_tma_load_3d(void* smem_dst, const CUtensorMap* map, int x, int y, int z,
+                                               uint64_t* bar) {
+    asm volatile(
+        "cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];"
+        ::"r"(kb_smem_u32(smem_dst)), "l"(map), "r"(x), "r"(y), "r"(z), "r"(kb_smem_u32(bar))
+        : "memory");
+}
+__device__ __forceinline__ void kb_prefetch_tensormap(const CUtensorMap* map) {
+    asm volatile("prefetch.tensormap [%0];" ::"l"(map) : "memory");
+}
+
+// host: driver entry point for cuTensorMapEncodeTiled
+typedef CUresult (*kb_encode_tiled_fn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                       const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                       CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+kb_encode_tiled_fn kb_get_encode_tiled();

@@ -250,3 +250,83 @@ def test_error_codes(kb):
     assert e.value.code == -1
     with pytest.raises(TypeError):
         kb.kbmod_search(d.cpu(), t, v, v, kb.SearchParams(K=1))  # no CPU fallback
+
+
+# ------------------------------------------------------------------------------------------- pruned search
+@pytest.mark.parametrize("seed,T,H,W,K,sig,fon,min_lh,min_obs", [
+    (61, 7, 45, 70, 4, 1, 0, 2.0, 1),
+    (62, 10, 33, 137, 8, 1, 1, 1.0, 4),
+    (63, 5, 20, 100, 3, 0, 0, 2.5, 2),
+    (64, 26, 50, 90, 8, 1, 0, 3.0, 13),
+    (65, 50, 40, 70, 16, 1, 0, 3.5, 25),
+    (66, 64, 17, 65, 2, 1, 0, 4.0, 1),
+    (67, 3, 16, 64, 32, 1, 0, -1.0, 1),
+])
+def test_search_pruned_random(kb, oracle, seed, T, H, W, K, sig, fon, min_lh, min_obs):
+    """The pruned kernel (TMA-staged bound + exact re-evaluation) against the oracle, every pixel; low
+    thresholds so that a large share of the trajectories goes through both phases."""
+    st = synth.random_stack(seed, T, H, W, mask_frac=0.06, t_span=1.5)
+    rng = np.random.default_rng(seed)
+    nv = 70  # not a multiple of the group size
+    vx = rng.uniform(-25, 25, nv).astype(np.float32)
+    vy = rng.uniform(-25, 25, nv).astype(np.float32)
+    vx[0] = vy[0] = 0.0
+    vx[1], vy[1] = 1e4, 0.0    # leaves the chip after the first epoch: its group cannot be staged
+    vx[2], vy[2] = 3e9, -3e9   # displacement beyond int32
+    d = _prep(kb, st)
+    sp = kb.SearchParams(sigmag_enable=sig, filter_on=fon, min_lh=min_lh, min_obs=min_obs, K=K, algo=kb.ALGO_PRUNED)
+    r = _search_and_compare(kb, oracle, d, st.times, vx, vy, sp)
+    assert r["n_entries"] > 0
+    ws = kb.kbmod_search.last_workspace
+    ev, nominal, launches, algo = kb.kbmod_search_stats(ws)
+    assert algo == kb.ALGO_PRUNED and nominal == H * W * nv and 0 < ev <= nominal
+
+
+def test_search_pruned_config1(kb, oracle):
+    st = synth.config1_tiny()
+    vx, vy = synth.config1_grid()
+    d = _prep(kb, st)
+    sp = kb.SearchParams(K=1, min_obs=3, min_lh=10.0, algo=kb.ALGO_PRUNED)
+    r = _search_and_compare(kb, oracle, d, st.times, vx, vy, sp)
+    assert r["n_entries"] > 50
+
+
+def test_search_pruned_equals_direct_decam_shaped(kb):
+    """Property that holds at any size: both kernels return identical arrays (same evaluation function,
+    order-independent top-K).  DECam-shaped stack scaled to 1024x600 with artefacts, masks and movers."""
+    import torch
+    st = synth.decam_stack(5, (7, 6, 7, 6), H=1024, W=600, n_movers=40, n_stars=60)
+    vx, vy = synth.config3_grid(32, 16)
+    d = _prep(kb, st)
+    outs = {}
+    for name, algo in (("direct", kb.ALGO_DIRECT), ("pruned", kb.ALGO_PRUNED)):
+        sp = kb.SearchParams(K=8, min_obs=13, min_lh=10.0, algo=algo)
+        outs[name] = [o.clone() for o in kb.kbmod_search(d, st.times, vx, vy, sp)]
+    ev, nominal, _, algo = kb.kbmod_search_stats(kb.kbmod_search.last_workspace)
+    assert algo == kb.ALGO_PRUNED and ev < 0.05 * nominal, (ev, nominal)
+    for a, b in zip(outs["direct"], outs["pruned"]):
+        assert torch.equal(a, b)
+    assert int((outs["pruned"][2] >= 0).sum()) > 100  # the movers are found
+
+
+def test_search_config3_full_size_sampled(kb, oracle):
+    """BASELINE configs[2] at full size in the launch configuration bench.py times (AUTO -> pruned,
+    min_lh = 10, K = 8): oracle on random pixels, windows on injected movers, and the borders."""
+    st = synth.config3_decam()
+    vx, vy = synth.config3_grid()
+    d = _prep(kb, st)
+    T, H, W = st.img.shape
+    rng = np.random.default_rng(3)
+    px = [rng.integers(0, W, 6000), np.array([0, W - 1, 0, W - 1, 5, W - 6]), rng.integers(0, W, 500), np.zeros(250), np.full(250, W - 1)]
+    py = [rng.integers(0, H, 6000), np.array([0, 0, H - 1, H - 1, 7, H - 8]), np.concatenate([np.zeros(250), np.full(250, H - 1)]),
+          rng.integers(0, H, 250), rng.integers(0, H, 250)]
+    for m in st.movers[:60]:  # 5x5 windows on mover starts: where results actually are
+        wy, wx = np.mgrid[-2:3, -2:3]
+        px.append(np.clip(int(m["x0"]) + wx.reshape(-1), 0, W - 1))
+        py.append(np.clip(int(m["y0"]) + wy.reshape(-1), 0, H - 1))
+    px, py = np.concatenate(px).astype(np.int32), np.concatenate(py).astype(np.int32)
+    sp = kb.SearchParams(K=8, min_obs=13, min_lh=10.0, algo=kb.ALGO_AUTO)
+    r = _search_and_compare(kb, oracle, d, st.times, vx, vy, sp, pixels=(px, py))
+    ev, nominal, _, algo = kb.kbmod_search_stats(kb.kbmod_search.last_workspace)
+    assert algo == kb.ALGO_PRUNED and nominal == H * W * len(vx)
+    assert r["n_entries"] > 500, r
