@@ -412,6 +412,9 @@ int kb_launch_search_pruned(const float* d_psiphi, int T, int TPv, int H, int W,
                 const int dx = h_dx[(size_t)v * T + t], dy = h_dy[(size_t)v * T + t];
                 x0 = std::min(x0, dx); x1 = std::max(x1, dx); y0 = std::min(y0, dy); y1 = std::max(y1, dy);
             }
+            // TMA: the box must start on a 16-byte boundary, i.e. at an even x for 8-byte elements (an odd
+            // start raises an illegal-instruction fault on sm_100a); tile origins are multiples of 64
+            x0 -= (x0 & 1);
             const long long bw = (long long)x1 - x0 + PR_TW, bh = (long long)y1 - y0 + PR_TH;
             const long long pk = (bw - PR_TW + 15) / 16, nb = (bh + PR_RB - 1) / PR_RB;
             const long long bytes = (PR_TW + 16 * pk) * PR_RB * nb * 8;

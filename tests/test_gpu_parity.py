@@ -296,7 +296,7 @@ def test_search_pruned_equals_direct_decam_shaped(kb):
     order-independent top-K).  DECam-shaped stack scaled to 1024x600 with artefacts, masks and movers."""
     import torch
     st = synth.decam_stack(5, (7, 6, 7, 6), H=1024, W=600, n_movers=40, n_stars=60)
-    vx, vy = synth.config3_grid(32, 16)
+    vx, vy = synth.config3_grid()  # the full 128 x 64 grid: dense enough for every velocity group to be staged
     d = _prep(kb, st)
     outs = {}
     for name, algo in (("direct", kb.ALGO_DIRECT), ("pruned", kb.ALGO_PRUNED)):
