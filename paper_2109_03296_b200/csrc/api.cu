@@ -227,7 +227,6 @@ extern "C" int kbmod_search(const float* d_psiphi, int T, int H, int W, const do
     }
     unsigned long long stats[8] = {0, (unsigned long long)plane * n_vel, 1, (unsigned long long)algo, 0, 0, 0, 0};
     if (algo == KBMOD_ALGO_DIRECT) stats[0] = stats[1];
-    else stats[2] = 3;
     // pageable source: cudaMemcpyAsync stages it before returning, so the vectors may go out of scope
     KB_CUDA(cudaMemcpyAsync(ws + pl.off_stats, stats, sizeof(stats), cudaMemcpyHostToDevice, st));
     if (n_vel > 0)
@@ -236,9 +235,14 @@ extern "C" int kbmod_search(const float* d_psiphi, int T, int H, int W, const do
     const DispEntry* d_tab = (const DispEntry*)(ws + pl.off_tab);
     if (algo == KBMOD_ALGO_DIRECT)
         return kb_launch_search_direct(d_psiphi, T, TP, H, W, d_tab, n_vel, P, d_lh, d_flux, d_vel_idx, d_n_obs, st);
-    return kb_launch_search_pruned(d_psiphi, T, TP, H, W, d_tab, hdx.data(), hdy.data(), n_vel, p, P, d_lh, d_flux,
-                                   d_vel_idx, d_n_obs, ws + pl.off_pruned, pl.pruned_bytes,
-                                   (unsigned long long*)(ws + pl.off_stats), st, 0, nullptr, nullptr);
+    int launches = 0;
+    rc = kb_launch_search_pruned(d_psiphi, T, TP, H, W, d_tab, hdx.data(), hdy.data(), n_vel, p, P, d_lh, d_flux,
+                                 d_vel_idx, d_n_obs, ws + pl.off_pruned, pl.pruned_bytes,
+                                 (unsigned long long*)(ws + pl.off_stats), st, 0, nullptr, &launches);
+    if (rc) return rc;
+    const unsigned long long nl = (unsigned long long)launches;  // kernels this call enqueued
+    KB_CUDA(cudaMemcpyAsync(ws + pl.off_stats + 2 * sizeof(unsigned long long), &nl, sizeof(nl), cudaMemcpyHostToDevice, st));
+    return KBMOD_OK;
 }
 
 extern "C" int kbmod_search_stats(const void* d_workspace, unsigned long long* h_out) {

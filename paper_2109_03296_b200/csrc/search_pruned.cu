@@ -10,15 +10,22 @@
 // U needs one float2 per trajectory-epoch: (a, q) = (psi_+, -1/sqrt(phi)), zero where invalid:
 //     A += a;  qmin = min(qmin, q);  n += (q < 0)        U = A * (-qmin) / sqrt(m(n))
 //
-// Phase 1 (where the time goes): epoch-outer; a CTA owns a 64x16 tile of start pixels and a group
-// of 16 neighbouring velocities; for each epoch the tile (+) the group's displacement bounding box
-// is staged by TMA (zero fill outside the image = the off-chip rule) into a double-buffered shared
-// memory region and every thread gathers its 2 pixels x 16 velocities from it (8 B per
-// trajectory-epoch evaluation, conflict-free LDS.64).  Phase 2: (pixel, velocity) pairs whose bound
-// reaches min_lh are compacted into a shared-memory queue and evaluated exactly by the same device
-// function as the direct kernel, gathering from the psi/phi stack in L2.  Results enter the per-pixel
-// top-K through a cascade of 64-bit atomicMax on (orderable L', ~vel_idx) keys; a last kernel turns
-// keys into the four output arrays.
+// Kernels (all on the caller's stream, per batch of tiles):
+//   bound_plane_kernel   once: the (a, q) planes, row pitch even so that TMA boxes start 16-byte aligned
+//   bound_phase_kernel   where the time goes.  Persistent, one CTA per SM = 16 consumer warps + 1
+//                        producer warp.  A CTA owns a 64x16 tile of start pixels and walks the velocity
+//                        groups (<= 16 neighbouring velocities); for each epoch the tile (+) the group's
+//                        displacement bounding box is staged by TMA (zero fill outside the image = the
+//                        off-chip rule) into a byte ring in shared memory, several epochs ahead, and
+//                        every consumer thread gathers its 2 pixels x 16 velocities from it (8 B per
+//                        trajectory-epoch evaluation, conflict-free LDS.64).  full/empty mbarriers per
+//                        in-flight region; no CTA-wide barrier anywhere in the loop.  (pixel, velocity)
+//                        pairs whose bound reaches min_lh are appended to a global queue.
+//   exact_queue_kernel   the queued pairs get the same device function as the direct kernel (gather from
+//                        the psi/phi stack in L2, register sorting network); results enter the per-pixel
+//                        top-K through a cascade of 64-bit atomicMax on (orderable L', ~vel_idx) keys.
+//   exact_overflow_kernel  pairs of (tile, group, warp) items that did not fit the queue, all evaluated.
+//   finalize_kernel      keys -> the four output arrays.
 #include <algorithm>
 #include <vector>
 
@@ -29,23 +36,41 @@ namespace {
 
 constexpr int PR_TW = 64, PR_TH = 16;      // tile of start pixels per CTA
 constexpr int PR_G = 16;                   // velocities per group
-constexpr int PR_THREADS = 512;            // 16 warps; thread = (x, y) and (x+32, y)
+constexpr int PR_CONSUMERS = 512;          // 16 warps; thread = (x, y) and (x+32, y)
+constexpr int PR_THREADS = PR_CONSUMERS + 128;  // + the producer warp group (one of its threads works)
 constexpr int PR_RB = 8;                   // rows per TMA box
 constexpr int PR_NPITCH = 12;              // tensor maps: pitch = 64 + 16*k elements, k < 12  (<= 240)
-constexpr int PR_BUF_BYTES = 96 * 1024;    // one staging buffer
-constexpr int PR_MAXT = KBMOD_MAX_T;
+constexpr int PR_NB = 8;                   // regions in flight (mbarrier pairs)
+constexpr int PR_NTBL = 4;                 // group tables in flight
+constexpr int PR_SMEM_MAX = 232448;        // 227 KB: the opt-in maximum of dynamic shared memory per CTA
+constexpr int PR_SMEM_MISC = 256;          // barriers + producer bookkeeping
+constexpr int PR_WAVES_PER_BATCH = 7;
+// 20 warps = 5 per scheduler: 16384 registers / (5 x 32) = 102 -> 96 per thread at launch.  setmaxnreg moves
+// registers inside the CTA's own allocation (640 x 96 = 61440): the producer warp group drops to 24 and the
+// 16 consumer warps rise to 112 (512 x 112 + 128 x 24 = 60416 <= 61440)
+constexpr int PR_REGS_PRODUCER = 24, PR_REGS_CONSUMER = 112;      // tiles per batch = SMs x this (the queue is reused per batch)
 
-struct __align__(8) GroupEpoch {
-    int16_t ox, oy;    // region origin relative to the tile origin (min dx, min dy of the group)
-    uint16_t pitch_k;  // tensor map / pitch index
-    uint16_t n_box;    // boxes of PR_RB rows; 0xFFFF in epoch 0 marks a group that cannot be staged
+// per (group, epoch): where the staged region comes from and where it goes in the ring
+struct __align__(16) GroupEpoch {
+    int32_t ox, oy;       // region origin relative to the tile origin (min dx rounded down to even, min dy)
+    uint16_t pitch_k;     // tensor map / pitch index: pitch = PR_TW + 16 * pitch_k elements
+    uint16_t n_box;       // boxes of PR_RB rows
+    uint32_t smem_off;    // byte offset of the region in the ring (the chain restarts at 0 for every tile)
+    uint32_t footprint;   // ring bytes charged to this region = its size + the unused tail skipped before it
+    uint32_t vmask;       // bit j: velocity slot j of the group is in use
+    uint32_t pad_[2];
 };
+static_assert(sizeof(GroupEpoch) == 32, "GroupEpoch must be 32 bytes");
+
+// table block of one group, copied to shared memory with the group's first region:
+//   int32 offs[T][PR_G] (element offset of velocity j's displacement inside the region), GroupEpoch ge[T]
+__host__ __device__ inline int tbl_bytes(int T) { return T * (PR_G * 4 + (int)sizeof(GroupEpoch)); }
 
 struct PrunedTables {  // device pointers into the workspace
-    const int32_t* gvel;     // [n_groups][PR_G]  velocity index or -1
-    const GroupEpoch* ge;    // [n_groups][T]
-    const int32_t* offs;     // [n_groups][T][PR_G] element offset inside the staged region
+    const int32_t* gvel;          // [n_groups][PR_G]  velocity index or -1
+    const unsigned char* gtbl;    // [n_groups] table blocks of tbl_bytes(T)
     int n_groups;
+    int ring_bytes;
 };
 
 struct TensorMaps {
@@ -54,6 +79,13 @@ struct TensorMaps {
 
 struct BoundParams {
     float minv[KBMOD_MAX_T + 1];  // (1 + eps) / sqrt(m(n))
+};
+
+struct Queue {
+    uint2* entries;                  // (pixel index y0*W+x0, velocity index); v = 0xFFFFFFFF: hole
+    unsigned long long* count;       // entries appended (may exceed cap: the excess overflowed)
+    unsigned long long cap;
+    unsigned int* overflow;          // bitmap over (tile, group, warp) items that did not fit
 };
 
 // ---------------------------------------------------------------------------------------------
@@ -80,9 +112,6 @@ __device__ __forceinline__ unsigned int orderable(float f) {
     const unsigned int u = __float_as_uint(f);
     return (u & 0x80000000u) ? ~u : (u | 0x80000000u);
 }
-__device__ __forceinline__ float unorderable(unsigned int u) {
-    return __uint_as_float((u & 0x80000000u) ? (u & 0x7FFFFFFFu) : ~u);
-}
 
 // insert into a descending list of K keys shared by all CTAs (empty = 0): each slot ends up
 // holding the maximum of everything that reached it, so the list is the top-K of all insertions.
@@ -93,98 +122,131 @@ __device__ __forceinline__ void topk_insert(unsigned long long* keys, int K, uns
     }
 }
 
-// ---------------------------------------------------------------------------------------------
-// shared memory carve-up (dynamic): two staging buffers, then the per-item tables
-struct PrSmemTail {
-    int32_t offs[PR_MAXT][PR_G];
-    GroupEpoch ge[PR_MAXT];
-    int32_t gvel[PR_G];
-    uint64_t full[2];
-    unsigned int qcount;
-};
-constexpr size_t PR_SMEM_BYTES = 2 * (size_t)PR_BUF_BYTES + sizeof(PrSmemTail);
+__device__ __forceinline__ void tile_origin(int tile_lin, int tiles_x, int tiles_y, int& tile_x0, int& tile_y0) {
+    // column-block order: 4 tile columns x all tile rows, then the next 4 columns, so that the CTAs
+    // running at the same time work on a compact block of tiles and share their staged regions in L2
+    const int cb = tile_lin / (4 * tiles_y), rem = tile_lin - cb * 4 * tiles_y;
+    const int cols_here = min(4, tiles_x - cb * 4);
+    const int tyi = rem / cols_here, txi = cb * 4 + rem - tyi * cols_here;
+    tile_x0 = txi * PR_TW;
+    tile_y0 = tyi * PR_TH;
+}
 
-template <int TP>
+// ---------------------------------------------------------------------------------------------
+// phase 1: bounds from shared-memory tiles; survivors -> queue
 __global__ void __launch_bounds__(PR_THREADS, 1)
-search_pruned_kernel(const __grid_constant__ TensorMaps maps, const float2* __restrict__ psiphi, int T, int H, int W,
-                     const DispEntry* __restrict__ tab, const __grid_constant__ PrunedTables tb,
-                     const __grid_constant__ DevParams P, const __grid_constant__ BoundParams BP,
-                     unsigned long long* __restrict__ keys, unsigned long long* __restrict__ stats) {
+bound_phase_kernel(const __grid_constant__ TensorMaps maps, int T, int H, int W, int tile_begin, int tile_end,
+                   const __grid_constant__ PrunedTables tb, const __grid_constant__ BoundParams BP, float min_lh,
+                   int min_obs, const __grid_constant__ Queue Qu) {
     extern __shared__ __align__(1024) unsigned char smem[];
-    float2* buf0 = reinterpret_cast<float2*>(smem);
-    float2* buf1 = reinterpret_cast<float2*>(smem + PR_BUF_BYTES);
-    PrSmemTail& S = *reinterpret_cast<PrSmemTail*>(smem + 2 * (size_t)PR_BUF_BYTES);
-    unsigned short* queue = reinterpret_cast<unsigned short*>(smem);         // phase 2: aliases buf0
-    float* scratch_all = reinterpret_cast<float*>(smem + PR_BUF_BYTES);      // phase 2: aliases buf1
-    constexpr int P2_THREADS = (TP <= 48) ? PR_THREADS : PR_THREADS / 2;     // scratch is [TP][P2_THREADS] floats
+    const int TBL = tbl_bytes(T);
+    unsigned char* tblbase = smem + tb.ring_bytes;
+    uint64_t* full = reinterpret_cast<uint64_t*>(tblbase + PR_NTBL * TBL);
+    uint64_t* empty = full + PR_NB;
+    uint32_t* fpq = reinterpret_cast<uint32_t*>(empty + PR_NB);  // producer only: footprint of each region in flight
 
     const int tid = threadIdx.x;
-    const int tx = tid & 31, ty = tid >> 5;
+    const int lane = tid & 31, warp = tid >> 5;
     if (tid == 0) {
-        kb_mbar_init(&S.full[0], 1);
-        kb_mbar_init(&S.full[1], 1);
+        for (int i = 0; i < PR_NB; ++i) {
+            kb_mbar_init(&full[i], 1);
+            kb_mbar_init(&empty[i], PR_CONSUMERS / 32);
+        }
         kb_fence_barrier_init();
         for (int k = 0; k < PR_NPITCH; ++k) kb_prefetch_tensormap(&maps.m[k]);
     }
     __syncthreads();
 
     const int tiles_x = (W + PR_TW - 1) / PR_TW, tiles_y = (H + PR_TH - 1) / PR_TH;
-    const int n_tiles = tiles_x * tiles_y;
-    // tiles are taken in compact blocks of gridDim.x tiles (4 tile columns wide) so that the CTAs
-    // running at the same time share their staged regions in L2
-    const int need = P.min_obs > 1 ? P.min_obs : 1;
-    unsigned int it = 0;  // epochs staged so far by this CTA: buffer = it & 1, parity = (it >> 1) & 1
-    unsigned long long n_eval = 0;
+    const int ng = tb.n_groups;
 
-    for (int tile_lin = blockIdx.x; tile_lin < n_tiles; tile_lin += gridDim.x) {
-        // column-block order: 4 tile columns x all tile rows, then the next 4 columns
-        const int cb = tile_lin / (4 * tiles_y), rem = tile_lin - cb * 4 * tiles_y;
-        const int cols_here = min(4, tiles_x - cb * 4);
-        const int tyi = rem / cols_here, txi = cb * 4 + rem - tyi * cols_here;
-        const int tile_x0 = txi * PR_TW, tile_y0 = tyi * PR_TH;
-        const int px0 = tile_x0 + tx, py0 = tile_y0 + ty;  // this thread's pixels: (px0, py0), (px0+32, py0)
-
-        for (int g = 0; g < tb.n_groups; ++g) {
-            __syncthreads();  // previous item completely done (tables, queue, scratch)
-            for (int i = tid; i < T * PR_G; i += PR_THREADS) S.offs[i / PR_G][i % PR_G] = tb.offs[(size_t)g * T * PR_G + i];
-            if (tid < T) S.ge[tid] = tb.ge[(size_t)g * T + tid];
-            if (tid < PR_G) S.gvel[tid] = tb.gvel[(size_t)g * PR_G + tid];
-            if (tid == 0) S.qcount = 0;
-            kb_fence_proxy_async();  // phase-2 st.shared into the buffers happen-before the next TMA writes
-            __syncthreads();
-            const bool stageable = S.ge[0].n_box != 0xFFFFu;
-
-            if (stageable) {
-                float A[2][PR_G], Q[2][PR_G];
-                int N[2][PR_G];
-#pragma unroll
-                for (int j = 0; j < PR_G; ++j) {
-                    A[0][j] = A[1][j] = 0.0f;
-                    Q[0][j] = Q[1][j] = 0.0f;
-                    N[0][j] = N[1][j] = 0;
-                }
-                auto issue = [&](int t, unsigned int slot) {
-                    const GroupEpoch e = S.ge[t];
-                    const int pitch = PR_TW + 16 * e.pitch_k;
-                    const unsigned int box_bytes = (unsigned int)pitch * PR_RB * sizeof(float2);
-                    unsigned char* dst = smem + (size_t)slot * PR_BUF_BYTES;
-                    kb_mbar_expect_tx(&S.full[slot], box_bytes * e.n_box);
-                    for (int b = 0; b < e.n_box; ++b)
-                        kb_tma_load_3d(dst + (size_t)b * box_bytes, &maps.m[e.pitch_k], tile_x0 + e.ox,
-                                       tile_y0 + e.oy + b * PR_RB, t, &S.full[slot]);
-                };
-                if (tid == 0) issue(0, it & 1);
-#pragma unroll 1
+    if (warp >= PR_CONSUMERS / 32) {
+        // ------------------------------------------------------------------ producer (one thread)
+        kb_reg_dec<PR_REGS_PRODUCER>();
+        if (tid != PR_CONSUMERS) return;
+        uint32_t q = 0, oldest = 0, used = 0, gcount = 0;
+        uint32_t qs0 = 0, qs1 = 0, qs2 = 0, qs3 = 0;  // first region of the last four groups
+        const uint32_t ring = (uint32_t)tb.ring_bytes;
+        for (int tile_lin = tile_begin + blockIdx.x; tile_lin < tile_end; tile_lin += gridDim.x) {
+            int tile_x0, tile_y0;
+            tile_origin(tile_lin, tiles_x, tiles_y, tile_x0, tile_y0);
+            // the ring chain of the tables restarts at offset 0 for every tile: drain first
+            while (oldest < q) {
+                kb_mbar_wait(&empty[oldest & (PR_NB - 1)], (oldest / PR_NB) & 1);
+                ++oldest;
+            }
+            used = 0;
+            for (int g = 0; g < ng; ++g, ++gcount) {
+                qs0 = qs1; qs1 = qs2; qs2 = qs3; qs3 = q;
+                const unsigned char* gt = tb.gtbl + (size_t)g * TBL;
+                const GroupEpoch* gge = reinterpret_cast<const GroupEpoch*>(gt + (size_t)T * PR_G * 4);
                 for (int t = 0; t < T; ++t) {
-                    __syncthreads();  // everyone finished reading buffer (it+1)&1 (epoch t-1)
-                    if (tid == 0 && t + 1 < T) issue(t + 1, (it + 1) & 1);
-                    kb_mbar_wait(&S.full[it & 1], (it >> 1) & 1);
-                    const float2* buf = (it & 1) ? buf1 : buf0;
-                    const int pitch = PR_TW + 16 * S.ge[t].pitch_k;
-                    const float2* base = buf + ty * pitch + tx;
+                    const int4 e0 = __ldg(reinterpret_cast<const int4*>(gge + t));  // ox, oy, pitch_k|n_box, smem_off
+                    const uint32_t fp = __ldg(&gge[t].footprint);
+                    const int pitch_k = e0.z & 0xFFFF, n_box = (unsigned)e0.z >> 16;
+                    // table slot gcount & 3 was last read by group gcount - 4: all its regions must be released
+                    const bool tbl_busy_possible = (t == 0) && gcount >= PR_NTBL;
+                    while (used + fp > ring || q - oldest >= PR_NB || (tbl_busy_possible && oldest < qs0)) {
+                        kb_mbar_wait(&empty[oldest & (PR_NB - 1)], (oldest / PR_NB) & 1);
+                        used -= fpq[oldest & (PR_NB - 1)];
+                        ++oldest;
+                    }
+                    const int slot = q & (PR_NB - 1);
+                    fpq[slot] = fp;
+                    used += fp;
+                    const int pitch = PR_TW + 16 * pitch_k;
+                    const uint32_t box_bytes = (uint32_t)pitch * PR_RB * sizeof(float2);
+                    kb_mbar_expect_tx(&full[slot], box_bytes * n_box + (t == 0 ? (uint32_t)TBL : 0u));
+                    if (t == 0) kb_bulk_load_1d(tblbase + (gcount & (PR_NTBL - 1)) * TBL, gt, (uint32_t)TBL, &full[slot]);
+                    unsigned char* dst = smem + (uint32_t)e0.w;
+                    for (int b = 0; b < n_box; ++b)
+                        kb_tma_load_3d(dst + (size_t)b * box_bytes, &maps.m[pitch_k], tile_x0 + e0.x,
+                                       tile_y0 + e0.y + b * PR_RB, t, &full[slot]);
+                    ++q;
+                }
+            }
+        }
+        return;
+    }
+
+    // ---------------------------------------------------------------------- consumers
+    kb_reg_inc<PR_REGS_CONSUMER>();
+    const int need = min_obs > 1 ? min_obs : 1;
+    uint32_t q = 0, gcount = 0;
+    for (int tile_lin = tile_begin + blockIdx.x; tile_lin < tile_end; tile_lin += gridDim.x) {
+        int tile_x0, tile_y0;
+        tile_origin(tile_lin, tiles_x, tiles_y, tile_x0, tile_y0);
+        const int px0 = tile_x0 + lane, py0 = tile_y0 + warp;  // this thread's pixels: (px0, py0), (px0+32, py0)
+
+        for (int g = 0; g < ng; ++g, ++gcount) {
+            const unsigned char* tblp = tblbase + (gcount & (PR_NTBL - 1)) * TBL;
+            const int4* offs4 = reinterpret_cast<const int4*>(tblp);
+            const GroupEpoch* ge = reinterpret_cast<const GroupEpoch*>(tblp + (size_t)T * PR_G * 4);
+            float A[2][PR_G], Q[2][PR_G];
+            int N[2][PR_G];
 #pragma unroll
-                    for (int j = 0; j < PR_G; ++j) {
-                        const float2* p = base + S.offs[t][j];
+            for (int j = 0; j < PR_G; ++j) {
+                A[0][j] = A[1][j] = 0.0f;
+                Q[0][j] = Q[1][j] = 0.0f;
+                N[0][j] = N[1][j] = 0;
+            }
+            uint32_t vmask = 0;
+#pragma unroll 1
+            for (int t = 0; t < T; ++t) {
+                const int slot = q & (PR_NB - 1);
+                kb_mbar_wait(&full[slot], (q / PR_NB) & 1);
+                const int4 e0 = *reinterpret_cast<const int4*>(ge + t);
+                if (t == 0) vmask = ge[0].vmask;
+                const int pitch = PR_TW + 16 * (e0.z & 0xFFFF);
+                const float2* base = reinterpret_cast<const float2*>(smem + (uint32_t)e0.w) + warp * pitch + lane;
+#pragma unroll
+                for (int k = 0; k < PR_G / 4; ++k) {
+                    const int4 o = offs4[t * (PR_G / 4) + k];
+                    const int oo[4] = {o.x, o.y, o.z, o.w};
+#pragma unroll
+                    for (int i = 0; i < 4; ++i) {
+                        const int j = 4 * k + i;
+                        const float2* p = base + oo[i];
                         const float2 v0 = p[0], v1 = p[32];
                         A[0][j] += v0.x;
                         Q[0][j] = fminf(Q[0][j], v0.y);
@@ -193,68 +255,153 @@ search_pruned_kernel(const __grid_constant__ TensorMaps maps, const float2* __re
                         Q[1][j] = fminf(Q[1][j], v1.y);
                         N[1][j] += (int)(__float_as_uint(v1.y) >> 31);
                     }
-                    ++it;
                 }
-                __syncthreads();  // all reads of the staging buffers done: the queue may overwrite buf0
-                // bound test; survivors -> queue entry = (pixel-in-tile << 4) | velocity-in-group
+                __syncwarp();
+                if (lane == 0) kb_mbar_arrive(&empty[slot]);  // this warp is done with the region
+                ++q;
+            }
+            // ---- bound test; survivors -> queue
+            unsigned int m[2] = {0u, 0u};
 #pragma unroll
-                for (int h = 0; h < 2; ++h) {
-                    const bool in_img = (px0 + 32 * h) < W && py0 < H;
+            for (int h = 0; h < 2; ++h) {
+                const bool in_img = (px0 + 32 * h) < W && py0 < H;
 #pragma unroll
-                    for (int j = 0; j < PR_G; ++j) {
-                        const int n = N[h][j];
-                        const float U = A[h][j] * (-Q[h][j]) * BP.minv[n];
-                        if (in_img && n >= need && U >= P.min_lh && S.gvel[j] >= 0) {
-                            const unsigned int pos = atomicAdd(&S.qcount, 1u);
-                            queue[pos] = (unsigned short)(((ty * PR_TW + tx + 32 * h) << 4) | j);
+                for (int j = 0; j < PR_G; ++j) {
+                    const int n = N[h][j];
+                    const float U = A[h][j] * (-Q[h][j]) * BP.minv[n];
+                    if (in_img && n >= need && U >= min_lh) m[h] |= 1u << j;
+                }
+                m[h] &= vmask;
+            }
+            const int cnt = __popc(m[0]) + __popc(m[1]);
+            int incl = cnt;
+#pragma unroll
+            for (int d = 1; d < 32; d <<= 1) {
+                const int v = __shfl_up_sync(0xFFFFFFFFu, incl, d);
+                if (lane >= d) incl += v;
+            }
+            const int total = __shfl_sync(0xFFFFFFFFu, incl, 31);
+            if (total > 0) {
+                unsigned long long base = 0;
+                if (lane == 0) base = atomicAdd(Qu.count, (unsigned long long)total);
+                base = __shfl_sync(0xFFFFFFFFu, base, 0);
+                if (base + (unsigned long long)total <= Qu.cap) {
+                    unsigned long long pos = base + (unsigned long long)(incl - cnt);
+                    const unsigned int pixlin = (unsigned int)(py0 * W + px0);
+#pragma unroll
+                    for (int h = 0; h < 2; ++h) {
+                        unsigned int mm = m[h];
+                        while (mm) {
+                            const int j = __ffs(mm) - 1;
+                            mm &= mm - 1;
+                            const int v = __ldg(tb.gvel + (size_t)g * PR_G + j);
+                            Qu.entries[pos++] = make_uint2(pixlin + 32u * h, (unsigned int)v);
                         }
                     }
-                }
-            } else {
-                // group cannot be staged (its displacement box does not fit): every pair is evaluated
-                for (int i = tid; i < PR_TW * PR_TH * PR_G; i += PR_THREADS) {
-                    const int pix = i >> 4, j = i & 15;
-                    const bool in_img = (tile_x0 + (pix & (PR_TW - 1))) < W && (tile_y0 + pix / PR_TW) < H;
-                    if (in_img && S.gvel[j] >= 0) queue[atomicAdd(&S.qcount, 1u)] = (unsigned short)i;
-                }
-            }
-            __syncthreads();
-            // ---- phase 2: exact evaluation of the queued pairs (the direct kernel's device function)
-            const unsigned int qn = S.qcount;
-            if (tid == 0) n_eval += qn;
-            for (unsigned int q0 = 0; q0 < qn; q0 += P2_THREADS) {
-                const unsigned int qi = q0 + tid;
-                if (tid < P2_THREADS && qi < qn) {
-                    const unsigned int e = queue[qi];
-                    const int pix = e >> 4, j = e & 15;
-                    const int x0 = tile_x0 + (pix & (PR_TW - 1)), y0 = tile_y0 + pix / PR_TW;
-                    const int v = S.gvel[j];
-                    const DispEntry* row = tab + (size_t)v * TP;
-                    const int pixlin = y0 * W + x0;
-                    float psi[TP], phi[TP];
-#pragma unroll
-                    for (int t = 0; t < TP; ++t) {
-                        const DispEntry d = row[t];
-                        const int x = x0 + d.dx, y = y0 + d.dy;
-                        float2 s = make_float2(0.0f, 0.0f);
-                        if ((unsigned)x < (unsigned)W && (unsigned)y < (unsigned)H) s = __ldg(psiphi + (pixlin + d.off));
-                        const bool ok = s.y > 0.0f;
-                        psi[t] = ok ? s.x : 0.0f;
-                        phi[t] = ok ? s.y : 0.0f;
-                    }
-                    float lh, flux;
-                    unsigned long long kept;
-                    const int nk = kb_score_lightcurve<TP>(psi, phi, P, scratch_all + tid, P2_THREADS, lh, flux, kept);
-                    if (nk > 0 && lh >= P.min_lh) {
-                        const unsigned long long key =
-                            ((unsigned long long)orderable(lh) << 32) | (unsigned long long)(0xFFFFFFFFu - (unsigned)v);
-                        topk_insert(keys + (size_t)pixlin * P.K, P.K, key);
-                    }
+                } else {
+                    // the queue is full: the whole (tile, group, warp) item goes to the overflow kernel;
+                    // the part of the reservation that lies inside the queue becomes holes
+                    const size_t item = ((size_t)tile_lin * ng + g) * (PR_CONSUMERS / 32) + warp;
+                    if (lane == 0) atomicOr(Qu.overflow + (item >> 5), 1u << (item & 31));
+                    for (unsigned long long i = base + lane; i < base + total && i < Qu.cap; i += 32)
+                        Qu.entries[i] = make_uint2(0u, 0xFFFFFFFFu);
                 }
             }
         }
     }
-    if (tid == 0 && n_eval) atomicAdd(stats, n_eval);
+}
+
+// ---------------------------------------------------------------------------------------------
+// phase 2: exact evaluation (steps 1-3 of kbmod_search) of one (pixel, velocity) pair + top-K insertion
+template <int TP>
+__device__ __forceinline__ void eval_pair(const float2* __restrict__ psiphi, int H, int W,
+                                          const DispEntry* __restrict__ tab, const DevParams& P, int x0, int y0, int v,
+                                          float* scratch, int stride, unsigned long long* __restrict__ keys) {
+    const DispEntry* row = tab + (size_t)v * TP;
+    const int pixlin = y0 * W + x0;
+    float psi[TP], phi[TP];
+#pragma unroll
+    for (int t = 0; t < TP; ++t) {
+        const DispEntry d = row[t];
+        const int x = x0 + d.dx, y = y0 + d.dy;
+        float2 s = make_float2(0.0f, 0.0f);
+        if ((unsigned)x < (unsigned)W && (unsigned)y < (unsigned)H) s = __ldg(psiphi + (pixlin + d.off));
+        const bool ok = s.y > 0.0f;
+        psi[t] = ok ? s.x : 0.0f;
+        phi[t] = ok ? s.y : 0.0f;
+    }
+    float lh, flux;
+    unsigned long long kept;
+    const int nk = kb_score_lightcurve<TP>(psi, phi, P, scratch, stride, lh, flux, kept);
+    if (nk > 0 && lh >= P.min_lh) {
+        const unsigned long long key =
+            ((unsigned long long)orderable(lh) << 32) | (unsigned long long)(0xFFFFFFFFu - (unsigned)v);
+        topk_insert(keys + (size_t)pixlin * P.K, P.K, key);
+    }
+}
+
+constexpr int EX_THREADS = 256;
+
+template <int TP>
+__global__ void __launch_bounds__(EX_THREADS)
+exact_queue_kernel(const float2* __restrict__ psiphi, int H, int W, const DispEntry* __restrict__ tab,
+                   const __grid_constant__ DevParams P, const __grid_constant__ Queue Qu,
+                   unsigned long long* __restrict__ keys, unsigned long long* __restrict__ stats) {
+    extern __shared__ float scratch_all[];  // [TP][EX_THREADS]
+    const unsigned long long cnt = *Qu.count;
+    const unsigned long long n = cnt < Qu.cap ? cnt : Qu.cap;
+    unsigned long long done = 0;
+    for (unsigned long long i = (unsigned long long)blockIdx.x * EX_THREADS + threadIdx.x; i < n;
+         i += (unsigned long long)gridDim.x * EX_THREADS) {
+        const uint2 e = Qu.entries[i];
+        if (e.y == 0xFFFFFFFFu) continue;
+        const int y0 = (int)(e.x / (unsigned)W), x0 = (int)(e.x - (unsigned)y0 * (unsigned)W);
+        eval_pair<TP>(psiphi, H, W, tab, P, x0, y0, (int)e.y, scratch_all + threadIdx.x, EX_THREADS, keys);
+        ++done;
+    }
+    // statistics: trajectories fully evaluated
+    for (int d = 16; d > 0; d >>= 1) done += __shfl_down_sync(0xFFFFFFFFu, done, d);
+    if ((threadIdx.x & 31) == 0 && done) atomicAdd(stats, done);
+}
+
+// items that did not fit the queue: every pair of the (tile, group, warp) item is evaluated
+template <int TP>
+__global__ void __launch_bounds__(EX_THREADS)
+exact_overflow_kernel(const float2* __restrict__ psiphi, int H, int W, const DispEntry* __restrict__ tab,
+                      const __grid_constant__ DevParams P, const unsigned int* __restrict__ overflow, size_t n_words,
+                      const int32_t* __restrict__ gvel, int ng, unsigned long long* __restrict__ keys,
+                      unsigned long long* __restrict__ stats) {
+    extern __shared__ float scratch_all[];
+    const int lane = threadIdx.x & 31;
+    const size_t warp_global = ((size_t)blockIdx.x * EX_THREADS + threadIdx.x) >> 5;
+    const size_t n_warps = ((size_t)gridDim.x * EX_THREADS) >> 5;
+    const int tiles_x = (W + PR_TW - 1) / PR_TW, tiles_y = (H + PR_TH - 1) / PR_TH;
+    unsigned long long done = 0;
+    for (size_t w = warp_global; w < n_words; w += n_warps) {
+        unsigned int bits = __ldg(overflow + w);
+        while (bits) {
+            const int b = __ffs(bits) - 1;
+            bits &= bits - 1;
+            const size_t item = w * 32 + b;
+            const int row = (int)(item % (PR_CONSUMERS / 32));
+            const size_t tg = item / (PR_CONSUMERS / 32);
+            const int g = (int)(tg % ng), tile_lin = (int)(tg / ng);
+            int tile_x0, tile_y0;
+            tile_origin(tile_lin, tiles_x, tiles_y, tile_x0, tile_y0);
+            const int y0 = tile_y0 + row;
+            for (int h = 0; h < 2; ++h) {
+                const int x0 = tile_x0 + lane + 32 * h;
+                for (int j = 0; j < PR_G; ++j) {
+                    const int v = __ldg(gvel + (size_t)g * PR_G + j);
+                    if (v < 0 || x0 >= W || y0 >= H) continue;
+                    eval_pair<TP>(psiphi, H, W, tab, P, x0, y0, v, scratch_all + threadIdx.x, EX_THREADS, keys);
+                    ++done;
+                }
+            }
+        }
+    }
+    for (int d = 16; d > 0; d >>= 1) done += __shfl_down_sync(0xFFFFFFFFu, done, d);
+    if (lane == 0 && done) atomicAdd(stats, done);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -316,40 +463,104 @@ kb_encode_tiled_fn kb_get_encode_tiled() {
 
 // ---------------------------------------------------------------------------------------------
 // host planner: velocity grouping (k-d bisection of the displacement at the epoch farthest from
-// times[0]) and the per-(group, epoch) staging geometry
+// times[0]; a group whose staged region would not fit half the ring is bisected further), the
+// per-(group, epoch) staging geometry and the ring offsets
 namespace {
 
-void kd_groups(std::vector<int>& idx, int lo, int hi, const std::vector<int>& px, const std::vector<int>& py,
-               std::vector<std::pair<int, int>>& leaves) {
-    const int n = hi - lo;
-    if (n <= PR_G) {
-        leaves.push_back({lo, hi});
-        return;
+struct Planner {
+    int T, n_vel, ring_bytes, max_region;
+    const int32_t *dx, *dy;  // [n_vel][T], clamped so that any |d| beyond every image size stays off-image
+    std::vector<int> idx, px, py;
+    std::vector<std::pair<int, int>> leaves;
+
+    // staged bytes of velocities idx[lo..hi) at epoch t (and the geometry, if asked for)
+    long long region(int lo, int hi, int t, GroupEpoch* e, int* x0_out, int* y0_out) const {
+        int x0 = INT32_MAX, x1 = INT32_MIN, y0 = INT32_MAX, y1 = INT32_MIN;
+        for (int i = lo; i < hi; ++i) {
+            const int v = idx[i];
+            const int ddx = dx[(size_t)v * T + t], ddy = dy[(size_t)v * T + t];
+            x0 = std::min(x0, ddx); x1 = std::max(x1, ddx); y0 = std::min(y0, ddy); y1 = std::max(y1, ddy);
+        }
+        // TMA: the box must start on a 16-byte boundary, i.e. at an even x for 8-byte elements (an odd
+        // start raises an illegal-instruction fault on sm_100a); tile origins are multiples of 64
+        x0 -= (x0 & 1);
+        const long long bw = (long long)x1 - x0 + PR_TW, bh = (long long)y1 - y0 + PR_TH;
+        const long long pk = (bw - PR_TW + 15) / 16, nb = (bh + PR_RB - 1) / PR_RB;
+        if (pk >= PR_NPITCH) return -1;
+        if (e) {
+            e->ox = x0; e->oy = y0; e->pitch_k = (uint16_t)pk; e->n_box = (uint16_t)nb;
+        }
+        if (x0_out) { *x0_out = x0; *y0_out = y0; }
+        return (PR_TW + 16 * pk) * PR_RB * nb * 8;
     }
-    int x0 = INT32_MAX, x1 = INT32_MIN, y0 = INT32_MAX, y1 = INT32_MIN;
-    for (int i = lo; i < hi; ++i) {
-        x0 = std::min(x0, px[idx[i]]); x1 = std::max(x1, px[idx[i]]);
-        y0 = std::min(y0, py[idx[i]]); y1 = std::max(y1, py[idx[i]]);
+    bool fits(int lo, int hi) const {
+        for (int t = 0; t < T; ++t) {
+            const long long b = region(lo, hi, t, nullptr, nullptr, nullptr);
+            if (b < 0 || b > max_region) return false;
+        }
+        return true;
     }
-    const bool by_x = (x1 - x0) >= (y1 - y0);
-    std::stable_sort(idx.begin() + lo, idx.begin() + hi, [&](int a, int b) {
-        return by_x ? (px[a] != px[b] ? px[a] < px[b] : py[a] < py[b]) : (py[a] != py[b] ? py[a] < py[b] : px[a] < px[b]);
-    });
-    const int ng = (n + PR_G - 1) / PR_G;
-    const int half = (ng / 2) * PR_G;  // split at a multiple of the group size: all leaves but one are full
-    kd_groups(idx, lo, lo + half, px, py, leaves);
-    kd_groups(idx, lo + half, hi, px, py, leaves);
+    void split(int lo, int hi) {
+        const int n = hi - lo;
+        if (n <= PR_G && (n == 1 || fits(lo, hi))) {
+            leaves.push_back({lo, hi});
+            return;
+        }
+        int x0 = INT32_MAX, x1 = INT32_MIN, y0 = INT32_MAX, y1 = INT32_MIN;
+        for (int i = lo; i < hi; ++i) {
+            x0 = std::min(x0, px[idx[i]]); x1 = std::max(x1, px[idx[i]]);
+            y0 = std::min(y0, py[idx[i]]); y1 = std::max(y1, py[idx[i]]);
+        }
+        const bool by_x = (x1 - x0) >= (y1 - y0);
+        std::stable_sort(idx.begin() + lo, idx.begin() + hi, [&](int a, int b) {
+            return by_x ? (px[a] != px[b] ? px[a] < px[b] : py[a] < py[b]) : (py[a] != py[b] ? py[a] < py[b] : px[a] < px[b]);
+        });
+        int half;
+        if (n > PR_G) {
+            const int ngr = (n + PR_G - 1) / PR_G;
+            half = (ngr / 2) * PR_G;  // split at a multiple of the group size: all leaves but one are full
+        } else {
+            half = n / 2;
+        }
+        split(lo, lo + half);
+        split(lo + half, hi);
+    }
+};
+
+int ring_bytes_for(int T) { return ((PR_SMEM_MAX - PR_SMEM_MISC - PR_NTBL * tbl_bytes(T)) / 1024) * 1024; }
+size_t max_groups(int n_vel) {
+    const size_t full = ((size_t)n_vel + PR_G - 1) / PR_G;
+    return std::min((size_t)n_vel, 2 * full + 16);
+}
+size_t queue_cap(int n_vel) {
+    const double want = 1100.0 * PR_TW * PR_TH * (double)n_vel / 32.0;
+    return (size_t)std::min(268435456.0, std::max(1048576.0, want));
+}
+size_t n_tiles_of(int H, int W) { return (size_t)((W + PR_TW - 1) / PR_TW) * ((H + PR_TH - 1) / PR_TH); }
+size_t al256(size_t x) { return (x + 255) & ~(size_t)255; }
+
+struct WsLayout {
+    size_t gvel, gtbl, B, keys, qentries, qcount, overflow, total, overflow_words;
+};
+WsLayout ws_layout(int T, int H, int W, int n_vel, int K) {
+    WsLayout L;
+    const size_t ngm = max_groups(n_vel), Wp = ((size_t)W + 1) & ~(size_t)1;
+    size_t o = 0;
+    L.gvel = o;     o += al256(ngm * PR_G * 4);
+    L.gtbl = o;     o += al256(ngm * tbl_bytes(T));
+    L.B = o;        o += al256((size_t)T * H * Wp * 8);
+    L.keys = o;     o += al256((size_t)H * W * K * 8);
+    L.qentries = o; o += al256(queue_cap(n_vel) * 8);
+    L.qcount = o;   o += 256;
+    L.overflow_words = (n_tiles_of(H, W) * ngm * (PR_CONSUMERS / 32) + 31) / 32;
+    L.overflow = o; o += al256(L.overflow_words * 4);
+    L.total = o;
+    return L;
 }
 
 }  // namespace
 
-size_t kb_pruned_workspace_bytes(int T, int H, int W, int n_vel, int K) {
-    const size_t ng = ((size_t)n_vel + PR_G - 1) / PR_G;
-    const size_t Wp = ((size_t)W + 1) & ~(size_t)1;
-    auto al = [](size_t x) { return (x + 255) & ~(size_t)255; };
-    return al(ng * PR_G * 4) + al(ng * T * sizeof(GroupEpoch)) + al(ng * T * PR_G * 4) + al((size_t)T * H * Wp * 8) +
-           al((size_t)H * W * K * 8);
-}
+size_t kb_pruned_workspace_bytes(int T, int H, int W, int n_vel, int K) { return ws_layout(T, H, W, n_vel, K).total; }
 
 // m(n): a lower bound on the number of epochs the sigma-G filter keeps out of n valid ones; 0 = no bound
 static bool bound_min_kept(const kbmod_search_params* p, const DevParams& P, int T, BoundParams* bp) {
@@ -377,95 +588,100 @@ int kb_launch_search_pruned(const float* d_psiphi, int T, int TPv, int H, int W,
         kb_set_error("pruned search needs n_sigma >= 0 and n_sigma*coeff >= 0");
         return KBMOD_ERR_UNSUPPORTED;
     }
-    const int ng = (n_vel + PR_G - 1) / PR_G;
-    // ---- grouping
+    const int TBL = tbl_bytes(T);
+    // ---- displacements as the staging sees them: anything beyond every possible image size is off-image
+    // for all start pixels, wherever exactly it is; clamping keeps the geometry inside int32 / TMA coordinates
+    std::vector<int32_t> cdx((size_t)n_vel * T), cdy((size_t)n_vel * T);
+    for (size_t i = 0; i < cdx.size(); ++i) {
+        cdx[i] = std::max(-40000, std::min(40000, h_dx[i]));
+        cdy[i] = std::max(-40000, std::min(40000, h_dy[i]));
+    }
+    Planner pl;
+    pl.T = T; pl.n_vel = n_vel; pl.ring_bytes = ring_bytes_for(T);
+    pl.max_region = (pl.ring_bytes / 2 / 1024) * 1024;
+    pl.dx = cdx.data(); pl.dy = cdy.data();
     int t_far = 0;
     {   // epoch with the largest displacement spread
         long long best = -1;
         for (int t = 0; t < T; ++t) {
             long long s = 0;
-            for (int v = 0; v < n_vel; v += std::max(1, n_vel / 64)) s += llabs((long long)h_dx[(size_t)v * T + t]) + llabs((long long)h_dy[(size_t)v * T + t]);
+            for (int v = 0; v < n_vel; v += std::max(1, n_vel / 64)) s += llabs((long long)cdx[(size_t)v * T + t]) + llabs((long long)cdy[(size_t)v * T + t]);
             if (s > best) { best = s; t_far = t; }
         }
     }
-    std::vector<int> idx(n_vel), px(n_vel), py(n_vel);
+    pl.idx.resize(n_vel); pl.px.resize(n_vel); pl.py.resize(n_vel);
     for (int v = 0; v < n_vel; ++v) {
-        idx[v] = v;
-        px[v] = std::max(-40000, std::min(40000, h_dx[(size_t)v * T + t_far]));
-        py[v] = std::max(-40000, std::min(40000, h_dy[(size_t)v * T + t_far]));
+        pl.idx[v] = v;
+        pl.px[v] = cdx[(size_t)v * T + t_far];
+        pl.py[v] = cdy[(size_t)v * T + t_far];
     }
-    std::vector<std::pair<int, int>> leaves;
-    if (n_vel > 0) kd_groups(idx, 0, n_vel, px, py, leaves);
-    std::vector<int32_t> gvel((size_t)ng * PR_G, -1), offs((size_t)ng * T * PR_G, 0);
-    std::vector<GroupEpoch> ge((size_t)ng * T);
+    if (n_vel > 0) pl.split(0, n_vel);
+    const int ng = (int)pl.leaves.size();
+    const size_t ngm = max_groups(n_vel);
+
+    // ---- tables: gvel, per-group blocks {offs[T][G], ge[T]}, ring chain
+    std::vector<int32_t> gvel((size_t)ng * PR_G, -1);
+    std::vector<unsigned char> gtbl((size_t)ng * TBL, 0);
     double staged = 0.0, evals = 0.0;
-    int n_unstageable = 0;
+    uint32_t ph = 0;
     for (int g = 0; g < ng; ++g) {
-        const int lo = leaves[g].first, cnt = leaves[g].second - leaves[g].first;
-        for (int j = 0; j < cnt; ++j) gvel[(size_t)g * PR_G + j] = idx[lo + j];
-        bool ok = true;
-        double g_staged = 0.0;
-        for (int t = 0; t < T && ok; ++t) {
-            int x0 = INT32_MAX, x1 = INT32_MIN, y0 = INT32_MAX, y1 = INT32_MIN;
-            for (int j = 0; j < cnt; ++j) {
-                const int v = idx[lo + j];
-                const int dx = h_dx[(size_t)v * T + t], dy = h_dy[(size_t)v * T + t];
-                x0 = std::min(x0, dx); x1 = std::max(x1, dx); y0 = std::min(y0, dy); y1 = std::max(y1, dy);
-            }
-            // TMA: the box must start on a 16-byte boundary, i.e. at an even x for 8-byte elements (an odd
-            // start raises an illegal-instruction fault on sm_100a); tile origins are multiples of 64
-            x0 -= (x0 & 1);
-            const long long bw = (long long)x1 - x0 + PR_TW, bh = (long long)y1 - y0 + PR_TH;
-            const long long pk = (bw - PR_TW + 15) / 16, nb = (bh + PR_RB - 1) / PR_RB;
-            const long long bytes = (PR_TW + 16 * pk) * PR_RB * nb * 8;
-            if (pk >= PR_NPITCH || bytes > PR_BUF_BYTES || x0 < -30000 || x1 > 30000 || y0 < -30000 || y1 > 30000) {
-                ok = false;
-                break;
-            }
+        const int lo = pl.leaves[g].first, cnt = pl.leaves[g].second - pl.leaves[g].first;
+        for (int j = 0; j < cnt; ++j) gvel[(size_t)g * PR_G + j] = pl.idx[lo + j];
+        int32_t* offs = reinterpret_cast<int32_t*>(gtbl.data() + (size_t)g * TBL);
+        GroupEpoch* ge = reinterpret_cast<GroupEpoch*>(gtbl.data() + (size_t)g * TBL + (size_t)T * PR_G * 4);
+        for (int t = 0; t < T; ++t) {
             GroupEpoch e;
-            e.ox = (int16_t)x0; e.oy = (int16_t)y0; e.pitch_k = (uint16_t)pk; e.n_box = (uint16_t)nb;
-            ge[(size_t)g * T + t] = e;
-            const int pitch = PR_TW + 16 * (int)pk;
+            memset(&e, 0, sizeof(e));
+            int x0, y0;
+            const long long bytes = pl.region(lo, lo + cnt, t, &e, &x0, &y0);
+            KB_REQUIRE(bytes > 0 && bytes <= pl.max_region, KBMOD_ERR_UNSUPPORTED, "planner: region of %lld bytes", bytes);
+            const int pitch = PR_TW + 16 * (int)e.pitch_k;
             for (int j = 0; j < cnt; ++j) {
-                const int v = idx[lo + j];
-                offs[((size_t)g * T + t) * PR_G + j] = (h_dy[(size_t)v * T + t] - y0) * pitch + (h_dx[(size_t)v * T + t] - x0);
+                const int v = pl.idx[lo + j];
+                offs[t * PR_G + j] = (cdy[(size_t)v * T + t] - y0) * pitch + (cdx[(size_t)v * T + t] - x0);
             }
-            g_staged += (double)bytes;
+            uint32_t pad = 0;
+            if (ph + (uint32_t)bytes > (uint32_t)pl.ring_bytes) { pad = (uint32_t)pl.ring_bytes - ph; ph = 0; }
+            e.smem_off = ph;
+            e.footprint = (uint32_t)bytes + pad;
+            e.vmask = cnt >= 32 ? 0xFFFFFFFFu : ((1u << cnt) - 1u);
+            ph += (uint32_t)bytes;
+            ge[t] = e;
+            staged += (double)bytes;
         }
-        if (!ok) {
-            for (int t = 0; t < T; ++t) ge[(size_t)g * T + t] = GroupEpoch{0, 0, 0, 0xFFFF};
-            ++n_unstageable;
-        } else {
-            staged += g_staged;
-            evals += (double)PR_TW * PR_TH * cnt * T;
-        }
+        evals += (double)PR_TW * PR_TH * cnt * T;
     }
     if (plan_stats) {
-        plan_stats[0] = ng ? (double)n_unstageable / ng : 0.0;  // fraction of groups that cannot be staged
-        plan_stats[1] = evals > 0 ? staged / evals : 0.0;       // staged bytes per evaluation
+        plan_stats[0] = (size_t)ng > ngm ? 1.0 : 0.0;       // the velocity list is too scattered to group
+        plan_stats[1] = evals > 0 ? staged / evals : 0.0;   // staged bytes per evaluation
     }
     if (plan_only) return KBMOD_OK;
+    KB_REQUIRE((size_t)ng <= ngm, KBMOD_ERR_UNSUPPORTED,
+               "pruned search: %d velocity groups needed, workspace holds %zu (velocities too scattered; use the direct kernel)",
+               ng, ngm);
 
     // ---- workspace carve-up
-    auto al = [](size_t x) { return (x + 255) & ~(size_t)255; };
+    const WsLayout L = ws_layout(T, H, W, n_vel, P.K);
+    KB_REQUIRE(L.total <= ws_bytes, KBMOD_ERR_WORKSPACE, "pruned search workspace: need %zu, have %zu", L.total, ws_bytes);
     const size_t Wp = ((size_t)W + 1) & ~(size_t)1;
-    char* w = (char*)d_ws;
-    size_t o = 0;
-    int32_t* d_gvel = (int32_t*)(w + o);        o += al((size_t)ng * PR_G * 4);
-    GroupEpoch* d_ge = (GroupEpoch*)(w + o);    o += al((size_t)ng * T * sizeof(GroupEpoch));
-    int32_t* d_offs = (int32_t*)(w + o);        o += al((size_t)ng * T * PR_G * 4);
-    float2* d_B = (float2*)(w + o);             o += al((size_t)T * H * Wp * 8);
-    unsigned long long* d_keys = (unsigned long long*)(w + o);
-    o += al((size_t)H * W * P.K * 8);
-    KB_REQUIRE(o <= ws_bytes, KBMOD_ERR_WORKSPACE, "pruned search workspace: need %zu, have %zu", o, ws_bytes);
     KB_REQUIRE((double)T * H * Wp < 2147483648.0, KBMOD_ERR_UNSUPPORTED, "T*H*Wp exceeds 2^31");
+    char* w = (char*)d_ws;
+    int32_t* d_gvel = (int32_t*)(w + L.gvel);
+    unsigned char* d_gtbl = (unsigned char*)(w + L.gtbl);
+    float2* d_B = (float2*)(w + L.B);
+    unsigned long long* d_keys = (unsigned long long*)(w + L.keys);
+    Queue Qu;
+    Qu.entries = (uint2*)(w + L.qentries);
+    Qu.count = (unsigned long long*)(w + L.qcount);
+    Qu.cap = queue_cap(n_vel);
+    Qu.overflow = (unsigned int*)(w + L.overflow);
 
     if (ng > 0) {
         KB_CUDA(cudaMemcpyAsync(d_gvel, gvel.data(), gvel.size() * 4, cudaMemcpyHostToDevice, st));
-        KB_CUDA(cudaMemcpyAsync(d_ge, ge.data(), ge.size() * sizeof(GroupEpoch), cudaMemcpyHostToDevice, st));
-        KB_CUDA(cudaMemcpyAsync(d_offs, offs.data(), offs.size() * 4, cudaMemcpyHostToDevice, st));
+        KB_CUDA(cudaMemcpyAsync(d_gtbl, gtbl.data(), gtbl.size(), cudaMemcpyHostToDevice, st));
     }
     KB_CUDA(cudaMemsetAsync(d_keys, 0, (size_t)H * W * P.K * 8, st));
+    KB_CUDA(cudaMemsetAsync(Qu.overflow, 0, L.overflow_words * 4, st));
 
     // ---- tensor maps over the bound planes: uint64 elements, dims {Wp, H, T}
     kb_encode_tiled_fn enc = kb_get_encode_tiled();
@@ -484,28 +700,52 @@ int kb_launch_search_pruned(const float* d_psiphi, int T, int TPv, int H, int W,
     }
 
     // ---- launches
+    int launches = 0;
     {
         const size_t n = (size_t)T * H * Wp;
         bound_plane_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(reinterpret_cast<const float2*>(d_psiphi), d_B, W,
                                                                         (int)Wp, (size_t)T * H);
+        ++launches;
     }
     int dev = 0, n_sm = 0;
     KB_CUDA(cudaGetDevice(&dev));
     KB_CUDA(cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev));
-    const int n_tiles = ((W + PR_TW - 1) / PR_TW) * ((H + PR_TH - 1) / PR_TH);
-    const int grid = std::min(n_sm, n_tiles);
-    PrunedTables tb{d_gvel, d_ge, d_offs, ng};
+    const int n_tiles = (int)n_tiles_of(H, W);
+    const int grid = std::max(1, std::min(n_sm, n_tiles));
+    // tiles per batch: whole waves, at most PR_WAVES_PER_BATCH of them, and few enough that 1/32 of the
+    // batch's trajectories fit the queue (what does not fit is evaluated by the overflow kernel)
+    long long waves = PR_WAVES_PER_BATCH;
+    if (n_vel > 0) waves = std::min<long long>(waves, (long long)((double)Qu.cap * 32.0 / ((double)grid * PR_TW * PR_TH * n_vel)));
+    waves = std::max<long long>(1, waves);
+    const int batch = (int)std::min<long long>((long long)n_tiles, waves * grid);
+    const size_t smem1 = (size_t)pl.ring_bytes + (size_t)PR_NTBL * TBL + PR_SMEM_MISC;
+    KB_CUDA(cudaFuncSetAttribute(bound_phase_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem1));
+    PrunedTables tb{d_gvel, d_gtbl, ng, pl.ring_bytes};
+    const float2* psiphi2 = reinterpret_cast<const float2*>(d_psiphi);
     KB_DISPATCH_TP(TPv, {
-        KB_CUDA(cudaFuncSetAttribute(search_pruned_kernel<TP>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                     (int)PR_SMEM_BYTES));
-        search_pruned_kernel<TP><<<grid, PR_THREADS, PR_SMEM_BYTES, st>>>(maps, reinterpret_cast<const float2*>(d_psiphi), T,
-                                                                         H, W, d_tab, tb, P, bp, d_keys, d_stats);
+        const size_t smem2 = (size_t)TP * EX_THREADS * sizeof(float);
+        KB_CUDA(cudaFuncSetAttribute(exact_queue_kernel<TP>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem2));
+        KB_CUDA(cudaFuncSetAttribute(exact_overflow_kernel<TP>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem2));
+        if (ng > 0) {
+            for (int b0 = 0; b0 < n_tiles; b0 += batch) {
+                const int b1 = std::min(n_tiles, b0 + batch);
+                KB_CUDA(cudaMemsetAsync(Qu.count, 0, sizeof(unsigned long long), st));
+                bound_phase_kernel<<<std::min(grid, b1 - b0), PR_THREADS, smem1, st>>>(maps, T, H, W, b0, b1, tb, bp, P.min_lh,
+                                                                                      P.min_obs, Qu);
+                exact_queue_kernel<TP><<<n_sm * 4, EX_THREADS, smem2, st>>>(psiphi2, H, W, d_tab, P, Qu, d_keys, d_stats);
+                launches += 2;
+            }
+            exact_overflow_kernel<TP><<<n_sm * 4, EX_THREADS, smem2, st>>>(psiphi2, H, W, d_tab, P, Qu.overflow,
+                                                                           L.overflow_words, d_gvel, ng, d_keys, d_stats);
+            ++launches;
+        }
         const size_t total = (size_t)H * W * P.K;
         finalize_kernel<TP><<<(unsigned)((total + FIN_THREADS - 1) / FIN_THREADS), FIN_THREADS,
-                              (size_t)TP * FIN_THREADS * sizeof(float), st>>>(d_keys, reinterpret_cast<const float2*>(d_psiphi),
-                                                                             H, W, d_tab, P, d_lh, d_flux, d_vel, d_nobs);
+                              (size_t)TP * FIN_THREADS * sizeof(float), st>>>(d_keys, psiphi2, H, W, d_tab, P, d_lh, d_flux,
+                                                                             d_vel, d_nobs);
+        ++launches;
     });
     KB_CUDA(cudaGetLastError());
-    if (n_launches) *n_launches = 3;
+    if (n_launches) *n_launches = launches;
     return KBMOD_OK;
 }

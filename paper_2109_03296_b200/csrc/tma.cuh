@@ -41,6 +41,20 @@ __device__ __forceinline__ void kb_tma_load_3d(void* smem_dst, const CUtensorMap
         ::"r"(kb_smem_u32(smem_dst)), "l"(map), "r"(x), "r"(y), "r"(z), "r"(kb_smem_u32(bar))
         : "memory");
 }
+// 1-D bulk copy global -> shared (SASS UBLKCP); src, dst 16-byte aligned, bytes a multiple of 16
+__device__ __forceinline__ void kb_bulk_load_1d(void* smem_dst, const void* gsrc, uint32_t bytes, uint64_t* bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(kb_smem_u32(smem_dst)), "l"(gsrc), "r"(bytes), "r"(kb_smem_u32(bar))
+                 : "memory");
+}
+// plain arrive (release.cta): a consumer warp hands a ring slot back to the producer
+__device__ __forceinline__ void kb_mbar_arrive(uint64_t* bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(kb_smem_u32(bar)) : "memory");
+}
+// warp-group register reallocation (setmaxnreg): the producer warp gives registers back, the consumer
+// warps take them; every warp of a warp group (4 consecutive warps) must execute the same instruction
+template <int R> __device__ __forceinline__ void kb_reg_inc() { asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(R)); }
+template <int R> __device__ __forceinline__ void kb_reg_dec() { asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(R)); }
 __device__ __forceinline__ void kb_prefetch_tensormap(const CUtensorMap* map) {
     asm volatile("prefetch.tensormap [%0];" ::"l"(map) : "memory");
 }
