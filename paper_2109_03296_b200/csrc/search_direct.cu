@@ -35,8 +35,10 @@ search_direct_kernel(const float2* __restrict__ psiphi, int H, int W, const Disp
     int cnt = 0;
     float kth = -CUDART_INF_F;  // L' of slot K-1 once the list is full
 
+    const unsigned warp_mask = __activemask();  // lanes past the right edge have left
 #pragma unroll 1
     for (int v = 0; v < n_vel; ++v) {
+        __syncwarp(warp_mask);  // re-converge after the divergent top-K insertion of the previous velocity
         const DispEntry* row = tab + (size_t)v * TP;
         float psi[TP], phi[TP];
 #pragma unroll
