@@ -26,6 +26,8 @@
 //                        top-K through a cascade of 64-bit atomicMax on (orderable L', ~vel_idx) keys.
 //   exact_overflow_kernel  pairs of (tile, group, warp) items that did not fit the queue, all evaluated.
 //   finalize_kernel      keys -> the four output arrays.
+#include <stddef.h>
+
 #include <algorithm>
 #include <vector>
 
@@ -53,7 +55,8 @@ constexpr int PR_REGS_PRODUCER = 24, PR_REGS_CONSUMER = 112;      // tiles per b
 // per (group, epoch): where the staged region comes from and where it goes in the ring
 struct __align__(16) GroupEpoch {
     int32_t ox, oy;       // region origin relative to the tile origin (min dx rounded down to even, min dy)
-    uint16_t pitch_k;     // tensor map / pitch index: pitch = PR_TW + 16 * pitch_k elements
+    uint16_t pitch_k;     // low byte: tensor map / pitch index (pitch = PR_TW + 16 * k elements); bit 8: every
+                          // velocity of the group has the same displacement at this epoch ("uniform")
     uint16_t n_box;       // boxes of PR_RB rows
     uint32_t smem_off;    // byte offset of the region in the ring (the chain restarts at 0 for every tile)
     uint32_t footprint;   // ring bytes charged to this region = its size + the unused tail skipped before it
@@ -89,9 +92,45 @@ struct Queue {
 };
 
 // ---------------------------------------------------------------------------------------------
-// bound planes: B[t][y][x] = (psi_+, -(1+eps)/sqrt(phi)) for valid pixels, (0, 0) otherwise; row pitch Wp
+// bound planes: B[t][y][x] = (an, q) for valid pixels, (0, 0) otherwise; row pitch Wp.
+//   an = ceil(psi_+ / unit) << 7 | 1   fixed point, rounded up, so that one integer add accumulates both the sum
+//                                      and the count of valid epochs (T <= 64 terms below 2^18 stay below 2^24)
+//   q  = -(1+eps)/sqrt(phi)            a term too large for the fixed point is clamped and gets q = -inf: the
+//                                      bound of every trajectory through it is +inf and it is evaluated exactly
+// unit = min_lh * sqrt(mean phi) / 4096 puts the decision threshold near 4096 * sqrt(m) units, so the rounding
+// (at most T units) loosens the bound by well under 1 %.  Any unit > 0 is CORRECT; this one is efficient.
+constexpr int AN_SHIFT = 7;
+constexpr float AN_TERM_MAX = 262143.0f;  // 2^18 - 1
+
+__global__ void bound_scale_kernel(const float2* __restrict__ psiphi, size_t n_px, float min_lh, float* __restrict__ scale) {
+    __shared__ float ssum[32];
+    __shared__ int scnt[32];
+    const size_t n_samp = n_px < 65536 ? n_px : 65536, stride = n_px / n_samp;
+    float sum = 0.0f;
+    int cnt = 0;
+    for (size_t k = threadIdx.x; k < n_samp; k += blockDim.x) {
+        const float phi = __ldg(psiphi + k * stride).y;
+        if (phi > 0.0f && phi < CUDART_INF_F) { sum += phi; ++cnt; }
+    }
+    for (int d = 16; d > 0; d >>= 1) {
+        sum += __shfl_down_sync(0xFFFFFFFFu, sum, d);
+        cnt += __shfl_down_sync(0xFFFFFFFFu, cnt, d);
+    }
+    if ((threadIdx.x & 31) == 0) { ssum[threadIdx.x >> 5] = sum; scnt[threadIdx.x >> 5] = cnt; }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        for (int w = 1; w < (int)(blockDim.x >> 5); ++w) { sum += ssum[w]; cnt += scnt[w]; }
+        const float mean = cnt > 0 ? sum / (float)cnt : 1.0f;
+        const float ml = (fabsf(min_lh) < CUDART_INF_F) ? fmaxf(fabsf(min_lh), 1e-3f) : 1.0f;
+        float unit = ml * sqrtf(mean) * (1.0f / 4096.0f);
+        if (!(unit > 1e-30f) || !(unit < 1e30f)) unit = 1.0f;
+        scale[0] = unit;
+        scale[1] = 1.0f / unit;
+    }
+}
+
 __global__ void bound_plane_kernel(const float2* __restrict__ psiphi, float2* __restrict__ B, int W, int Wp,
-                                   size_t rows /* T*H */) {
+                                   size_t rows /* T*H */, const float* __restrict__ scale) {
     const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= rows * (size_t)Wp) return;
     const size_t r = i / Wp;
@@ -100,9 +139,19 @@ __global__ void bound_plane_kernel(const float2* __restrict__ psiphi, float2* __
     if (x < W) {
         const float2 s = __ldg(psiphi + r * W + x);
         if (s.y > 0.0f) {
+            // rounded up twice over: the factor covers the float32 product, ceilf the quantisation
+            const float f = fmaxf(s.x, 0.0f) * __ldg(scale + 1) * 1.000001f;
             // 1/sqrt(phi) rounded up: rsqrtf is within 2 ulp, the factor 1 + 2^-20 covers it
-            o.x = fmaxf(s.x, 0.0f);
-            o.y = -(rsqrtf(s.y) * 1.00000095367431640625f);
+            float q = -(rsqrtf(s.y) * 1.00000095367431640625f);
+            unsigned int fix;
+            if (f < AN_TERM_MAX) {
+                fix = (unsigned int)ceilf(f);
+            } else {  // too large (or inf): clamp, and make the bound infinite
+                fix = (unsigned int)AN_TERM_MAX;
+                q = -CUDART_INF_F;
+            }
+            o.x = __uint_as_float((fix << AN_SHIFT) | 1u);
+            o.y = q;
         }
     }
     B[i] = o;
@@ -137,7 +186,7 @@ __device__ __forceinline__ void tile_origin(int tile_lin, int tiles_x, int tiles
 __global__ void __launch_bounds__(PR_THREADS, 1)
 bound_phase_kernel(const __grid_constant__ TensorMaps maps, int T, int H, int W, int tile_begin, int tile_end,
                    const __grid_constant__ PrunedTables tb, const __grid_constant__ BoundParams BP, float min_lh,
-                   int min_obs, const __grid_constant__ Queue Qu) {
+                   int min_obs, const float* __restrict__ scale, const __grid_constant__ Queue Qu) {
     extern __shared__ __align__(1024) unsigned char smem[];
     const int TBL = tbl_bytes(T);
     unsigned char* tblbase = smem + tb.ring_bytes;
@@ -183,7 +232,7 @@ bound_phase_kernel(const __grid_constant__ TensorMaps maps, int T, int H, int W,
                 for (int t = 0; t < T; ++t) {
                     const int4 e0 = __ldg(reinterpret_cast<const int4*>(gge + t));  // ox, oy, pitch_k|n_box, smem_off
                     const uint32_t fp = __ldg(&gge[t].footprint);
-                    const int pitch_k = e0.z & 0xFFFF, n_box = (unsigned)e0.z >> 16;
+                    const int pitch_k = e0.z & 0xFF, n_box = (unsigned)e0.z >> 16;
                     // table slot gcount & 3 was last read by group gcount - 4: all its regions must be released
                     const bool tbl_busy_possible = (t == 0) && gcount >= PR_NTBL;
                     while (used + fp > ring || q - oldest >= PR_NB || (tbl_busy_possible && oldest < qs0)) {
@@ -222,38 +271,49 @@ bound_phase_kernel(const __grid_constant__ TensorMaps maps, int T, int H, int W,
             const unsigned char* tblp = tblbase + (gcount & (PR_NTBL - 1)) * TBL;
             const int4* offs4 = reinterpret_cast<const int4*>(tblp);
             const GroupEpoch* ge = reinterpret_cast<const GroupEpoch*>(tblp + (size_t)T * PR_G * 4);
-            float A[2][PR_G], Q[2][PR_G];
-            int N[2][PR_G];
+            unsigned int AN[2][PR_G];  // sum of the fixed-point psi_+ terms << 7 | number of valid epochs
+            float Q[2][PR_G];          // min of -1/sqrt(phi)
 #pragma unroll
             for (int j = 0; j < PR_G; ++j) {
-                A[0][j] = A[1][j] = 0.0f;
+                AN[0][j] = AN[1][j] = 0u;
                 Q[0][j] = Q[1][j] = 0.0f;
-                N[0][j] = N[1][j] = 0;
             }
-            uint32_t vmask = 0;
+            // epochs at which the whole group shares one displacement (the first night: a few pixels of motion)
+            // are gathered once per pixel and folded into the 16 accumulators at the end
+            unsigned int ANU[2] = {0u, 0u};
+            float QU[2] = {0.0f, 0.0f};
+            uint2 gw = make_uint2(0u, 0u);  // {pitch_k | uniform << 8 | n_box << 16, smem_off} of the next epoch
 #pragma unroll 1
             for (int t = 0; t < T; ++t) {
                 const int slot = q & (PR_NB - 1);
                 kb_mbar_wait(&full[slot], (q / PR_NB) & 1);
-                const int4 e0 = *reinterpret_cast<const int4*>(ge + t);
-                if (t == 0) vmask = ge[0].vmask;
-                const int pitch = PR_TW + 16 * (e0.z & 0xFFFF);
-                const float2* base = reinterpret_cast<const float2*>(smem + (uint32_t)e0.w) + warp * pitch + lane;
+                if (t == 0) gw = *reinterpret_cast<const uint2*>(&ge[0].pitch_k);  // the tables came with this region
+                const uint2 cur = gw;
+                if (t + 1 < T) gw = *reinterpret_cast<const uint2*>(&ge[t + 1].pitch_k);
+                const int pitch = PR_TW + 16 * (int)(cur.x & 0xFFu);
+                const unsigned char* base = smem + cur.y + (size_t)(warp * pitch + lane) * sizeof(float2);
+                if (cur.x & 0x100u) {
+                    const float2* p = reinterpret_cast<const float2*>(base + offs4[t * (PR_G / 4)].x);
+                    const float2 v0 = p[0], v1 = p[32];
+                    ANU[0] += __float_as_uint(v0.x);
+                    QU[0] = fminf(QU[0], v0.y);
+                    ANU[1] += __float_as_uint(v1.x);
+                    QU[1] = fminf(QU[1], v1.y);
+                } else {
 #pragma unroll
-                for (int k = 0; k < PR_G / 4; ++k) {
-                    const int4 o = offs4[t * (PR_G / 4) + k];
-                    const int oo[4] = {o.x, o.y, o.z, o.w};
+                    for (int k = 0; k < PR_G / 4; ++k) {
+                        const int4 o = offs4[t * (PR_G / 4) + k];  // byte offsets inside the region
+                        const int oo[4] = {o.x, o.y, o.z, o.w};
 #pragma unroll
-                    for (int i = 0; i < 4; ++i) {
-                        const int j = 4 * k + i;
-                        const float2* p = base + oo[i];
-                        const float2 v0 = p[0], v1 = p[32];
-                        A[0][j] += v0.x;
-                        Q[0][j] = fminf(Q[0][j], v0.y);
-                        N[0][j] += (int)(__float_as_uint(v0.y) >> 31);
-                        A[1][j] += v1.x;
-                        Q[1][j] = fminf(Q[1][j], v1.y);
-                        N[1][j] += (int)(__float_as_uint(v1.y) >> 31);
+                        for (int i = 0; i < 4; ++i) {
+                            const int j = 4 * k + i;
+                            const float2* p = reinterpret_cast<const float2*>(base + oo[i]);
+                            const float2 v0 = p[0], v1 = p[32];
+                            AN[0][j] += __float_as_uint(v0.x);
+                            Q[0][j] = fminf(Q[0][j], v0.y);
+                            AN[1][j] += __float_as_uint(v1.x);
+                            Q[1][j] = fminf(Q[1][j], v1.y);
+                        }
                     }
                 }
                 __syncwarp();
@@ -262,40 +322,46 @@ bound_phase_kernel(const __grid_constant__ TensorMaps maps, int T, int H, int W,
             }
             // ---- bound test; survivors -> queue
             unsigned int m[2] = {0u, 0u};
+            const uint32_t vmask = __ldg(reinterpret_cast<const uint32_t*>(tb.gtbl + (size_t)g * TBL + (size_t)T * PR_G * 4 +
+                                                                            offsetof(GroupEpoch, vmask)));
+            const float unit = __ldg(scale);
 #pragma unroll
             for (int h = 0; h < 2; ++h) {
                 const bool in_img = (px0 + 32 * h) < W && py0 < H;
 #pragma unroll
                 for (int j = 0; j < PR_G; ++j) {
-                    const int n = N[h][j];
-                    const float U = A[h][j] * (-Q[h][j]) * BP.minv[n];
-                    if (in_img && n >= need && U >= min_lh) m[h] |= 1u << j;
+                    const unsigned int an = AN[h][j] + ANU[h];
+                    const int n = (int)(an & ((1u << AN_SHIFT) - 1u));
+                    const float U = ((float)(an >> AN_SHIFT) * unit) * (-fminf(Q[h][j], QU[h])) * BP.minv[n];
+                    // "not below": a NaN (0 x inf) must pass as well
+                    if (in_img && n >= need && !(U < min_lh)) m[h] |= 1u << j;
                 }
                 m[h] &= vmask;
             }
-            const int cnt = __popc(m[0]) + __popc(m[1]);
-            int incl = cnt;
-#pragma unroll
-            for (int d = 1; d < 32; d <<= 1) {
-                const int v = __shfl_up_sync(0xFFFFFFFFu, incl, d);
-                if (lane >= d) incl += v;
-            }
-            const int total = __shfl_sync(0xFFFFFFFFu, incl, 31);
+            const int total = __reduce_add_sync(0xFFFFFFFFu, __popc(m[0]) + __popc(m[1]));
             if (total > 0) {
                 unsigned long long base = 0;
                 if (lane == 0) base = atomicAdd(Qu.count, (unsigned long long)total);
                 base = __shfl_sync(0xFFFFFFFFu, base, 0);
                 if (base + (unsigned long long)total <= Qu.cap) {
-                    unsigned long long pos = base + (unsigned long long)(incl - cnt);
+                    // entries in (half, velocity, lane) order: neighbours in the queue are neighbouring pixels with
+                    // the same velocity, so the exact kernel's gathers coalesce
+                    unsigned long long pos = base;
                     const unsigned int pixlin = (unsigned int)(py0 * W + px0);
+                    const unsigned int lt = (1u << lane) - 1u;
 #pragma unroll
                     for (int h = 0; h < 2; ++h) {
-                        unsigned int mm = m[h];
-                        while (mm) {
-                            const int j = __ffs(mm) - 1;
-                            mm &= mm - 1;
-                            const int v = __ldg(tb.gvel + (size_t)g * PR_G + j);
-                            Qu.entries[pos++] = make_uint2(pixlin + 32u * h, (unsigned int)v);
+                        unsigned int any = __reduce_or_sync(0xFFFFFFFFu, m[h]);
+                        while (any) {
+                            const int j = __ffs(any) - 1;
+                            any &= any - 1;
+                            const bool mine = (m[h] >> j) & 1u;
+                            const unsigned int bal = __ballot_sync(0xFFFFFFFFu, mine);
+                            if (mine) {
+                                const int v = __ldg(tb.gvel + (size_t)g * PR_G + j);
+                                Qu.entries[pos + __popc(bal & lt)] = make_uint2(pixlin + 32u * h, (unsigned int)v);
+                            }
+                            pos += __popc(bal);
                         }
                     }
                 } else {
@@ -645,16 +711,19 @@ int kb_launch_search_pruned(const float* d_psiphi, int T, int TPv, int H, int W,
             int x0, y0;
             const long long bytes = pl.region(lo, lo + cnt, t, &e, &x0, &y0);
             KB_REQUIRE(bytes > 0 && bytes <= pl.max_region, KBMOD_ERR_UNSUPPORTED, "planner: region of %lld bytes", bytes);
-            const int pitch = PR_TW + 16 * (int)e.pitch_k;
+            const int pitch = PR_TW + 16 * (int)(e.pitch_k & 0xFF);
             for (int j = 0; j < cnt; ++j) {
                 const int v = pl.idx[lo + j];
-                offs[t * PR_G + j] = (cdy[(size_t)v * T + t] - y0) * pitch + (cdx[(size_t)v * T + t] - x0);
+                offs[t * PR_G + j] = ((cdy[(size_t)v * T + t] - y0) * pitch + (cdx[(size_t)v * T + t] - x0)) * (int)sizeof(float2);
             }
             uint32_t pad = 0;
             if (ph + (uint32_t)bytes > (uint32_t)pl.ring_bytes) { pad = (uint32_t)pl.ring_bytes - ph; ph = 0; }
             e.smem_off = ph;
             e.footprint = (uint32_t)bytes + pad;
             e.vmask = cnt >= 32 ? 0xFFFFFFFFu : ((1u << cnt) - 1u);
+            bool same = true;
+            for (int j = 1; j < cnt; ++j) same = same && offs[t * PR_G + j] == offs[t * PR_G];
+            if (same) e.pitch_k |= 0x100;
             ph += (uint32_t)bytes;
             ge[t] = e;
             staged += (double)bytes;
@@ -683,6 +752,7 @@ int kb_launch_search_pruned(const float* d_psiphi, int T, int TPv, int H, int W,
     Queue Qu;
     Qu.entries = (uint2*)(w + L.qentries);
     Qu.count = (unsigned long long*)(w + L.qcount);
+    float* d_scale = (float*)(w + L.qcount + 64);  // {unit, 1/unit} of the fixed-point bound planes
     Qu.cap = queue_cap(n_vel);
     Qu.overflow = (unsigned int*)(w + L.overflow);
 
@@ -713,8 +783,10 @@ int kb_launch_search_pruned(const float* d_psiphi, int T, int TPv, int H, int W,
     int launches = 0;
     {
         const size_t n = (size_t)T * H * Wp;
+        bound_scale_kernel<<<1, 1024, 0, st>>>(reinterpret_cast<const float2*>(d_psiphi), (size_t)T * H * W, P.min_lh, d_scale);
         bound_plane_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(reinterpret_cast<const float2*>(d_psiphi), d_B, W,
-                                                                        (int)Wp, (size_t)T * H);
+                                                                        (int)Wp, (size_t)T * H, d_scale);
+        ++launches;
         ++launches;
     }
     int dev = 0, n_sm = 0;
@@ -741,7 +813,7 @@ int kb_launch_search_pruned(const float* d_psiphi, int T, int TPv, int H, int W,
                 const int b1 = std::min(n_tiles, b0 + batch);
                 KB_CUDA(cudaMemsetAsync(Qu.count, 0, sizeof(unsigned long long), st));
                 bound_phase_kernel<<<std::min(grid, b1 - b0), PR_THREADS, smem1, st>>>(maps, T, H, W, b0, b1, tb, bp, P.min_lh,
-                                                                                      P.min_obs, Qu);
+                                                                                      P.min_obs, d_scale, Qu);
                 exact_queue_kernel<TP><<<n_sm * 4, EX_THREADS, smem2, st>>>(psiphi2, H, W, d_tab, P, Qu, d_keys, d_stats);
                 launches += 2;
             }
