@@ -34,23 +34,38 @@
 #include "common.cuh"
 #include "tma.cuh"
 
+// timing experiments (never defined in the product build): 1 = consumers skip the gathers (producer / TMA
+// limited time), 2 = the producer stages only the tables (consumer limited time; results are garbage)
+#ifndef KB_EXPERIMENT
+#define KB_EXPERIMENT 0
+#endif
+#if KB_EXPERIMENT == 1
+#define KB_EXP1_GUARD if (false)
+#else
+#define KB_EXP1_GUARD
+#endif
+
 namespace {
 
-constexpr int PR_TW = 64, PR_TH = 16;      // tile of start pixels per CTA
+constexpr int PR_TW = 64, PR_TH = 32;      // tile of start pixels per CTA
+constexpr int PR_PIX = (PR_TW / 32) * (PR_TH / 16);  // pixels per consumer thread: (x + 32 h, y + 16 v), index 2 v + h
 constexpr int PR_G = 16;                   // velocities per group
 constexpr int PR_CONSUMERS = 512;          // 16 warps; thread = (x, y) and (x+32, y)
 constexpr int PR_THREADS = PR_CONSUMERS + 128;  // + the producer warp group (one of its threads works)
 constexpr int PR_RB = 8;                   // rows per TMA box
 constexpr int PR_NPITCH = 12;              // tensor maps: pitch = 64 + 16*k elements, k < 12  (<= 240)
-constexpr int PR_NB = 8;                   // regions in flight (mbarrier pairs)
+#ifndef KB_NB
+#define KB_NB 16
+#endif
+constexpr int PR_NB = KB_NB;               // regions in flight (mbarrier pairs); a power of two
 constexpr int PR_NTBL = 4;                 // group tables in flight
 constexpr int PR_SMEM_MAX = 232448;        // 227 KB: the opt-in maximum of dynamic shared memory per CTA
-constexpr int PR_SMEM_MISC = 256;          // barriers + producer bookkeeping
+constexpr int PR_SMEM_MISC = 512;          // barriers + producer bookkeeping
 constexpr int PR_WAVES_PER_BATCH = 7;
 // 20 warps = 5 per scheduler: 16384 registers / (5 x 32) = 102 -> 96 per thread at launch.  setmaxnreg moves
 // registers inside the CTA's own allocation (640 x 96 = 61440): the producer warp group drops to 24 and the
-// 16 consumer warps rise to 112 (512 x 112 + 128 x 24 = 60416 <= 61440)
-constexpr int PR_REGS_PRODUCER = 24, PR_REGS_CONSUMER = 112;      // tiles per batch = SMs x this (the queue is reused per batch)
+// 16 consumer warps rise (512 x 104 + 128 x 40 = 58368 <= 61440)
+constexpr int PR_REGS_PRODUCER = 40, PR_REGS_CONSUMER = 104;      // tiles per batch = SMs x this (the queue is reused per batch)
 
 // per (group, epoch): where the staged region comes from and where it goes in the ring
 struct __align__(16) GroupEpoch {
@@ -81,7 +96,9 @@ struct TensorMaps {
 };
 
 struct BoundParams {
-    float minv[KBMOD_MAX_T + 1];  // (1 + eps) / sqrt(m(n))
+    float thr[KBMOD_MAX_T + 1];            // pass iff sum (in units) >= thr[m_eff]; thr[0] = 0: always
+    unsigned char mkept[KBMOD_MAX_T + 1];  // m(n)
+    int pass_all;                          // min_lh <= 0 (or not finite): nothing can be pruned
 };
 
 struct Queue {
@@ -92,20 +109,28 @@ struct Queue {
 };
 
 // ---------------------------------------------------------------------------------------------
-// bound planes: B[t][y][x] = (an, q) for valid pixels, (0, 0) otherwise; row pitch Wp.
-//   an = ceil(psi_+ / unit) << 7 | 1   fixed point, rounded up, so that one integer add accumulates both the sum
-//                                      and the count of valid epochs (T <= 64 terms below 2^18 stay below 2^24)
-//   q  = -(1+eps)/sqrt(phi)            a term too large for the fixed point is clamped and gets q = -inf: the
-//                                      bound of every trajectory through it is +inf and it is evaluated exactly
-// unit = min_lh * sqrt(mean phi) / 4096 puts the decision threshold near 4096 * sqrt(m) units, so the rounding
-// (at most T units) loosens the bound by well under 1 %.  Any unit > 0 is CORRECT; this one is efficient.
-constexpr int AN_SHIFT = 7;
-constexpr float AN_TERM_MAX = 262143.0f;  // 2^18 - 1
+// bound planes: one 32-bit word per pixel, 0 for invalid pixels (and outside the image, by TMA zero fill);
+// row pitch Wp (a multiple of 4 so that TMA boxes start 16-byte aligned).  For a valid pixel
+//     word = ceil(psi_+ / unit) << 14  |  (phi < f) << 7  |  1
+// so that ONE integer add per trajectory-epoch accumulates the fixed-point sum of psi_+ (rounded up), the
+// number of "low" samples and the number of valid samples.  f = 0.8 x the smallest per-epoch mean of phi (a
+// sample); unit = min_lh * sqrt(f) / PR_THR_UNITS.  A term is clamped to 2^12 - 1 units, which alone exceeds
+// the threshold PR_THR_UNITS * sqrt(m) for every m <= 64, so a clamped term always passes.  Any f > 0 and any
+// unit > 0 give a CORRECT bound; these make it tight.
+constexpr int AN_LOW_SHIFT = 7, AN_SUM_SHIFT = 14;
+constexpr float AN_TERM_MAX = 4095.0f;  // 2^12 - 1: 64 terms stay below 2^18
+constexpr float PR_THR_UNITS = 500.0f;
 
+// One block: f = the largest of the candidates (0.40 + 0.02 k) x mean(phi) that at most 3 % of a strided
+// sample of the valid pixels fall below (so that "low" samples stay rare and f stays just under the level of
+// the noisiest epoch); then unit.  scale = {unit, 1/unit, f}.
+constexpr int SC_BINS = 40, SC_SAMPLES = 65536;
 __global__ void bound_scale_kernel(const float2* __restrict__ psiphi, size_t n_px, float min_lh, float* __restrict__ scale) {
     __shared__ float ssum[32];
     __shared__ int scnt[32];
-    const size_t n_samp = n_px < 65536 ? n_px : 65536, stride = n_px / n_samp;
+    __shared__ int hist[SC_BINS + 1];
+    __shared__ float s_mean;
+    const size_t n_samp = n_px < SC_SAMPLES ? n_px : SC_SAMPLES, stride = n_px / n_samp;
     float sum = 0.0f;
     int cnt = 0;
     for (size_t k = threadIdx.x; k < n_samp; k += blockDim.x) {
@@ -117,41 +142,59 @@ __global__ void bound_scale_kernel(const float2* __restrict__ psiphi, size_t n_p
         cnt += __shfl_down_sync(0xFFFFFFFFu, cnt, d);
     }
     if ((threadIdx.x & 31) == 0) { ssum[threadIdx.x >> 5] = sum; scnt[threadIdx.x >> 5] = cnt; }
+    if (threadIdx.x <= SC_BINS) hist[threadIdx.x] = 0;
     __syncthreads();
     if (threadIdx.x == 0) {
         for (int w = 1; w < (int)(blockDim.x >> 5); ++w) { sum += ssum[w]; cnt += scnt[w]; }
-        const float mean = cnt > 0 ? sum / (float)cnt : 1.0f;
-        const float ml = (fabsf(min_lh) < CUDART_INF_F) ? fmaxf(fabsf(min_lh), 1e-3f) : 1.0f;
-        float unit = ml * sqrtf(mean) * (1.0f / 4096.0f);
+        scnt[0] = cnt;
+        s_mean = cnt > 0 ? sum / (float)cnt : 0.0f;
+    }
+    __syncthreads();
+    const float mean = s_mean;
+    if (mean > 0.0f && mean < CUDART_INF_F) {
+        for (size_t k = threadIdx.x; k < n_samp; k += blockDim.x) {
+            const float phi = __ldg(psiphi + k * stride).y;
+            if (phi > 0.0f && phi < CUDART_INF_F) {
+                const float r = (phi / mean - 0.40f) * 50.0f;  // bin k holds [0.40 + 0.02 k, 0.40 + 0.02 (k+1))
+                const int bin = r < 0.0f ? 0 : (r >= (float)SC_BINS ? SC_BINS : 1 + (int)r);
+                atomicAdd(&hist[bin > SC_BINS ? SC_BINS : bin], 1);  // bin 0: below 0.40 x mean
+            }
+        }
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        float f = 1.0f;
+        if (mean > 0.0f && mean < CUDART_INF_F) {
+            const int budget = (int)(0.03f * (float)scnt[0]);
+            int below = hist[0], k = 0;  // below = samples under 0.40 + 0.02 k
+            while (k + 1 < SC_BINS && below + hist[k + 1] <= budget) { below += hist[k + 1]; ++k; }
+            f = (0.40f + 0.02f * (float)k) * mean;
+        }
+        if (!(f > 1e-30f) || !(f < 1e30f)) f = 1.0f;
+        const float ml = (min_lh > 0.0f && min_lh < CUDART_INF_F) ? min_lh : 1.0f;
+        float unit = ml * sqrtf(f) / PR_THR_UNITS;
         if (!(unit > 1e-30f) || !(unit < 1e30f)) unit = 1.0f;
         scale[0] = unit;
         scale[1] = 1.0f / unit;
+        scale[2] = f;
     }
 }
 
-__global__ void bound_plane_kernel(const float2* __restrict__ psiphi, float2* __restrict__ B, int W, int Wp,
+__global__ void bound_plane_kernel(const float2* __restrict__ psiphi, unsigned int* __restrict__ B, int W, int Wp,
                                    size_t rows /* T*H */, const float* __restrict__ scale) {
     const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= rows * (size_t)Wp) return;
     const size_t r = i / Wp;
     const int x = (int)(i - r * Wp);
-    float2 o = make_float2(0.0f, 0.0f);
+    unsigned int o = 0u;
     if (x < W) {
         const float2 s = __ldg(psiphi + r * W + x);
         if (s.y > 0.0f) {
             // rounded up twice over: the factor covers the float32 product, ceilf the quantisation
-            const float f = fmaxf(s.x, 0.0f) * __ldg(scale + 1) * 1.000001f;
-            // 1/sqrt(phi) rounded up: rsqrtf is within 2 ulp, the factor 1 + 2^-20 covers it
-            float q = -(rsqrtf(s.y) * 1.00000095367431640625f);
-            unsigned int fix;
-            if (f < AN_TERM_MAX) {
-                fix = (unsigned int)ceilf(f);
-            } else {  // too large (or inf): clamp, and make the bound infinite
-                fix = (unsigned int)AN_TERM_MAX;
-                q = -CUDART_INF_F;
-            }
-            o.x = __uint_as_float((fix << AN_SHIFT) | 1u);
-            o.y = q;
+            const float t = fmaxf(s.x, 0.0f) * __ldg(scale + 1) * 1.000001f;
+            const unsigned int fix = (t < AN_TERM_MAX) ? (unsigned int)ceilf(t) : (unsigned int)AN_TERM_MAX;  // inf, too
+            const unsigned int low = (s.y < __ldg(scale + 2)) ? 1u : 0u;
+            o = (fix << AN_SUM_SHIFT) | (low << AN_LOW_SHIFT) | 1u;
         }
     }
     B[i] = o;
@@ -185,8 +228,8 @@ __device__ __forceinline__ void tile_origin(int tile_lin, int tiles_x, int tiles
 // phase 1: bounds from shared-memory tiles; survivors -> queue
 __global__ void __launch_bounds__(PR_THREADS, 1)
 bound_phase_kernel(const __grid_constant__ TensorMaps maps, int T, int H, int W, int tile_begin, int tile_end,
-                   const __grid_constant__ PrunedTables tb, const __grid_constant__ BoundParams BP, float min_lh,
-                   int min_obs, const float* __restrict__ scale, const __grid_constant__ Queue Qu) {
+                   const __grid_constant__ PrunedTables tb, const __grid_constant__ BoundParams BP, int min_obs,
+                   const __grid_constant__ Queue Qu) {
     extern __shared__ __align__(1024) unsigned char smem[];
     const int TBL = tbl_bytes(T);
     unsigned char* tblbase = smem + tb.ring_bytes;
@@ -216,6 +259,13 @@ bound_phase_kernel(const __grid_constant__ TensorMaps maps, int T, int H, int W,
         uint32_t q = 0, oldest = 0, used = 0, gcount = 0;
         uint32_t qs0 = 0, qs1 = 0, qs2 = 0, qs3 = 0;  // first region of the last four groups
         const uint32_t ring = (uint32_t)tb.ring_bytes;
+        int4 nxt0 = make_int4(0, 0, 0, 0);
+        uint32_t nxt_fp = 0;
+        if (ng > 0) {
+            const GroupEpoch* nge = reinterpret_cast<const GroupEpoch*>(tb.gtbl + (size_t)T * PR_G * 4);
+            nxt0 = __ldg(reinterpret_cast<const int4*>(nge));
+            nxt_fp = __ldg(&nge->footprint);
+        }
         for (int tile_lin = tile_begin + blockIdx.x; tile_lin < tile_end; tile_lin += gridDim.x) {
             int tile_x0, tile_y0;
             tile_origin(tile_lin, tiles_x, tiles_y, tile_x0, tile_y0);
@@ -228,10 +278,22 @@ bound_phase_kernel(const __grid_constant__ TensorMaps maps, int T, int H, int W,
             for (int g = 0; g < ng; ++g, ++gcount) {
                 qs0 = qs1; qs1 = qs2; qs2 = qs3; qs3 = q;
                 const unsigned char* gt = tb.gtbl + (size_t)g * TBL;
-                const GroupEpoch* gge = reinterpret_cast<const GroupEpoch*>(gt + (size_t)T * PR_G * 4);
+                // the first epoch's entry was fetched from global memory one group ago (nxt0 / nxt_fp); the other
+                // epochs are read from the group's table in shared memory once it has landed: no global-memory
+                // latency on the producer's critical path
+                int4 e0 = nxt0;
+                uint32_t fp = nxt_fp;
+                const unsigned char* tblp = tblbase + (gcount & (PR_NTBL - 1)) * TBL;
+                const GroupEpoch* sge = reinterpret_cast<const GroupEpoch*>(tblp + (size_t)T * PR_G * 4);
+                const uint32_t q_first = q;
                 for (int t = 0; t < T; ++t) {
-                    const int4 e0 = __ldg(reinterpret_cast<const int4*>(gge + t));  // ox, oy, pitch_k|n_box, smem_off
-                    const uint32_t fp = __ldg(&gge[t].footprint);
+                    if (t == 1) {
+                        kb_mbar_wait(&full[q_first & (PR_NB - 1)], (q_first / PR_NB) & 1);  // the table is in
+                    }
+                    if (t >= 1) {
+                        e0 = *reinterpret_cast<const int4*>(sge + t);
+                        fp = sge[t].footprint;
+                    }
                     const int pitch_k = e0.z & 0xFF, n_box = (unsigned)e0.z >> 16;
                     // table slot gcount & 3 was last read by group gcount - 4: all its regions must be released
                     const bool tbl_busy_possible = (t == 0) && gcount >= PR_NTBL;
@@ -244,14 +306,24 @@ bound_phase_kernel(const __grid_constant__ TensorMaps maps, int T, int H, int W,
                     fpq[slot] = fp;
                     used += fp;
                     const int pitch = PR_TW + 16 * pitch_k;
-                    const uint32_t box_bytes = (uint32_t)pitch * PR_RB * sizeof(float2);
+                    const uint32_t box_bytes = (uint32_t)pitch * PR_RB * sizeof(unsigned int);
+#if KB_EXPERIMENT == 2
+                    kb_mbar_expect_tx(&full[slot], (t == 0 ? (uint32_t)TBL : 0u));
+#else
                     kb_mbar_expect_tx(&full[slot], box_bytes * n_box + (t == 0 ? (uint32_t)TBL : 0u));
+#endif
                     if (t == 0) kb_bulk_load_1d(tblbase + (gcount & (PR_NTBL - 1)) * TBL, gt, (uint32_t)TBL, &full[slot]);
                     unsigned char* dst = smem + (uint32_t)e0.w;
-                    for (int b = 0; b < n_box; ++b)
+                    for (int b = 0; b < (KB_EXPERIMENT == 2 ? 0 : n_box); ++b)
                         kb_tma_load_3d(dst + (size_t)b * box_bytes, &maps.m[pitch_k], tile_x0 + e0.x,
                                        tile_y0 + e0.y + b * PR_RB, t, &full[slot]);
                     ++q;
+                    if (t == 0) {  // fetch the next group's first entry now: a whole group of time to arrive
+                        const int gn = (g + 1 < ng) ? g + 1 : 0;
+                        const GroupEpoch* nge = reinterpret_cast<const GroupEpoch*>(tb.gtbl + (size_t)gn * TBL + (size_t)T * PR_G * 4);
+                        nxt0 = __ldg(reinterpret_cast<const int4*>(nge));
+                        nxt_fp = __ldg(&nge->footprint);
+                    }
                 }
             }
         }
@@ -271,17 +343,17 @@ bound_phase_kernel(const __grid_constant__ TensorMaps maps, int T, int H, int W,
             const unsigned char* tblp = tblbase + (gcount & (PR_NTBL - 1)) * TBL;
             const int4* offs4 = reinterpret_cast<const int4*>(tblp);
             const GroupEpoch* ge = reinterpret_cast<const GroupEpoch*>(tblp + (size_t)T * PR_G * 4);
-            unsigned int AN[2][PR_G];  // sum of the fixed-point psi_+ terms << 7 | number of valid epochs
-            float Q[2][PR_G];          // min of -1/sqrt(phi)
+            // per (pixel, velocity): fixed-point sum of psi_+ << 14 | low-phi samples << 7 | valid samples
+            unsigned int AN[PR_PIX][PR_G];
 #pragma unroll
-            for (int j = 0; j < PR_G; ++j) {
-                AN[0][j] = AN[1][j] = 0u;
-                Q[0][j] = Q[1][j] = 0.0f;
-            }
+            for (int j = 0; j < PR_G; ++j)
+#pragma unroll
+                for (int i = 0; i < PR_PIX; ++i) AN[i][j] = 0u;
             // epochs at which the whole group shares one displacement (the first night: a few pixels of motion)
             // are gathered once per pixel and folded into the 16 accumulators at the end
-            unsigned int ANU[2] = {0u, 0u};
-            float QU[2] = {0.0f, 0.0f};
+            unsigned int ANU[PR_PIX];
+#pragma unroll
+            for (int i = 0; i < PR_PIX; ++i) ANU[i] = 0u;
             uint2 gw = make_uint2(0u, 0u);  // {pitch_k | uniform << 8 | n_box << 16, smem_off} of the next epoch
 #pragma unroll 1
             for (int t = 0; t < T; ++t) {
@@ -291,28 +363,35 @@ bound_phase_kernel(const __grid_constant__ TensorMaps maps, int T, int H, int W,
                 const uint2 cur = gw;
                 if (t + 1 < T) gw = *reinterpret_cast<const uint2*>(&ge[t + 1].pitch_k);
                 const int pitch = PR_TW + 16 * (int)(cur.x & 0xFFu);
-                const unsigned char* base = smem + cur.y + (size_t)(warp * pitch + lane) * sizeof(float2);
+                const unsigned char* base = smem + cur.y + (size_t)(warp * pitch + lane) * sizeof(unsigned int);
+                const int rows16 = 16 * pitch * (int)sizeof(unsigned int);  // this thread's second row of pixels
+#if KB_EXPERIMENT == 1
+                if (false) {
+                } else if (false) {
+#else
                 if (cur.x & 0x100u) {
-                    const float2* p = reinterpret_cast<const float2*>(base + offs4[t * (PR_G / 4)].x);
-                    const float2 v0 = p[0], v1 = p[32];
-                    ANU[0] += __float_as_uint(v0.x);
-                    QU[0] = fminf(QU[0], v0.y);
-                    ANU[1] += __float_as_uint(v1.x);
-                    QU[1] = fminf(QU[1], v1.y);
-                } else {
+#endif
+                    const unsigned char* p = base + offs4[t * (PR_G / 4)].x;
+#pragma unroll
+                    for (int v = 0; v < PR_TH / 16; ++v) {
+                        const unsigned int* pv = reinterpret_cast<const unsigned int*>(p + v * rows16);
+                        ANU[2 * v] += pv[0];
+                        ANU[2 * v + 1] += pv[32];
+                    }
+                } else KB_EXP1_GUARD {
 #pragma unroll
                     for (int k = 0; k < PR_G / 4; ++k) {
                         const int4 o = offs4[t * (PR_G / 4) + k];  // byte offsets inside the region
                         const int oo[4] = {o.x, o.y, o.z, o.w};
 #pragma unroll
                         for (int i = 0; i < 4; ++i) {
-                            const int j = 4 * k + i;
-                            const float2* p = reinterpret_cast<const float2*>(base + oo[i]);
-                            const float2 v0 = p[0], v1 = p[32];
-                            AN[0][j] += __float_as_uint(v0.x);
-                            Q[0][j] = fminf(Q[0][j], v0.y);
-                            AN[1][j] += __float_as_uint(v1.x);
-                            Q[1][j] = fminf(Q[1][j], v1.y);
+                            const unsigned char* p = base + oo[i];
+#pragma unroll
+                            for (int v = 0; v < PR_TH / 16; ++v) {
+                                const unsigned int* pv = reinterpret_cast<const unsigned int*>(p + v * rows16);
+                                AN[2 * v][4 * k + i] += pv[0];
+                                AN[2 * v + 1][4 * k + i] += pv[32];
+                            }
                         }
                     }
                 }
@@ -321,24 +400,27 @@ bound_phase_kernel(const __grid_constant__ TensorMaps maps, int T, int H, int W,
                 ++q;
             }
             // ---- bound test; survivors -> queue
-            unsigned int m[2] = {0u, 0u};
+            unsigned int m[PR_PIX];
             const uint32_t vmask = __ldg(reinterpret_cast<const uint32_t*>(tb.gtbl + (size_t)g * TBL + (size_t)T * PR_G * 4 +
                                                                             offsetof(GroupEpoch, vmask)));
-            const float unit = __ldg(scale);
+            int my_cnt = 0;
 #pragma unroll
-            for (int h = 0; h < 2; ++h) {
-                const bool in_img = (px0 + 32 * h) < W && py0 < H;
+            for (int h = 0; h < PR_PIX; ++h) {
+                const bool in_img = (px0 + 32 * (h & 1)) < W && (py0 + 16 * (h >> 1)) < H;
+                m[h] = 0u;
 #pragma unroll
                 for (int j = 0; j < PR_G; ++j) {
                     const unsigned int an = AN[h][j] + ANU[h];
-                    const int n = (int)(an & ((1u << AN_SHIFT) - 1u));
-                    const float U = ((float)(an >> AN_SHIFT) * unit) * (-fminf(Q[h][j], QU[h])) * BP.minv[n];
-                    // "not below": a NaN (0 x inf) must pass as well
-                    if (in_img && n >= need && !(U < min_lh)) m[h] |= 1u << j;
+                    const int n = (int)(an & 127u), n_low = (int)((an >> AN_LOW_SHIFT) & 127u);
+                    // at least m(n) epochs are kept, at least m(n) - n_low of them with phi >= f
+                    const int m_eff = max((int)BP.mkept[n] - n_low, 0);
+                    const bool pass = BP.pass_all || (float)(an >> AN_SUM_SHIFT) >= BP.thr[m_eff];
+                    if (in_img && n >= need && pass && KB_EXPERIMENT != 2) m[h] |= 1u << j;
                 }
                 m[h] &= vmask;
+                my_cnt += __popc(m[h]);
             }
-            const int total = __reduce_add_sync(0xFFFFFFFFu, __popc(m[0]) + __popc(m[1]));
+            const int total = __reduce_add_sync(0xFFFFFFFFu, my_cnt);
             if (total > 0) {
                 unsigned long long base = 0;
                 if (lane == 0) base = atomicAdd(Qu.count, (unsigned long long)total);
@@ -350,7 +432,7 @@ bound_phase_kernel(const __grid_constant__ TensorMaps maps, int T, int H, int W,
                     const unsigned int pixlin = (unsigned int)(py0 * W + px0);
                     const unsigned int lt = (1u << lane) - 1u;
 #pragma unroll
-                    for (int h = 0; h < 2; ++h) {
+                    for (int h = 0; h < PR_PIX; ++h) {
                         unsigned int any = __reduce_or_sync(0xFFFFFFFFu, m[h]);
                         while (any) {
                             const int j = __ffs(any) - 1;
@@ -359,7 +441,8 @@ bound_phase_kernel(const __grid_constant__ TensorMaps maps, int T, int H, int W,
                             const unsigned int bal = __ballot_sync(0xFFFFFFFFu, mine);
                             if (mine) {
                                 const int v = __ldg(tb.gvel + (size_t)g * PR_G + j);
-                                Qu.entries[pos + __popc(bal & lt)] = make_uint2(pixlin + 32u * h, (unsigned int)v);
+                                Qu.entries[pos + __popc(bal & lt)] =
+                                    make_uint2(pixlin + 32u * (h & 1) + 16u * (unsigned int)W * (h >> 1), (unsigned int)v);
                             }
                             pos += __popc(bal);
                         }
@@ -462,9 +545,8 @@ exact_overflow_kernel(const float2* __restrict__ psiphi, int H, int W, const Dis
             const int g = (int)(tg % ng), tile_lin = (int)(tg / ng);
             int tile_x0, tile_y0;
             tile_origin(tile_lin, tiles_x, tiles_y, tile_x0, tile_y0);
-            const int y0 = tile_y0 + row;
-            for (int h = 0; h < 2; ++h) {
-                const int x0 = tile_x0 + lane + 32 * h;
+            for (int h = 0; h < PR_PIX; ++h) {
+                const int x0 = tile_x0 + lane + 32 * (h & 1), y0 = tile_y0 + row + 16 * (h >> 1);
                 for (int j = 0; j < PR_G; ++j) {
                     const int v = __ldg(gvel + (size_t)g * PR_G + j);
                     if (v >= 0 && x0 < W && y0 < H) {
@@ -557,9 +639,9 @@ struct Planner {
             const int ddx = dx[(size_t)v * T + t], ddy = dy[(size_t)v * T + t];
             x0 = std::min(x0, ddx); x1 = std::max(x1, ddx); y0 = std::min(y0, ddy); y1 = std::max(y1, ddy);
         }
-        // TMA: the box must start on a 16-byte boundary, i.e. at an even x for 8-byte elements (an odd
-        // start raises an illegal-instruction fault on sm_100a); tile origins are multiples of 64
-        x0 -= (x0 & 1);
+        // TMA: the box must start on a 16-byte boundary, i.e. at a multiple of 4 in x for 4-byte elements (a
+        // misaligned start raises an illegal-instruction fault on sm_100a); tile origins are multiples of 64
+        x0 -= (x0 & 3);
         const long long bw = (long long)x1 - x0 + PR_TW, bh = (long long)y1 - y0 + PR_TH;
         const long long pk = (bw - PR_TW + 15) / 16, nb = (bh + PR_RB - 1) / PR_RB;
         if (pk >= PR_NPITCH) return -1;
@@ -567,7 +649,7 @@ struct Planner {
             e->ox = x0; e->oy = y0; e->pitch_k = (uint16_t)pk; e->n_box = (uint16_t)nb;
         }
         if (x0_out) { *x0_out = x0; *y0_out = y0; }
-        return (PR_TW + 16 * pk) * PR_RB * nb * 8;
+        return (PR_TW + 16 * pk) * PR_RB * nb * (long long)sizeof(unsigned int);
     }
     bool fits(int lo, int hi) const {
         for (int t = 0; t < T; ++t) {
@@ -620,11 +702,11 @@ struct WsLayout {
 };
 WsLayout ws_layout(int T, int H, int W, int n_vel, int K) {
     WsLayout L;
-    const size_t ngm = max_groups(n_vel), Wp = ((size_t)W + 1) & ~(size_t)1;
+    const size_t ngm = max_groups(n_vel), Wp = ((size_t)W + 3) & ~(size_t)3;
     size_t o = 0;
     L.gvel = o;     o += al256(ngm * PR_G * 4);
     L.gtbl = o;     o += al256(ngm * tbl_bytes(T));
-    L.B = o;        o += al256((size_t)T * H * Wp * 8);
+    L.B = o;        o += al256((size_t)T * H * Wp * 4);
     L.keys = o;     o += al256((size_t)H * W * K * 8);
     L.qentries = o; o += al256(queue_cap(n_vel) * 8);
     L.qcount = o;   o += 256;
@@ -638,7 +720,8 @@ WsLayout ws_layout(int T, int H, int W, int n_vel, int K) {
 
 size_t kb_pruned_workspace_bytes(int T, int H, int W, int n_vel, int K) { return ws_layout(T, H, W, n_vel, K).total; }
 
-// m(n): a lower bound on the number of epochs the sigma-G filter keeps out of n valid ones; 0 = no bound
+// m(n): a lower bound on the number of epochs the sigma-G filter keeps out of n valid ones, and the
+// thresholds of the bound test in fixed-point units
 static bool bound_min_kept(const kbmod_search_params* p, const DevParams& P, int T, BoundParams* bp) {
     const float prod = p->n_sigma * p->sigmag_coeff;
     for (int n = 0; n <= KBMOD_MAX_T; ++n) {
@@ -649,8 +732,12 @@ static bool bound_min_kept(const kbmod_search_params* p, const DevParams& P, int
             else if (prod >= 0.0f && p->n_sigma >= 0.0f) m = 1;
             else return false;
         }
-        bp->minv[n] = (float)(1.00003 / sqrt((double)m));  // + slack for the float32 sum and product
+        bp->mkept[n] = (unsigned char)(n == 0 ? 0 : m);
+        // U = sum * unit / sqrt(m f) >= min_lh  <=>  sum >= PR_THR_UNITS * sqrt(m); slack for float32 rounding
+        bp->thr[n] = (float)(PR_THR_UNITS * sqrt((double)n) * (1.0 - 1e-4));
     }
+    bp->thr[0] = 0.0f;  // no epoch is known to have phi >= f: no bound
+    bp->pass_all = !(p->min_lh > 0.0f && p->min_lh < INFINITY);
     return true;
 }
 
@@ -714,7 +801,7 @@ int kb_launch_search_pruned(const float* d_psiphi, int T, int TPv, int H, int W,
             const int pitch = PR_TW + 16 * (int)(e.pitch_k & 0xFF);
             for (int j = 0; j < cnt; ++j) {
                 const int v = pl.idx[lo + j];
-                offs[t * PR_G + j] = ((cdy[(size_t)v * T + t] - y0) * pitch + (cdx[(size_t)v * T + t] - x0)) * (int)sizeof(float2);
+                offs[t * PR_G + j] = ((cdy[(size_t)v * T + t] - y0) * pitch + (cdx[(size_t)v * T + t] - x0)) * (int)sizeof(unsigned int);
             }
             uint32_t pad = 0;
             if (ph + (uint32_t)bytes > (uint32_t)pl.ring_bytes) { pad = (uint32_t)pl.ring_bytes - ph; ph = 0; }
@@ -742,17 +829,17 @@ int kb_launch_search_pruned(const float* d_psiphi, int T, int TPv, int H, int W,
     // ---- workspace carve-up
     const WsLayout L = ws_layout(T, H, W, n_vel, P.K);
     KB_REQUIRE(L.total <= ws_bytes, KBMOD_ERR_WORKSPACE, "pruned search workspace: need %zu, have %zu", L.total, ws_bytes);
-    const size_t Wp = ((size_t)W + 1) & ~(size_t)1;
+    const size_t Wp = ((size_t)W + 3) & ~(size_t)3;
     KB_REQUIRE((double)T * H * Wp < 2147483648.0, KBMOD_ERR_UNSUPPORTED, "T*H*Wp exceeds 2^31");
     char* w = (char*)d_ws;
     int32_t* d_gvel = (int32_t*)(w + L.gvel);
     unsigned char* d_gtbl = (unsigned char*)(w + L.gtbl);
-    float2* d_B = (float2*)(w + L.B);
+    unsigned int* d_B = (unsigned int*)(w + L.B);
     unsigned long long* d_keys = (unsigned long long*)(w + L.keys);
     Queue Qu;
     Qu.entries = (uint2*)(w + L.qentries);
     Qu.count = (unsigned long long*)(w + L.qcount);
-    float* d_scale = (float*)(w + L.qcount + 64);  // {unit, 1/unit} of the fixed-point bound planes
+    float* d_scale = (float*)(w + L.qcount + 64);  // {unit, 1/unit, f} of the fixed-point bound planes
     Qu.cap = queue_cap(n_vel);
     Qu.overflow = (unsigned int*)(w + L.overflow);
 
@@ -763,16 +850,16 @@ int kb_launch_search_pruned(const float* d_psiphi, int T, int TPv, int H, int W,
     KB_CUDA(cudaMemsetAsync(d_keys, 0, (size_t)H * W * P.K * 8, st));
     KB_CUDA(cudaMemsetAsync(Qu.overflow, 0, L.overflow_words * 4, st));
 
-    // ---- tensor maps over the bound planes: uint64 elements, dims {Wp, H, T}
+    // ---- tensor maps over the bound planes: uint32 elements, dims {Wp, H, T}
     kb_encode_tiled_fn enc = kb_get_encode_tiled();
     KB_REQUIRE(enc != nullptr, KBMOD_ERR_CUDA, "cuTensorMapEncodeTiled is not available from the driver");
     TensorMaps maps;
     for (int k = 0; k < PR_NPITCH; ++k) {
         cuuint64_t dims[3] = {(cuuint64_t)Wp, (cuuint64_t)H, (cuuint64_t)T};
-        cuuint64_t strides[2] = {(cuuint64_t)Wp * 8, (cuuint64_t)Wp * 8 * (cuuint64_t)H};
+        cuuint64_t strides[2] = {(cuuint64_t)Wp * 4, (cuuint64_t)Wp * 4 * (cuuint64_t)H};
         cuuint32_t box[3] = {(cuuint32_t)(PR_TW + 16 * k), (cuuint32_t)PR_RB, 1};
         cuuint32_t estr[3] = {1, 1, 1};
-        CUresult r = enc(&maps.m[k], CU_TENSOR_MAP_DATA_TYPE_UINT64, 3, (void*)d_B, dims, strides, box, estr,
+        CUresult r = enc(&maps.m[k], CU_TENSOR_MAP_DATA_TYPE_UINT32, 3, (void*)d_B, dims, strides, box, estr,
                          CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
                          CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
         KB_REQUIRE(r == CUDA_SUCCESS, KBMOD_ERR_CUDA, "cuTensorMapEncodeTiled failed with %d (pitch %d)", (int)r,
@@ -786,7 +873,7 @@ int kb_launch_search_pruned(const float* d_psiphi, int T, int TPv, int H, int W,
         bound_scale_kernel<<<1, 1024, 0, st>>>(reinterpret_cast<const float2*>(d_psiphi), (size_t)T * H * W, P.min_lh, d_scale);
         bound_plane_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(reinterpret_cast<const float2*>(d_psiphi), d_B, W,
                                                                         (int)Wp, (size_t)T * H, d_scale);
-        ++launches;
+        launches += 2;
         ++launches;
     }
     int dev = 0, n_sm = 0;
@@ -812,8 +899,7 @@ int kb_launch_search_pruned(const float* d_psiphi, int T, int TPv, int H, int W,
             for (int b0 = 0; b0 < n_tiles; b0 += batch) {
                 const int b1 = std::min(n_tiles, b0 + batch);
                 KB_CUDA(cudaMemsetAsync(Qu.count, 0, sizeof(unsigned long long), st));
-                bound_phase_kernel<<<std::min(grid, b1 - b0), PR_THREADS, smem1, st>>>(maps, T, H, W, b0, b1, tb, bp, P.min_lh,
-                                                                                      P.min_obs, d_scale, Qu);
+                bound_phase_kernel<<<std::min(grid, b1 - b0), PR_THREADS, smem1, st>>>(maps, T, H, W, b0, b1, tb, bp, P.min_obs, Qu);
                 exact_queue_kernel<TP><<<n_sm * 4, EX_THREADS, smem2, st>>>(psiphi2, H, W, d_tab, P, Qu, d_keys, d_stats);
                 launches += 2;
             }
