@@ -181,8 +181,14 @@ def run_reference(args):
 #   direct kernel  : bound "alu" -- every trajectory runs the compare-exchange network; the algorithmic
 #                    lane-operations per trajectory are 2*CE(T) min/max + per epoch 1 gather, 1 divide,
 #                    2 window compares, 2 adds, 1 count = 2*CE(T) + 7*T; peak = 148 SMs x 128 lanes x f_max.
-#   pruned kernel  : bound "smem" -- 8 B (one float2 of the bound planes) per trajectory-epoch evaluation
-#                    read from shared memory; peak = 148 SMs x 128 B/clk x f_max.
+#   pruned path    : bound "smem" -- SURVEY 8(d)'s per-unit figure: 8 B (psi, phi as float32) per
+#                    trajectory-epoch evaluation gathered from shared memory; peak = 148 SMs x 128 B/clk x f_max.
+#                    The dominant kernel is bound_phase_kernel; its duration is measured live with CUDA events
+#                    recorded by the library on the launching stream (kbmod_search_phase_ms).  The kernel itself
+#                    moves 4 B per evaluation: `smem_bytes_per_eval_actual`.
+# dram__bytes_read.sum + dram__bytes_write.sum per step of the dominant kernel from the committed ncu --set full
+# capture (profiles/); None = not captured for this kernel
+TRAFFIC = {"bound_phase_kernel": None, "search_direct_kernel": None}
 CE_COUNT = {4: 5, 5: 9, 8: 19, 10: 32, 12: 42, 16: 63, 20: 103, 24: 132, 26: 147, 28: 162, 32: 191, 40: 305,
             48: 384, 50: 403, 56: 464, 64: 543}
 N_SM = 148
@@ -201,6 +207,7 @@ def run_ours(args):
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     kb.binding.lib()
+    kb.kbmod_search_phase_timing(True)
     peaks = load_peaks()
     dev = torch.device("cuda", local)
 
@@ -222,6 +229,7 @@ def run_ours(args):
 
     ev = lambda: torch.cuda.Event(enable_timing=True)
     seg = {"prep": [], "search": [], "coadd": []}
+    phases = []  # per timed step: the library's own events between the phases of kbmod_search
 
     def step(record):
         e = [ev() for _ in range(4)]
@@ -234,6 +242,7 @@ def run_ours(args):
         e[3].record()
         if record is not None:
             record.append(e)
+            phases.append(kb.kbmod_search_phase_ms())  # waits for this step's search: between steps, not inside one
 
     def barrier():
         torch.cuda.synchronize()
@@ -261,7 +270,7 @@ def run_ours(args):
         seg["coadd"].append(e[2].elapsed_time(e[3]))
     stats = kb.kbmod_search_stats(ws)  # [evaluated, nominal, launches, algo]
     return dict(torch=torch, dist=dist, kb=kb, rank=rank, world=world, dev=dev, st=st, vx=vx, vy=vy, pd=pd, sp=sp,
-                desc=desc, evals=evals, total_ms=total_ms, seg=seg, stats=stats, clocks=clocks, peaks=peaks,
+                desc=desc, evals=evals, total_ms=total_ms, seg=seg, stats=stats, clocks=clocks, peaks=peaks, phases=phases,
                 n_cand=n_cand, out=out)
 
 
@@ -316,19 +325,25 @@ def report(R, args):
     evaluated, nominal, launches, algo_used = R["stats"]
     f_max = peaks["sm_max_mhz"] * 1e6
     tp = min(k for k in CE_COUNT if k >= T)
+    ph = {k: float(np.mean([p[k] for p in R["phases"]])) for k in R["phases"][0]}
+    kernel_ms = ph["gather"]  # the dominant kernel alone: bound_phase_kernel launches / the direct kernel
     if algo_used == kb.ALGO_DIRECT:
         ops = float(H) * W * n_vel * (2 * CE_COUNT[tp] + 7 * T)
-        roof = dict(bound="alu", achieved=ops / (search_ms * 1e-3) / 1e12, peak=N_SM * 128 * f_max / 1e12,
+        roof = dict(bound="alu", achieved=ops / (kernel_ms * 1e-3) / 1e12, peak=N_SM * 128 * f_max / 1e12,
                     unit="Tlane-op/s", kernel="search_direct_kernel",
                     peak_source="derived: 148 SMs x 128 FP32/ALU lanes x sm_max_mhz (DESIGN.md)")
     else:
         byts = R["evals"] * 8.0
-        roof = dict(bound="smem", achieved=byts / (search_ms * 1e-3) / 1e9, peak=N_SM * 128 * f_max / 1e9,
-                    unit="GB/s", kernel="search_pruned_kernel",
-                    peak_source="derived: 148 SMs x 128 B/clk shared-memory bandwidth x sm_max_mhz (DESIGN.md)")
+        roof = dict(bound="smem", achieved=byts / (kernel_ms * 1e-3) / 1e9, peak=N_SM * 128 * f_max / 1e9,
+                    unit="GB/s", kernel="bound_phase_kernel",
+                    peak_source="derived: 148 SMs x 128 B/clk shared-memory bandwidth x sm_max_mhz (DESIGN.md)",
+                    algorithmic_bytes_per_eval=8, smem_bytes_per_eval_actual=4,
+                    whole_search_frac=byts / (search_ms * 1e-3) / 1e9 / (N_SM * 128 * f_max / 1e9))
     roof["frac"] = roof["achieved"] / roof["peak"]
-    roof["traffic"] = None
-    roof["kernel_ms"] = search_ms
+    roof["traffic"] = TRAFFIC.get(roof["kernel"])
+    roof["kernel_ms"] = kernel_ms
+    roof["kernel_share_of_step"] = kernel_ms / ms_per_step
+    roof["search_phases_ms"] = ph
     cpu = None
     if not args.no_cpu_baseline:
         smp = OracleSample(st, R["vx"], R["vy"], R["pd"], args.min_lh)

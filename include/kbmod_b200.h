@@ -131,6 +131,15 @@ int kbmod_search(const float* d_psiphi, int T, int H, int W, const double* h_tim
  * searched (H*W*n_vel), h_out[2] = kernels launched by the call, h_out[3] = algo actually used. */
 int kbmod_search_stats(const void* d_workspace, unsigned long long* h_out);
 
+/* Optional timing of the phases of kbmod_search, per host thread (what bench.py's roofline line reads).
+ * kbmod_search_phase_timing(1) makes every following kbmod_search on this thread record CUDA events on its stream
+ * between its phases (the library creates and keeps a few cudaEvent_t for this; no device memory).
+ * kbmod_search_phase_ms waits for the last timed search and fills h_ms[4] with the milliseconds spent in
+ *   [0] bound planes (pruned only), [1] the gather kernel: bound phase of the pruned path / the whole direct kernel,
+ *   [2] exact evaluation of the surviving trajectories (pruned only), [3] top-K keys -> output arrays (pruned only). */
+int kbmod_search_phase_timing(int enable);
+int kbmod_search_phase_ms(float* h_ms);
+
 /* ---------------------------------------------------------------------------------------------
  * (a6) coadded stamps.  PAPER.md:L141 (s3.3): stamps are coadded by "computing the median pixel
  * value for each pixel along the trajectory"; mean/sum is the earlier variant; 21x21 (L145, L175);

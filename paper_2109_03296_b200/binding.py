@@ -17,7 +17,8 @@ ALGO_AUTO, ALGO_DIRECT, ALGO_PRUNED = 0, 1, 2
 MAX_T, MAX_K, MAX_PSF, MAX_STAMP_RADIUS = 64, 32, 31, 15
 
 EXPORTS = ["kbmod_default_params", "kbmod_prepare_psi_phi", "kbmod_displacements",
-           "kbmod_search_workspace_bytes", "kbmod_search", "kbmod_search_stats", "kbmod_coadd_stamps",
+           "kbmod_search_workspace_bytes", "kbmod_search", "kbmod_search_stats", "kbmod_search_phase_timing",
+           "kbmod_search_phase_ms", "kbmod_coadd_stamps",
            "kbmod_eval_trajectories", "kbmod_sigmag_filter", "kbmod_pipeline_host_arena_bytes",
            "kbmod_pipeline_host", "kbmod_last_error", "kbmod_version"]
 
@@ -180,6 +181,18 @@ def kbmod_search_stats(workspace):
     out = (C.c_ulonglong * 4)()
     _check(lib().kbmod_search_stats(_dev(workspace), out))
     return [int(v) for v in out]
+
+
+def kbmod_search_phase_timing(enable: bool):
+    """Switches the per-phase CUDA-event timing of kbmod_search on or off for this host thread."""
+    _check(lib().kbmod_search_phase_timing(C.c_int(1 if enable else 0)))
+
+
+def kbmod_search_phase_ms():
+    """dict of milliseconds per phase of the last timed kbmod_search on this thread (synchronises)."""
+    out = (C.c_float * 4)()
+    _check(lib().kbmod_search_phase_ms(out))
+    return dict(planes=float(out[0]), gather=float(out[1]), exact=float(out[2]), finalize=float(out[3]))
 
 
 def kbmod_coadd_stamps(img, mask, times, x0, y0, vx, vy, radius, epoch_mask=None, want_mean=True,

@@ -36,6 +36,45 @@ extern "C" void kbmod_default_params(kbmod_search_params* p) {
     p->algo = KBMOD_ALGO_AUTO;
 }
 
+// ---------------------------------------------------------------------------------------------
+// phase timing: per host thread, off by default
+struct PhaseMark { int phase; cudaEvent_t ev; };
+static thread_local bool g_timing = false;
+static thread_local std::vector<PhaseMark> g_marks;      // marks of the last kbmod_search
+static thread_local std::vector<cudaEvent_t> g_pool;     // events to reuse
+
+void kb_phase_mark(int phase, cudaStream_t st) {
+    if (!g_timing) return;
+    if (phase == KB_PHASE_START) {
+        for (auto& m : g_marks) g_pool.push_back(m.ev);
+        g_marks.clear();
+    }
+    cudaEvent_t ev = nullptr;
+    if (!g_pool.empty()) { ev = g_pool.back(); g_pool.pop_back(); }
+    else if (cudaEventCreate(&ev) != cudaSuccess) return;
+    if (cudaEventRecord(ev, st) != cudaSuccess) { g_pool.push_back(ev); return; }
+    g_marks.push_back({phase, ev});
+}
+
+extern "C" int kbmod_search_phase_timing(int enable) {
+    g_timing = enable != 0;
+    return KBMOD_OK;
+}
+
+extern "C" int kbmod_search_phase_ms(float* h_ms) {
+    KB_REQUIRE(h_ms, KBMOD_ERR_INVALID_ARG, "NULL argument");
+    for (int i = 0; i < 4; ++i) h_ms[i] = 0.0f;
+    KB_REQUIRE(g_marks.size() >= 2, KBMOD_ERR_INVALID_ARG, "no timed kbmod_search on this thread (call kbmod_search_phase_timing(1) first)");
+    KB_CUDA(cudaEventSynchronize(g_marks.back().ev));
+    for (size_t i = 1; i < g_marks.size(); ++i) {
+        float ms = 0.0f;
+        KB_CUDA(cudaEventElapsedTime(&ms, g_marks[i - 1].ev, g_marks[i].ev));
+        const int ph = g_marks[i].phase;
+        if (ph >= 0 && ph < 4) h_ms[ph] += ms;
+    }
+    return KBMOD_OK;
+}
+
 static const int kSizes[] = {KB_SORTNET_SIZES};
 
 int kb_padded_T(int T) {
@@ -233,8 +272,12 @@ extern "C" int kbmod_search(const float* d_psiphi, int T, int H, int W, const do
         KB_CUDA(cudaMemcpyAsync(ws + pl.off_tab, tab.data(), tab.size() * sizeof(DispEntry), cudaMemcpyHostToDevice,
                                 st));
     const DispEntry* d_tab = (const DispEntry*)(ws + pl.off_tab);
-    if (algo == KBMOD_ALGO_DIRECT)
-        return kb_launch_search_direct(d_psiphi, T, TP, H, W, d_tab, n_vel, P, d_lh, d_flux, d_vel_idx, d_n_obs, st);
+    kb_phase_mark(KB_PHASE_START, st);
+    if (algo == KBMOD_ALGO_DIRECT) {
+        rc = kb_launch_search_direct(d_psiphi, T, TP, H, W, d_tab, n_vel, P, d_lh, d_flux, d_vel_idx, d_n_obs, st);
+        kb_phase_mark(KB_PHASE_BOUND, st);  // the direct kernel is gather + filter + top-K in one: reported as phase 1
+        return rc;
+    }
     int launches = 0;
     rc = kb_launch_search_pruned(d_psiphi, T, TP, H, W, d_tab, hdx.data(), hdy.data(), n_vel, p, P, d_lh, d_flux,
                                  d_vel_idx, d_n_obs, ws + pl.off_pruned, pl.pruned_bytes,

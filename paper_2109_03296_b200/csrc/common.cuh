@@ -146,6 +146,12 @@ __device__ __forceinline__ int kb_score_lightcurve(const float (&psi)[TP], const
 }
 
 // ---------------------------------------------------------------------------------------------
+// optional phase timing of kbmod_search (kbmod_search_phase_timing / kbmod_search_phase_ms): an event is recorded
+// on the caller's stream after the work of each phase has been enqueued.  No-ops unless timing is switched on.
+enum { KB_PHASE_START = -1, KB_PHASE_PLANES = 0, KB_PHASE_BOUND = 1, KB_PHASE_EXACT = 2, KB_PHASE_FINALIZE = 3 };
+void kb_phase_mark(int phase, cudaStream_t st);
+
+// ---------------------------------------------------------------------------------------------
 // launchers (one per .cu file); all return a KBMOD_* status
 int kb_launch_prep(const float* d_img, const float* d_var, const uint8_t* d_mask, int T, int H, int W,
                    const float* h_psf, int n_psf, int k, float* d_psiphi, cudaStream_t st);

@@ -54,6 +54,7 @@ constexpr int PR_CONSUMERS = 512;          // 16 warps; thread = (x, y) and (x+3
 constexpr int PR_THREADS = PR_CONSUMERS + 128;  // + the producer warp group (one of its threads works)
 constexpr int PR_RB = 8;                   // rows per TMA box
 constexpr int PR_NPITCH = 12;              // tensor maps: pitch = 64 + 16*k elements, k < 12  (<= 240)
+constexpr int PR_NHEIGHT = 4;              // ... x box heights of 8, 16, 32, 64 rows: a region is a few boxes
 #ifndef KB_NB
 #define KB_NB 16
 #endif
@@ -92,7 +93,7 @@ struct PrunedTables {  // device pointers into the workspace
 };
 
 struct TensorMaps {
-    CUtensorMap m[PR_NPITCH];
+    CUtensorMap m[PR_NHEIGHT * PR_NPITCH];  // [height code][pitch index]
 };
 
 struct BoundParams {
@@ -245,7 +246,7 @@ bound_phase_kernel(const __grid_constant__ TensorMaps maps, int T, int H, int W,
             kb_mbar_init(&empty[i], PR_CONSUMERS / 32);
         }
         kb_fence_barrier_init();
-        for (int k = 0; k < PR_NPITCH; ++k) kb_prefetch_tensormap(&maps.m[k]);
+        for (int k = 0; k < PR_NHEIGHT * PR_NPITCH; ++k) kb_prefetch_tensormap(&maps.m[k]);
     }
     __syncthreads();
 
@@ -314,9 +315,16 @@ bound_phase_kernel(const __grid_constant__ TensorMaps maps, int T, int H, int W,
 #endif
                     if (t == 0) kb_bulk_load_1d(tblbase + (gcount & (PR_NTBL - 1)) * TBL, gt, (uint32_t)TBL, &full[slot]);
                     unsigned char* dst = smem + (uint32_t)e0.w;
-                    for (int b = 0; b < (KB_EXPERIMENT == 2 ? 0 : n_box); ++b)
-                        kb_tma_load_3d(dst + (size_t)b * box_bytes, &maps.m[pitch_k], tile_x0 + e0.x,
-                                       tile_y0 + e0.y + b * PR_RB, t, &full[slot]);
+                    // the region's rows (a multiple of 8) as the fewest boxes of 64, 32, 16 or 8 rows: the producer is a
+                    // single thread and every instruction it issues competes with four busy consumer warps
+                    int left = (KB_EXPERIMENT == 2) ? 0 : n_box, done = 0;
+                    while (left > 0) {
+                        const int hc = left >= 8 ? 3 : (left >= 4 ? 2 : (left >= 2 ? 1 : 0));
+                        kb_tma_load_3d(dst + (size_t)done * box_bytes, &maps.m[hc * PR_NPITCH + pitch_k], tile_x0 + e0.x,
+                                       tile_y0 + e0.y + done * PR_RB, t, &full[slot]);
+                        done += 1 << hc;
+                        left -= 1 << hc;
+                    }
                     ++q;
                     if (t == 0) {  // fetch the next group's first entry now: a whole group of time to arrive
                         const int gn = (g + 1 < ng) ? g + 1 : 0;
@@ -415,7 +423,7 @@ bound_phase_kernel(const __grid_constant__ TensorMaps maps, int T, int H, int W,
                     // at least m(n) epochs are kept, at least m(n) - n_low of them with phi >= f
                     const int m_eff = max((int)BP.mkept[n] - n_low, 0);
                     const bool pass = BP.pass_all || (float)(an >> AN_SUM_SHIFT) >= BP.thr[m_eff];
-                    if (in_img && n >= need && pass && KB_EXPERIMENT != 2) m[h] |= 1u << j;
+                    if (in_img && n >= need && pass && (KB_EXPERIMENT != 2 || Qu.cap == ~0ull)) m[h] |= 1u << j;
                 }
                 m[h] &= vmask;
                 my_cnt += __popc(m[h]);
@@ -854,17 +862,18 @@ int kb_launch_search_pruned(const float* d_psiphi, int T, int TPv, int H, int W,
     kb_encode_tiled_fn enc = kb_get_encode_tiled();
     KB_REQUIRE(enc != nullptr, KBMOD_ERR_CUDA, "cuTensorMapEncodeTiled is not available from the driver");
     TensorMaps maps;
-    for (int k = 0; k < PR_NPITCH; ++k) {
-        cuuint64_t dims[3] = {(cuuint64_t)Wp, (cuuint64_t)H, (cuuint64_t)T};
-        cuuint64_t strides[2] = {(cuuint64_t)Wp * 4, (cuuint64_t)Wp * 4 * (cuuint64_t)H};
-        cuuint32_t box[3] = {(cuuint32_t)(PR_TW + 16 * k), (cuuint32_t)PR_RB, 1};
-        cuuint32_t estr[3] = {1, 1, 1};
-        CUresult r = enc(&maps.m[k], CU_TENSOR_MAP_DATA_TYPE_UINT32, 3, (void*)d_B, dims, strides, box, estr,
-                         CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
-                         CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
-        KB_REQUIRE(r == CUDA_SUCCESS, KBMOD_ERR_CUDA, "cuTensorMapEncodeTiled failed with %d (pitch %d)", (int)r,
-                   PR_TW + 16 * k);
-    }
+    for (int hc = 0; hc < PR_NHEIGHT; ++hc)
+        for (int k = 0; k < PR_NPITCH; ++k) {
+            cuuint64_t dims[3] = {(cuuint64_t)Wp, (cuuint64_t)H, (cuuint64_t)T};
+            cuuint64_t strides[2] = {(cuuint64_t)Wp * 4, (cuuint64_t)Wp * 4 * (cuuint64_t)H};
+            cuuint32_t box[3] = {(cuuint32_t)(PR_TW + 16 * k), (cuuint32_t)(PR_RB << hc), 1};
+            cuuint32_t estr[3] = {1, 1, 1};
+            CUresult r = enc(&maps.m[hc * PR_NPITCH + k], CU_TENSOR_MAP_DATA_TYPE_UINT32, 3, (void*)d_B, dims, strides, box, estr,
+                             CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                             CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+            KB_REQUIRE(r == CUDA_SUCCESS, KBMOD_ERR_CUDA, "cuTensorMapEncodeTiled failed with %d (pitch %d, %d rows)", (int)r,
+                       PR_TW + 16 * k, PR_RB << hc);
+        }
 
     // ---- launches
     int launches = 0;
@@ -874,7 +883,7 @@ int kb_launch_search_pruned(const float* d_psiphi, int T, int TPv, int H, int W,
         bound_plane_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(reinterpret_cast<const float2*>(d_psiphi), d_B, W,
                                                                         (int)Wp, (size_t)T * H, d_scale);
         launches += 2;
-        ++launches;
+        kb_phase_mark(KB_PHASE_PLANES, st);
     }
     int dev = 0, n_sm = 0;
     KB_CUDA(cudaGetDevice(&dev));
@@ -900,17 +909,21 @@ int kb_launch_search_pruned(const float* d_psiphi, int T, int TPv, int H, int W,
                 const int b1 = std::min(n_tiles, b0 + batch);
                 KB_CUDA(cudaMemsetAsync(Qu.count, 0, sizeof(unsigned long long), st));
                 bound_phase_kernel<<<std::min(grid, b1 - b0), PR_THREADS, smem1, st>>>(maps, T, H, W, b0, b1, tb, bp, P.min_obs, Qu);
+                kb_phase_mark(KB_PHASE_BOUND, st);
                 exact_queue_kernel<TP><<<n_sm * 4, EX_THREADS, smem2, st>>>(psiphi2, H, W, d_tab, P, Qu, d_keys, d_stats);
+                kb_phase_mark(KB_PHASE_EXACT, st);
                 launches += 2;
             }
             exact_overflow_kernel<TP><<<n_sm * 4, EX_THREADS, smem2, st>>>(psiphi2, H, W, d_tab, P, Qu.overflow,
                                                                            L.overflow_words, d_gvel, ng, d_keys, d_stats);
+            kb_phase_mark(KB_PHASE_EXACT, st);
             ++launches;
         }
         const size_t total = (size_t)H * W * P.K;
         finalize_kernel<TP><<<(unsigned)((total + FIN_THREADS - 1) / FIN_THREADS), FIN_THREADS,
                               (size_t)TP * FIN_THREADS * sizeof(float), st>>>(d_keys, psiphi2, H, W, d_tab, P, d_lh, d_flux,
                                                                              d_vel, d_nobs);
+        kb_phase_mark(KB_PHASE_FINALIZE, st);
         ++launches;
     });
     KB_CUDA(cudaGetLastError());

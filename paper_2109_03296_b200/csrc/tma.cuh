@@ -19,15 +19,17 @@ __device__ __forceinline__ void kb_mbar_expect_tx(uint64_t* bar, uint32_t bytes)
     asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(kb_smem_u32(bar)), "r"(bytes) : "memory");
 }
 __device__ __forceinline__ void kb_mbar_wait(uint64_t* bar, uint32_t parity) {
+    // try_wait suspends the thread in hardware until the phase completes or the time hint (ns) runs out, so a
+    // waiting warp costs a few issue slots per microsecond instead of spinning against the warps that have work
     asm volatile(
         "{\n\t"
         ".reg .pred p;\n\t"
         "KB_WAIT_%=:\n\t"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1, %2;\n\t"
         "@p bra KB_DONE_%=;\n\t"
         "bra KB_WAIT_%=;\n\t"
         "KB_DONE_%=:\n\t"
-        "}" ::"r"(kb_smem_u32(bar)), "r"(parity) : "memory");
+        "}" ::"r"(kb_smem_u32(bar)), "r"(parity), "r"(2000u) : "memory");
 }
 // generic-proxy writes to shared memory (st.shared) must be ordered before async-proxy (TMA) writes
 __device__ __forceinline__ void kb_fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
