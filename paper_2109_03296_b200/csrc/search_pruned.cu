@@ -97,10 +97,14 @@ struct TensorMaps {
 };
 
 struct BoundParams {
-    float thr[KBMOD_MAX_T + 1];            // pass iff sum (in units) >= thr[m_eff]; thr[0] = 0: always
     unsigned char mkept[KBMOD_MAX_T + 1];  // m(n)
     int pass_all;                          // min_lh <= 0 (or not finite): nothing can be pruned
+    int cbits;                             // width of the two count fields of a plane word: 2^cbits > T
 };
+
+// device-side scalars and tables of the fixed-point planes, written by bound_scale_kernel (floats)
+constexpr int SC_UNIT = 0, SC_INV_UNIT = 1, SC_CAP = 2, SC_FLOOR = 4, SC_THR = SC_FLOOR + KBMOD_MAX_T,
+              SC_FLOATS = SC_THR + KBMOD_MAX_T + 1;
 
 struct Queue {
     uint2* entries;                  // (pixel index y0*W+x0, velocity index); v = 0xFFFFFFFF: hole
@@ -111,78 +115,114 @@ struct Queue {
 
 // ---------------------------------------------------------------------------------------------
 // bound planes: one 32-bit word per pixel, 0 for invalid pixels (and outside the image, by TMA zero fill);
-// row pitch Wp (a multiple of 4 so that TMA boxes start 16-byte aligned).  For a valid pixel
-//     word = ceil(psi_+ / unit) << 14  |  (phi < f) << 7  |  1
-// so that ONE integer add per trajectory-epoch accumulates the fixed-point sum of psi_+ (rounded up), the
-// number of "low" samples and the number of valid samples.  f = 0.8 x the smallest per-epoch mean of phi (a
-// sample); unit = min_lh * sqrt(f) / PR_THR_UNITS.  A term is clamped to 2^12 - 1 units, which alone exceeds
-// the threshold PR_THR_UNITS * sqrt(m) for every m <= 64, so a clamped term always passes.  Any f > 0 and any
-// unit > 0 give a CORRECT bound; these make it tight.
-constexpr int AN_LOW_SHIFT = 7, AN_SUM_SHIFT = 14;
-constexpr float AN_TERM_MAX = 4095.0f;  // 2^12 - 1: 64 terms stay below 2^18
-constexpr float PR_THR_UNITS = 500.0f;
-
-// One block: f = the largest of the candidates (0.40 + 0.02 k) x mean(phi) that at most 3 % of a strided
-// sample of the valid pixels fall below (so that "low" samples stay rare and f stays just under the level of
-// the noisiest epoch); then unit.  scale = {unit, 1/unit, f}.
-constexpr int SC_BINS = 40, SC_SAMPLES = 65536;
-__global__ void bound_scale_kernel(const float2* __restrict__ psiphi, size_t n_px, float min_lh, float* __restrict__ scale) {
+// row pitch Wp (a multiple of 4 so that TMA boxes start 16-byte aligned).  With c = cbits, for a valid pixel
+//     word = ceil(psi_+ / unit) << 2c  |  (phi < f_t) << c  |  1
+// so that ONE integer add per trajectory-epoch accumulates the fixed-point sum of psi_+ (rounded up), the number
+// of "low" samples and the number of valid samples.  f_t = the floor of epoch t: the largest of the candidates
+// (0.40 + 0.02 k) x mean_t(phi) that at most 3 % of a sample of the epoch's valid pixels fall below.
+// A kept set S has at least m(n) members, at most n_low of them low, and the others have phi >= f_t of their
+// epoch, so  sum_S phi >= F(m(n) - n_low),  F(k) = the sum of the k smallest floors of the stack, and
+//     L' <= sum psi_+ / sqrt(F(m(n) - n_low)).
+// In units: pass iff sum >= thr[k] = THR sqrt(F(k) / f_min), unit = min_lh sqrt(f_min) / THR.  A term is clamped
+// to `cap` units (T terms stay inside the sum field) and THR is chosen so that thr[k] <= 0.98 cap for every k:
+// a clamped term passes on its own.  Any floors > 0 and any unit > 0 give a CORRECT bound; these make it tight.
+constexpr int SC_BINS = 40, SC_SAMPLES = 16384;
+__global__ void __launch_bounds__(1024)
+bound_scale_kernel(const float2* __restrict__ psiphi, int T, size_t plane, float min_lh,
+                                   const __grid_constant__ BoundParams BP, float* __restrict__ scale) {
     __shared__ float ssum[32];
     __shared__ int scnt[32];
     __shared__ int hist[SC_BINS + 1];
     __shared__ float s_mean;
-    const size_t n_samp = n_px < SC_SAMPLES ? n_px : SC_SAMPLES, stride = n_px / n_samp;
-    float sum = 0.0f;
-    int cnt = 0;
-    for (size_t k = threadIdx.x; k < n_samp; k += blockDim.x) {
-        const float phi = __ldg(psiphi + k * stride).y;
-        if (phi > 0.0f && phi < CUDART_INF_F) { sum += phi; ++cnt; }
-    }
-    for (int d = 16; d > 0; d >>= 1) {
-        sum += __shfl_down_sync(0xFFFFFFFFu, sum, d);
-        cnt += __shfl_down_sync(0xFFFFFFFFu, cnt, d);
-    }
-    if ((threadIdx.x & 31) == 0) { ssum[threadIdx.x >> 5] = sum; scnt[threadIdx.x >> 5] = cnt; }
-    if (threadIdx.x <= SC_BINS) hist[threadIdx.x] = 0;
-    __syncthreads();
-    if (threadIdx.x == 0) {
-        for (int w = 1; w < (int)(blockDim.x >> 5); ++w) { sum += ssum[w]; cnt += scnt[w]; }
-        scnt[0] = cnt;
-        s_mean = cnt > 0 ? sum / (float)cnt : 0.0f;
-    }
-    __syncthreads();
-    const float mean = s_mean;
-    if (mean > 0.0f && mean < CUDART_INF_F) {
+    __shared__ float floors[KBMOD_MAX_T];
+    const size_t n_samp = plane < SC_SAMPLES ? plane : SC_SAMPLES, stride = plane / n_samp;
+    for (int t = 0; t < T; ++t) {
+        const float2* pl = psiphi + (size_t)t * plane;
+        float sum = 0.0f;
+        int cnt = 0;
         for (size_t k = threadIdx.x; k < n_samp; k += blockDim.x) {
-            const float phi = __ldg(psiphi + k * stride).y;
-            if (phi > 0.0f && phi < CUDART_INF_F) {
-                const float r = (phi / mean - 0.40f) * 50.0f;  // bin k holds [0.40 + 0.02 k, 0.40 + 0.02 (k+1))
-                const int bin = r < 0.0f ? 0 : (r >= (float)SC_BINS ? SC_BINS : 1 + (int)r);
-                atomicAdd(&hist[bin > SC_BINS ? SC_BINS : bin], 1);  // bin 0: below 0.40 x mean
+            const float phi = __ldg(pl + k * stride).y;
+            if (phi > 0.0f && phi < CUDART_INF_F) { sum += phi; ++cnt; }
+        }
+        for (int d = 16; d > 0; d >>= 1) {
+            sum += __shfl_down_sync(0xFFFFFFFFu, sum, d);
+            cnt += __shfl_down_sync(0xFFFFFFFFu, cnt, d);
+        }
+        __syncthreads();  // the previous epoch's hist / s_mean are no longer read
+        if ((threadIdx.x & 31) == 0) { ssum[threadIdx.x >> 5] = sum; scnt[threadIdx.x >> 5] = cnt; }
+        if (threadIdx.x <= SC_BINS) hist[threadIdx.x] = 0;
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            for (int w = 1; w < (int)(blockDim.x >> 5); ++w) { sum += ssum[w]; cnt += scnt[w]; }
+            scnt[0] = cnt;
+            s_mean = cnt > 0 ? sum / (float)cnt : 0.0f;
+        }
+        __syncthreads();
+        const float mean = s_mean;
+        const bool usable = mean > 0.0f && mean < CUDART_INF_F;
+        if (usable) {
+            for (size_t k = threadIdx.x; k < n_samp; k += blockDim.x) {
+                const float phi = __ldg(pl + k * stride).y;
+                if (phi > 0.0f && phi < CUDART_INF_F) {
+                    const float r = (phi / mean - 0.40f) * 50.0f;  // bin 1 + k holds [0.40 + 0.02 k, 0.40 + 0.02 (k+1))
+                    const int bin = r < 0.0f ? 0 : (r >= (float)(SC_BINS - 1) ? SC_BINS : 1 + (int)r);
+                    atomicAdd(&hist[bin], 1);  // bin 0: below 0.40 x mean
+                }
             }
         }
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            float f = 0.0f;  // 0: this epoch has no usable sample; it gets the smallest floor of the others
+            if (usable) {
+                const int budget = (int)(0.03f * (float)scnt[0]);
+                int below = hist[0], k = 0;  // below = samples under 0.40 + 0.02 k
+                while (k + 1 < SC_BINS && below + hist[k + 1] <= budget) { below += hist[k + 1]; ++k; }
+                f = (0.40f + 0.02f * (float)k) * mean;
+                if (!(f > 1e-30f) || !(f < 1e30f)) f = 0.0f;
+            }
+            floors[t] = f;
+        }
     }
     __syncthreads();
     if (threadIdx.x == 0) {
-        float f = 1.0f;
-        if (mean > 0.0f && mean < CUDART_INF_F) {
-            const int budget = (int)(0.03f * (float)scnt[0]);
-            int below = hist[0], k = 0;  // below = samples under 0.40 + 0.02 k
-            while (k + 1 < SC_BINS && below + hist[k + 1] <= budget) { below += hist[k + 1]; ++k; }
-            f = (0.40f + 0.02f * (float)k) * mean;
+        float fmin = CUDART_INF_F;
+        for (int t = 0; t < T; ++t)
+            if (floors[t] > 0.0f) fmin = fminf(fmin, floors[t]);
+        if (!(fmin < CUDART_INF_F)) fmin = 1.0f;
+        for (int t = 0; t < T; ++t) {
+            if (!(floors[t] > 0.0f)) floors[t] = fmin;
+            scale[SC_FLOOR + t] = floors[t];
         }
-        if (!(f > 1e-30f) || !(f < 1e30f)) f = 1.0f;
+        // F(k): sum of the k smallest floors (insertion sort, T <= 64)
+        for (int i = 1; i < T; ++i) {
+            const float key = floors[i];
+            int j = i - 1;
+            while (j >= 0 && floors[j] > key) { floors[j + 1] = floors[j]; --j; }
+            floors[j + 1] = key;
+        }
+        float Fk = 0.0f, ratio[KBMOD_MAX_T + 1];
+        ratio[0] = 0.0f;
+        for (int k = 1; k <= KBMOD_MAX_T; ++k) {
+            if (k <= T) Fk += floors[k - 1] * 0.999999f;  // rounded down
+            ratio[k] = sqrtf(Fk / fmin);
+        }
+        const int sum_bits = 32 - 2 * BP.cbits;
+        const float cap = floorf((float)((1u << sum_bits) - 1u) / (float)T);
+        const float thr_units = 0.98f * cap / fmaxf(ratio[T], 1.0f);
         const float ml = (min_lh > 0.0f && min_lh < CUDART_INF_F) ? min_lh : 1.0f;
-        float unit = ml * sqrtf(f) / PR_THR_UNITS;
+        float unit = ml * sqrtf(fmin) / thr_units;
         if (!(unit > 1e-30f) || !(unit < 1e30f)) unit = 1.0f;
-        scale[0] = unit;
-        scale[1] = 1.0f / unit;
-        scale[2] = f;
+        scale[SC_UNIT] = unit;
+        scale[SC_INV_UNIT] = 1.0f / unit;
+        scale[SC_CAP] = cap;
+        // U = sum * unit / sqrt(F(k)) >= min_lh  <=>  sum >= thr_units * sqrt(F(k) / fmin); slack for float32 rounding
+        for (int k = 0; k <= KBMOD_MAX_T; ++k) scale[SC_THR + k] = thr_units * ratio[k] * (1.0f - 1e-4f);
+        scale[SC_THR] = 0.0f;  // no epoch is known to have phi >= its floor: no bound, always pass
     }
 }
 
-__global__ void bound_plane_kernel(const float2* __restrict__ psiphi, unsigned int* __restrict__ B, int W, int Wp,
-                                   size_t rows /* T*H */, const float* __restrict__ scale) {
+__global__ void bound_plane_kernel(const float2* __restrict__ psiphi, unsigned int* __restrict__ B, int H, int W, int Wp,
+                                   size_t rows /* T*H */, int cbits, const float* __restrict__ scale) {
     const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= rows * (size_t)Wp) return;
     const size_t r = i / Wp;
@@ -192,10 +232,11 @@ __global__ void bound_plane_kernel(const float2* __restrict__ psiphi, unsigned i
         const float2 s = __ldg(psiphi + r * W + x);
         if (s.y > 0.0f) {
             // rounded up twice over: the factor covers the float32 product, ceilf the quantisation
-            const float t = fmaxf(s.x, 0.0f) * __ldg(scale + 1) * 1.000001f;
-            const unsigned int fix = (t < AN_TERM_MAX) ? (unsigned int)ceilf(t) : (unsigned int)AN_TERM_MAX;  // inf, too
-            const unsigned int low = (s.y < __ldg(scale + 2)) ? 1u : 0u;
-            o = (fix << AN_SUM_SHIFT) | (low << AN_LOW_SHIFT) | 1u;
+            const float t = fmaxf(s.x, 0.0f) * __ldg(scale + SC_INV_UNIT) * 1.000001f;
+            const float cap = __ldg(scale + SC_CAP);
+            const unsigned int fix = (t < cap) ? (unsigned int)ceilf(t) : (unsigned int)cap;  // inf, too
+            const unsigned int low = (s.y < __ldg(scale + SC_FLOOR + (int)(r / (size_t)H))) ? 1u : 0u;
+            o = (fix << (2 * cbits)) | (low << cbits) | 1u;
         }
     }
     B[i] = o;
@@ -230,7 +271,7 @@ __device__ __forceinline__ void tile_origin(int tile_lin, int tiles_x, int tiles
 __global__ void __launch_bounds__(PR_THREADS, 1)
 bound_phase_kernel(const __grid_constant__ TensorMaps maps, int T, int H, int W, int tile_begin, int tile_end,
                    const __grid_constant__ PrunedTables tb, const __grid_constant__ BoundParams BP, int min_obs,
-                   const __grid_constant__ Queue Qu) {
+                   const float* __restrict__ scale, const __grid_constant__ Queue Qu) {
     extern __shared__ __align__(1024) unsigned char smem[];
     const int TBL = tbl_bytes(T);
     unsigned char* tblbase = smem + tb.ring_bytes;
@@ -412,6 +453,8 @@ bound_phase_kernel(const __grid_constant__ TensorMaps maps, int T, int H, int W,
             const uint32_t vmask = __ldg(reinterpret_cast<const uint32_t*>(tb.gtbl + (size_t)g * TBL + (size_t)T * PR_G * 4 +
                                                                             offsetof(GroupEpoch, vmask)));
             int my_cnt = 0;
+            const unsigned int cmask = (1u << BP.cbits) - 1u;
+            const float* thr = scale + SC_THR;
 #pragma unroll
             for (int h = 0; h < PR_PIX; ++h) {
                 const bool in_img = (px0 + 32 * (h & 1)) < W && (py0 + 16 * (h >> 1)) < H;
@@ -419,10 +462,10 @@ bound_phase_kernel(const __grid_constant__ TensorMaps maps, int T, int H, int W,
 #pragma unroll
                 for (int j = 0; j < PR_G; ++j) {
                     const unsigned int an = AN[h][j] + ANU[h];
-                    const int n = (int)(an & 127u), n_low = (int)((an >> AN_LOW_SHIFT) & 127u);
-                    // at least m(n) epochs are kept, at least m(n) - n_low of them with phi >= f
+                    const int n = (int)(an & cmask), n_low = (int)((an >> BP.cbits) & cmask);
+                    // at least m(n) epochs are kept, at least m(n) - n_low of them with phi >= their epoch's floor
                     const int m_eff = max((int)BP.mkept[n] - n_low, 0);
-                    const bool pass = BP.pass_all || (float)(an >> AN_SUM_SHIFT) >= BP.thr[m_eff];
+                    const bool pass = BP.pass_all || (float)(an >> (2 * BP.cbits)) >= __ldg(thr + m_eff);
                     if (in_img && n >= need && pass && (KB_EXPERIMENT != 2 || Qu.cap == ~0ull)) m[h] |= 1u << j;
                 }
                 m[h] &= vmask;
@@ -717,7 +760,7 @@ WsLayout ws_layout(int T, int H, int W, int n_vel, int K) {
     L.B = o;        o += al256((size_t)T * H * Wp * 4);
     L.keys = o;     o += al256((size_t)H * W * K * 8);
     L.qentries = o; o += al256(queue_cap(n_vel) * 8);
-    L.qcount = o;   o += 256;
+    L.qcount = o;   o += 256 + al256(SC_FLOATS * sizeof(float));  // queue counter, then the scale table
     L.overflow_words = (n_tiles_of(H, W) * ngm * (PR_CONSUMERS / 32) + 31) / 32;
     L.overflow = o; o += al256(L.overflow_words * 4);
     L.total = o;
@@ -741,11 +784,10 @@ static bool bound_min_kept(const kbmod_search_params* p, const DevParams& P, int
             else return false;
         }
         bp->mkept[n] = (unsigned char)(n == 0 ? 0 : m);
-        // U = sum * unit / sqrt(m f) >= min_lh  <=>  sum >= PR_THR_UNITS * sqrt(m); slack for float32 rounding
-        bp->thr[n] = (float)(PR_THR_UNITS * sqrt((double)n) * (1.0 - 1e-4));
     }
-    bp->thr[0] = 0.0f;  // no epoch is known to have phi >= f: no bound
     bp->pass_all = !(p->min_lh > 0.0f && p->min_lh < INFINITY);
+    bp->cbits = 1;
+    while ((1 << bp->cbits) <= T) ++bp->cbits;  // counts up to T fit: 2^cbits > T  (T = 26 -> 5, T = 64 -> 7)
     return true;
 }
 
@@ -847,7 +889,7 @@ int kb_launch_search_pruned(const float* d_psiphi, int T, int TPv, int H, int W,
     Queue Qu;
     Qu.entries = (uint2*)(w + L.qentries);
     Qu.count = (unsigned long long*)(w + L.qcount);
-    float* d_scale = (float*)(w + L.qcount + 64);  // {unit, 1/unit, f} of the fixed-point bound planes
+    float* d_scale = (float*)(w + L.qcount + 256);  // unit, cap, floors and thresholds of the fixed-point bound planes
     Qu.cap = queue_cap(n_vel);
     Qu.overflow = (unsigned int*)(w + L.overflow);
 
@@ -879,9 +921,10 @@ int kb_launch_search_pruned(const float* d_psiphi, int T, int TPv, int H, int W,
     int launches = 0;
     {
         const size_t n = (size_t)T * H * Wp;
-        bound_scale_kernel<<<1, 1024, 0, st>>>(reinterpret_cast<const float2*>(d_psiphi), (size_t)T * H * W, P.min_lh, d_scale);
-        bound_plane_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(reinterpret_cast<const float2*>(d_psiphi), d_B, W,
-                                                                        (int)Wp, (size_t)T * H, d_scale);
+        bound_scale_kernel<<<1, 1024, 0, st>>>(reinterpret_cast<const float2*>(d_psiphi), T, (size_t)H * W, P.min_lh, bp, d_scale);
+        bound_plane_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(reinterpret_cast<const float2*>(d_psiphi), d_B, H, W,
+                                                                        (int)Wp, (size_t)T * H, bp.cbits, d_scale);
+        KB_CUDA(cudaGetLastError());
         launches += 2;
         kb_phase_mark(KB_PHASE_PLANES, st);
     }
@@ -908,7 +951,7 @@ int kb_launch_search_pruned(const float* d_psiphi, int T, int TPv, int H, int W,
             for (int b0 = 0; b0 < n_tiles; b0 += batch) {
                 const int b1 = std::min(n_tiles, b0 + batch);
                 KB_CUDA(cudaMemsetAsync(Qu.count, 0, sizeof(unsigned long long), st));
-                bound_phase_kernel<<<std::min(grid, b1 - b0), PR_THREADS, smem1, st>>>(maps, T, H, W, b0, b1, tb, bp, P.min_obs, Qu);
+                bound_phase_kernel<<<std::min(grid, b1 - b0), PR_THREADS, smem1, st>>>(maps, T, H, W, b0, b1, tb, bp, P.min_obs, d_scale, Qu);
                 kb_phase_mark(KB_PHASE_BOUND, st);
                 exact_queue_kernel<TP><<<n_sm * 4, EX_THREADS, smem2, st>>>(psiphi2, H, W, d_tab, P, Qu, d_keys, d_stats);
                 kb_phase_mark(KB_PHASE_EXACT, st);
