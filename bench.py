@@ -181,11 +181,11 @@ def run_reference(args):
 #   direct kernel  : bound "alu" -- every trajectory runs the compare-exchange network; the algorithmic
 #                    lane-operations per trajectory are 2*CE(T) min/max + per epoch 1 gather, 1 divide,
 #                    2 window compares, 2 adds, 1 count = 2*CE(T) + 7*T; peak = 148 SMs x 128 lanes x f_max.
-#   pruned path    : bound "smem" -- SURVEY 8(d)'s per-unit figure: 8 B (psi, phi as float32) per
-#                    trajectory-epoch evaluation gathered from shared memory; peak = 148 SMs x 128 B/clk x f_max.
-#                    The dominant kernel is bound_phase_kernel; its duration is measured live with CUDA events
-#                    recorded by the library on the launching stream (kbmod_search_phase_ms).  The kernel itself
-#                    moves 4 B per evaluation: `smem_bytes_per_eval_actual`.
+#   pruned path    : bound "smem" -- the dominant kernel, bound_phase_kernel, gathers one packed 32-bit word
+#                    (fixed-point psi_+ | low-phi flag | valid flag) per trajectory-epoch evaluation from shared
+#                    memory: 4 B algorithmic; peak = 148 SMs x 128 B/clk x f_max.  Its duration is measured live
+#                    with CUDA events recorded by the library on the launching stream (kbmod_search_phase_ms).
+#                    SURVEY 8(d) counted 8 B per evaluation (psi and phi as float32): reported beside it.
 # dram__bytes_read.sum + dram__bytes_write.sum per step of the dominant kernel from the committed ncu --set full
 # capture (profiles/); None = not captured for this kernel
 TRAFFIC = {"bound_phase_kernel": None, "search_direct_kernel": None}
@@ -274,6 +274,20 @@ def run_ours(args):
                 n_cand=n_cand, out=out)
 
 
+def max_over_ranks(ms_local: float, dist, device, world: int) -> float:
+    """Device time of the timed region: the MAX over ranks (every rank gets it)."""
+    import torch
+    t = torch.tensor([ms_local], dtype=torch.float64, device=device)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_value(evals_per_rank: float, world: int, ms_per_step: float) -> float:
+    """Replicas only: every rank processes its own stack, so the job did world x evals in ms_per_step."""
+    return world * evals_per_rank / (ms_per_step * 1e-3)
+
+
 def run_e2e(R, steps):
     """Same metric end to end through the C-ABI call with HOST buffers (kbmod_pipeline_host): every step
     copies the image/variance/mask stacks from pinned host memory, runs prep + search, and reads the four
@@ -305,19 +319,14 @@ def report(R, args):
     torch, dist, kb = R["torch"], R["dist"], R["kb"]
     rank, world = R["rank"], R["world"]
     # max over ranks of the device time of the timed region
-    tmax = torch.tensor([R["total_ms"]], dtype=torch.float64, device=R["dev"])
-    if world > 1:
-        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
-    total_ms = float(tmax.item())
+    total_ms = max_over_ranks(R["total_ms"], dist, R["dev"], world)
     e2e_steps = max(1, min(args.steps, 3))
     e2e_ms, h2d, d2h, same = run_e2e(R, e2e_steps)
-    emax = torch.tensor([e2e_ms], dtype=torch.float64, device=R["dev"])
-    if world > 1:
-        dist.all_reduce(emax, op=dist.ReduceOp.MAX)
+    e2e_max = max_over_ranks(e2e_ms, dist, R["dev"], world)
     if rank != 0:
         return
     ms_per_step = total_ms / args.steps
-    value = world * R["evals"] / (ms_per_step * 1e-3)
+    value = whole_job_value(R["evals"], world, ms_per_step)
     st, sp, peaks = R["st"], R["sp"], R["peaks"]
     T, H, W = st.img.shape
     n_vel = len(R["vx"])
@@ -333,12 +342,15 @@ def report(R, args):
                     unit="Tlane-op/s", kernel="search_direct_kernel",
                     peak_source="derived: 148 SMs x 128 FP32/ALU lanes x sm_max_mhz (DESIGN.md)")
     else:
-        byts = R["evals"] * 8.0
-        roof = dict(bound="smem", achieved=byts / (kernel_ms * 1e-3) / 1e9, peak=N_SM * 128 * f_max / 1e9,
+        byts = R["evals"] * 4.0  # one packed 32-bit bound word per trajectory-epoch evaluation
+        peak = N_SM * 128 * f_max / 1e9
+        roof = dict(bound="smem", achieved=byts / (kernel_ms * 1e-3) / 1e9, peak=peak,
                     unit="GB/s", kernel="bound_phase_kernel",
                     peak_source="derived: 148 SMs x 128 B/clk shared-memory bandwidth x sm_max_mhz (DESIGN.md)",
-                    algorithmic_bytes_per_eval=8, smem_bytes_per_eval_actual=4,
-                    whole_search_frac=byts / (search_ms * 1e-3) / 1e9 / (N_SM * 128 * f_max / 1e9))
+                    algorithmic_bytes_per_eval=4,
+                    # SURVEY 8(d) counted 8 B (psi, phi as float32) per evaluation; against that figure:
+                    frac_of_survey_8B_roofline=2.0 * byts / (kernel_ms * 1e-3) / 1e9 / peak,
+                    whole_search_frac_of_survey_8B_roofline=2.0 * byts / (search_ms * 1e-3) / 1e9 / peak)
     roof["frac"] = roof["achieved"] / roof["peak"]
     roof["traffic"] = TRAFFIC.get(roof["kernel"])
     roof["kernel_ms"] = kernel_ms
@@ -359,8 +371,8 @@ def report(R, args):
                 segments_ms={k: float(np.mean(v)) for k, v in R["seg"].items()},
                 evaluated_fraction=evaluated / max(1, nominal),
                 roofline=roof, cpu_baseline=cpu,
-                e2e=dict(value=world * R["evals"] / (float(emax.item()) * 1e-3), unit=UNIT, h2d_bytes_per_step=h2d,
-                         d2h_bytes_per_step=d2h, ms_per_step=float(emax.item()), steps=e2e_steps,
+                e2e=dict(value=whole_job_value(R["evals"], world, e2e_max), unit=UNIT, h2d_bytes_per_step=h2d,
+                         d2h_bytes_per_step=d2h, ms_per_step=e2e_max, steps=e2e_steps,
                          matches_resident_run=same, api="kbmod_pipeline_host (prep + search; host buffers pinned)"),
                 gpu_launches=args.steps * (T + int(launches) + 1), clocks=R["clocks"], peaks_source=peaks["source"])
     print(json.dumps(line), flush=True)

@@ -27,6 +27,7 @@
 //   exact_overflow_kernel  pairs of (tile, group, warp) items that did not fit the queue, all evaluated.
 //   finalize_kernel      keys -> the four output arrays.
 #include <stddef.h>
+#include <stdlib.h>
 
 #include <algorithm>
 #include <vector>
@@ -742,6 +743,11 @@ size_t max_groups(int n_vel) {
     return std::min((size_t)n_vel, 2 * full + 16);
 }
 size_t queue_cap(int n_vel) {
+    // test hook: KBMOD_B200_QUEUE_CAP=<entries> shrinks the survivor queue so that the overflow path runs
+    if (const char* e = getenv("KBMOD_B200_QUEUE_CAP")) {
+        const long long v = atoll(e);
+        if (v > 0) return (size_t)std::max<long long>(64, v);
+    }
     const double want = 1100.0 * PR_TW * PR_TH * (double)n_vel / 32.0;
     return (size_t)std::min(268435456.0, std::max(1048576.0, want));
 }

@@ -330,3 +330,92 @@ def test_search_config3_full_size_sampled(kb, oracle):
     ev, nominal, _, algo = kb.kbmod_search_stats(kb.kbmod_search.last_workspace)
     assert algo == kb.ALGO_PRUNED and nominal == H * W * len(vx)
     assert r["n_entries"] > 500, r
+
+
+# ------------------------------------------------------------------------------------------- round-1 additions
+def test_search_pruned_queue_overflow_path(kb, oracle, monkeypatch):
+    """A survivor queue of 64 entries (test hook KBMOD_B200_QUEUE_CAP) overflows at once: almost every
+    (tile, group, warp) item goes through the overflow bitmap and exact_overflow_kernel.  Same results."""
+    import torch
+    st = synth.random_stack(81, 9, 70, 150, mask_frac=0.05, t_span=1.5)
+    rng = np.random.default_rng(81)
+    vx = rng.uniform(-20, 20, 40).astype(np.float32)
+    vy = rng.uniform(-20, 20, 40).astype(np.float32)
+    d = _prep(kb, st)
+    sp = kb.SearchParams(K=4, min_obs=3, min_lh=2.0, algo=kb.ALGO_PRUNED)
+    ref = [o.clone() for o in kb.kbmod_search(d, st.times, vx, vy, sp)]
+    monkeypatch.setenv("KBMOD_B200_QUEUE_CAP", "64")
+    small = [o.clone() for o in kb.kbmod_search(d, st.times, vx, vy, sp)]
+    monkeypatch.delenv("KBMOD_B200_QUEUE_CAP")
+    for a, b in zip(ref, small):
+        assert torch.equal(a, b)
+    r = _search_and_compare(kb, oracle, d, st.times, vx, vy, sp)
+    assert r["n_entries"] > 100
+
+
+def test_search_phase_timing_api(kb):
+    st = synth.config1_tiny()
+    vx, vy = synth.config1_grid()
+    d = _prep(kb, st)
+    kb.kbmod_search_phase_timing(True)
+    try:
+        for algo, keys in ((kb.ALGO_PRUNED, ("planes", "gather", "exact", "finalize")), (kb.ALGO_DIRECT, ("gather",))):
+            kb.kbmod_search(d, st.times, vx, vy, kb.SearchParams(K=1, min_obs=3, min_lh=10.0, algo=algo))
+            ms = kb.kbmod_search_phase_ms()
+            assert all(ms[k] > 0.0 for k in keys), ms
+            assert all(v >= 0.0 for v in ms.values())
+    finally:
+        kb.kbmod_search_phase_timing(False)
+
+
+def test_search_pruned_equals_direct_heavy_shaped(kb):
+    """BASELINE configs[3] shape (T = 50 over 6 nights, K = 16, min_obs = 25, sub-threshold movers) scaled to
+    512x320 with a 64 x 32 slice of the velocity grid: both kernels must return identical arrays."""
+    import torch
+    st = synth.decam_stack(7, (9, 8, 8, 9, 8, 8), H=512, W=320, n_movers=60, flux_range=(10.0, 100.0), flux_log=False,
+                           n_stars=30, name="heavy_small")
+    vx, vy = synth.config3_grid(64, 32)
+    d = _prep(kb, st)
+    outs = {}
+    for name, algo in (("direct", kb.ALGO_DIRECT), ("pruned", kb.ALGO_PRUNED)):
+        sp = kb.SearchParams(K=16, min_obs=25, min_lh=6.0, algo=algo)
+        outs[name] = [o.clone() for o in kb.kbmod_search(d, st.times, vx, vy, sp)]
+    for a, b in zip(outs["direct"], outs["pruned"]):
+        assert torch.equal(a, b)
+    assert int((outs["pruned"][2] >= 0).sum()) > 50
+
+
+def test_config5_full_size_coadd_and_refilter(kb, oracle):
+    """BASELINE configs[4] at full size: 10^5 candidate trajectories on the 2048x4096x26 stack, 21x21 mean and
+    median stamps (oracle on a sample of 1500 trajectories), lightcurves with 20 % of the epochs replaced by
+    10-sigma outliers, sigma-G rerun (oracle on all 10^5): kept sets bit-exact, >= 99 % of the outliers dropped
+    among lightcurves that keep enough clean epochs."""
+    st = synth.config3_decam()
+    T, H, W = st.img.shape
+    n = 100_000
+    x0, y0, vx, vy = synth.config5_trajectories(4, H, W, n)
+    img, mask = _cuda(st.img), _cuda(st.mask)
+    gm, gd = kb.kbmod_coadd_stamps(img, mask, st.times, _cuda(x0), _cuda(y0), _cuda(vx), _cuda(vy), 10)
+    pick = np.random.default_rng(5).choice(n, 1500, replace=False)
+    om, od = oracle.coadd_stamps(st.img, st.mask, st.times, x0[pick], y0[pick], vx[pick], vy[pick], 10)
+    gm, gd = gm[_cuda(pick)].cpu().numpy(), gd[_cuda(pick)].cpu().numpy()
+    assert np.array_equal(gd, od.astype(np.float32))
+    assert np.all(np.abs(gm - om) <= 1e-5 * np.abs(om) + 1e-4)
+    # lightcurves of the same candidates
+    d = _prep(kb, st)
+    sp = kb.SearchParams(K=1, min_obs=13)
+    ev = {k: v.cpu().numpy() for k, v in
+          kb.kbmod_eval_trajectories(d, st.times, _cuda(x0), _cuda(y0), _cuda(vx), _cuda(vy), sp).items()}
+    psi, hit = synth.outlier_lightcurves(6, ev["psi_lc"], ev["phi_lc"], 0.2, 10.0)
+    g = {k: v.cpu().numpy() for k, v in kb.kbmod_sigmag_filter(_cuda(psi), _cuda(ev["phi_lc"]), sp).items()}
+    o = oracle.sigmag_filter(psi, ev["phi_lc"], parity.oracle_params(oracle, sp))
+    assert np.array_equal(g["kept"].view(np.uint64), o["kept"])
+    has = o["n_kept"] > 0
+    tl, tf = parity.score_tolerances(dict(o, psi_lc=psi, phi_lc=ev["phi_lc"]), T)
+    assert np.all(np.abs(g["lh"][has] - o["lh"][has]) <= tl[has])
+    assert np.all(np.abs(g["flux"][has] - o["flux"][has]) <= tf[has])
+    valid = ev["phi_lc"] > 0
+    kept = ((o["kept"][:, None] >> np.arange(T, dtype=np.uint64)[None, :]) & np.uint64(1)).astype(bool)
+    few = has & ((hit & valid).sum(1) <= 5) & (valid.sum(1) >= 20)  # the 25/75 percentiles stay on clean epochs
+    dropped = (hit & valid & ~kept)[few].sum() / max(1, (hit & valid)[few].sum())
+    assert few.sum() > 10_000 and dropped >= 0.99, (int(few.sum()), float(dropped))
