@@ -26,6 +26,7 @@
 //                        top-K through a cascade of 64-bit atomicMax on (orderable L', ~vel_idx) keys.
 //   exact_overflow_kernel  pairs of (tile, group, warp) items that did not fit the queue, all evaluated.
 //   finalize_kernel      keys -> the four output arrays.
+#include <math.h>
 #include <stddef.h>
 #include <stdlib.h>
 
@@ -34,17 +35,6 @@
 
 #include "common.cuh"
 #include "tma.cuh"
-
-// timing experiments (never defined in the product build): 1 = consumers skip the gathers (producer / TMA
-// limited time), 2 = the producer stages only the tables (consumer limited time; results are garbage)
-#ifndef KB_EXPERIMENT
-#define KB_EXPERIMENT 0
-#endif
-#if KB_EXPERIMENT == 1
-#define KB_EXP1_GUARD if (false)
-#else
-#define KB_EXP1_GUARD
-#endif
 
 namespace {
 
@@ -271,6 +261,7 @@ __device__ __forceinline__ void tile_origin(int tile_lin, int tiles_x, int tiles
 // phase 1: bounds from shared-memory tiles; survivors -> queue
 __global__ void __launch_bounds__(PR_THREADS, 1)
 bound_phase_kernel(const __grid_constant__ TensorMaps maps, int T, int H, int W, int tile_begin, int tile_end,
+                   int g_begin, int g_end,
                    const __grid_constant__ PrunedTables tb, const __grid_constant__ BoundParams BP, int min_obs,
                    const float* __restrict__ scale, const __grid_constant__ Queue Qu) {
     extern __shared__ __align__(1024) unsigned char smem[];
@@ -304,8 +295,8 @@ bound_phase_kernel(const __grid_constant__ TensorMaps maps, int T, int H, int W,
         const uint32_t ring = (uint32_t)tb.ring_bytes;
         int4 nxt0 = make_int4(0, 0, 0, 0);
         uint32_t nxt_fp = 0;
-        if (ng > 0) {
-            const GroupEpoch* nge = reinterpret_cast<const GroupEpoch*>(tb.gtbl + (size_t)T * PR_G * 4);
+        if (g_begin < g_end) {
+            const GroupEpoch* nge = reinterpret_cast<const GroupEpoch*>(tb.gtbl + (size_t)g_begin * TBL + (size_t)T * PR_G * 4);
             nxt0 = __ldg(reinterpret_cast<const int4*>(nge));
             nxt_fp = __ldg(&nge->footprint);
         }
@@ -318,7 +309,7 @@ bound_phase_kernel(const __grid_constant__ TensorMaps maps, int T, int H, int W,
                 ++oldest;
             }
             used = 0;
-            for (int g = 0; g < ng; ++g, ++gcount) {
+            for (int g = g_begin; g < g_end; ++g, ++gcount) {
                 qs0 = qs1; qs1 = qs2; qs2 = qs3; qs3 = q;
                 const unsigned char* gt = tb.gtbl + (size_t)g * TBL;
                 // the first epoch's entry was fetched from global memory one group ago (nxt0 / nxt_fp); the other
@@ -350,16 +341,12 @@ bound_phase_kernel(const __grid_constant__ TensorMaps maps, int T, int H, int W,
                     used += fp;
                     const int pitch = PR_TW + 16 * pitch_k;
                     const uint32_t box_bytes = (uint32_t)pitch * PR_RB * sizeof(unsigned int);
-#if KB_EXPERIMENT == 2
-                    kb_mbar_expect_tx(&full[slot], (t == 0 ? (uint32_t)TBL : 0u));
-#else
                     kb_mbar_expect_tx(&full[slot], box_bytes * n_box + (t == 0 ? (uint32_t)TBL : 0u));
-#endif
                     if (t == 0) kb_bulk_load_1d(tblbase + (gcount & (PR_NTBL - 1)) * TBL, gt, (uint32_t)TBL, &full[slot]);
                     unsigned char* dst = smem + (uint32_t)e0.w;
                     // the region's rows (a multiple of 8) as the fewest boxes of 64, 32, 16 or 8 rows: the producer is a
                     // single thread and every instruction it issues competes with four busy consumer warps
-                    int left = (KB_EXPERIMENT == 2) ? 0 : n_box, done = 0;
+                    int left = n_box, done = 0;
                     while (left > 0) {
                         const int hc = left >= 8 ? 3 : (left >= 4 ? 2 : (left >= 2 ? 1 : 0));
                         kb_tma_load_3d(dst + (size_t)done * box_bytes, &maps.m[hc * PR_NPITCH + pitch_k], tile_x0 + e0.x,
@@ -369,7 +356,7 @@ bound_phase_kernel(const __grid_constant__ TensorMaps maps, int T, int H, int W,
                     }
                     ++q;
                     if (t == 0) {  // fetch the next group's first entry now: a whole group of time to arrive
-                        const int gn = (g + 1 < ng) ? g + 1 : 0;
+                        const int gn = (g + 1 < g_end) ? g + 1 : g_begin;
                         const GroupEpoch* nge = reinterpret_cast<const GroupEpoch*>(tb.gtbl + (size_t)gn * TBL + (size_t)T * PR_G * 4);
                         nxt0 = __ldg(reinterpret_cast<const int4*>(nge));
                         nxt_fp = __ldg(&nge->footprint);
@@ -389,7 +376,7 @@ bound_phase_kernel(const __grid_constant__ TensorMaps maps, int T, int H, int W,
         tile_origin(tile_lin, tiles_x, tiles_y, tile_x0, tile_y0);
         const int px0 = tile_x0 + lane, py0 = tile_y0 + warp;  // this thread's pixels: (px0, py0), (px0+32, py0)
 
-        for (int g = 0; g < ng; ++g, ++gcount) {
+        for (int g = g_begin; g < g_end; ++g, ++gcount) {
             const unsigned char* tblp = tblbase + (gcount & (PR_NTBL - 1)) * TBL;
             const int4* offs4 = reinterpret_cast<const int4*>(tblp);
             const GroupEpoch* ge = reinterpret_cast<const GroupEpoch*>(tblp + (size_t)T * PR_G * 4);
@@ -415,12 +402,7 @@ bound_phase_kernel(const __grid_constant__ TensorMaps maps, int T, int H, int W,
                 const int pitch = PR_TW + 16 * (int)(cur.x & 0xFFu);
                 const unsigned char* base = smem + cur.y + (size_t)(warp * pitch + lane) * sizeof(unsigned int);
                 const int rows16 = 16 * pitch * (int)sizeof(unsigned int);  // this thread's second row of pixels
-#if KB_EXPERIMENT == 1
-                if (false) {
-                } else if (false) {
-#else
                 if (cur.x & 0x100u) {
-#endif
                     const unsigned char* p = base + offs4[t * (PR_G / 4)].x;
 #pragma unroll
                     for (int v = 0; v < PR_TH / 16; ++v) {
@@ -428,7 +410,7 @@ bound_phase_kernel(const __grid_constant__ TensorMaps maps, int T, int H, int W,
                         ANU[2 * v] += pv[0];
                         ANU[2 * v + 1] += pv[32];
                     }
-                } else KB_EXP1_GUARD {
+                } else {
 #pragma unroll
                     for (int k = 0; k < PR_G / 4; ++k) {
                         const int4 o = offs4[t * (PR_G / 4) + k];  // byte offsets inside the region
@@ -467,7 +449,7 @@ bound_phase_kernel(const __grid_constant__ TensorMaps maps, int T, int H, int W,
                     // at least m(n) epochs are kept, at least m(n) - n_low of them with phi >= their epoch's floor
                     const int m_eff = max((int)BP.mkept[n] - n_low, 0);
                     const bool pass = BP.pass_all || (float)(an >> (2 * BP.cbits)) >= __ldg(thr + m_eff);
-                    if (in_img && n >= need && pass && (KB_EXPERIMENT != 2 || Qu.cap == ~0ull)) m[h] |= 1u << j;
+                    if (in_img && n >= need && pass) m[h] |= 1u << j;
                 }
                 m[h] &= vmask;
                 my_cnt += __popc(m[h]);
@@ -837,6 +819,20 @@ int kb_launch_search_pruned(const float* d_psiphi, int T, int TPv, int H, int W,
     if (n_vel > 0) pl.split(0, n_vel);
     const int ng = (int)pl.leaves.size();
     const size_t ngm = max_groups(n_vel);
+    // launches cover (a batch of whole waves of tiles) x (a chunk of the groups), sized so that 1/4 of the launch's
+    // trajectories fit the survivor queue (what does not fit is evaluated wholesale by the overflow kernel)
+    int n_sm = 148;
+    if (!plan_only) {
+        int dev = 0;
+        KB_CUDA(cudaGetDevice(&dev));
+        KB_CUDA(cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev));
+    }
+    const int n_tiles = (int)n_tiles_of(H, W);
+    const int grid = std::max(1, std::min(n_sm, n_tiles));
+    const double budget = 4.0 * (double)queue_cap(n_vel);
+    const double wave_nominal = (double)grid * PR_TW * PR_TH * (double)ng * PR_G;  // one wave, all groups
+    const int n_chunks = std::max(1, std::min(std::max(ng, 1), (int)ceil(wave_nominal / budget)));
+    const int groups_per_chunk = std::max(1, (ng + n_chunks - 1) / n_chunks);
 
     // ---- tables: gvel, per-group blocks {offs[T][G], ge[T]}, ring chain
     std::vector<int32_t> gvel((size_t)ng * PR_G, -1);
@@ -844,6 +840,7 @@ int kb_launch_search_pruned(const float* d_psiphi, int T, int TPv, int H, int W,
     double staged = 0.0, evals = 0.0;
     uint32_t ph = 0;
     for (int g = 0; g < ng; ++g) {
+        if (g % groups_per_chunk == 0) ph = 0;  // a launch starts its ring chain at offset 0
         const int lo = pl.leaves[g].first, cnt = pl.leaves[g].second - pl.leaves[g].first;
         for (int j = 0; j < cnt; ++j) gvel[(size_t)g * PR_G + j] = pl.idx[lo + j];
         int32_t* offs = reinterpret_cast<int32_t*>(gtbl.data() + (size_t)g * TBL);
@@ -934,16 +931,8 @@ int kb_launch_search_pruned(const float* d_psiphi, int T, int TPv, int H, int W,
         launches += 2;
         kb_phase_mark(KB_PHASE_PLANES, st);
     }
-    int dev = 0, n_sm = 0;
-    KB_CUDA(cudaGetDevice(&dev));
-    KB_CUDA(cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev));
-    const int n_tiles = (int)n_tiles_of(H, W);
-    const int grid = std::max(1, std::min(n_sm, n_tiles));
-    // tiles per batch: whole waves, at most PR_WAVES_PER_BATCH of them, and few enough that 1/32 of the
-    // batch's trajectories fit the queue (what does not fit is evaluated by the overflow kernel)
-    long long waves = PR_WAVES_PER_BATCH;
-    if (n_vel > 0) waves = std::min<long long>(waves, (long long)((double)Qu.cap * 32.0 / ((double)grid * PR_TW * PR_TH * n_vel)));
-    waves = std::max<long long>(1, waves);
+    long long waves = (long long)(budget / std::max(1.0, wave_nominal / n_chunks));
+    waves = std::max<long long>(1, std::min<long long>(PR_WAVES_PER_BATCH, waves));
     const int batch = (int)std::min<long long>((long long)n_tiles, waves * grid);
     const size_t smem1 = (size_t)pl.ring_bytes + (size_t)PR_NTBL * TBL + PR_SMEM_MISC;
     KB_CUDA(cudaFuncSetAttribute(bound_phase_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem1));
@@ -956,12 +945,16 @@ int kb_launch_search_pruned(const float* d_psiphi, int T, int TPv, int H, int W,
         if (ng > 0) {
             for (int b0 = 0; b0 < n_tiles; b0 += batch) {
                 const int b1 = std::min(n_tiles, b0 + batch);
-                KB_CUDA(cudaMemsetAsync(Qu.count, 0, sizeof(unsigned long long), st));
-                bound_phase_kernel<<<std::min(grid, b1 - b0), PR_THREADS, smem1, st>>>(maps, T, H, W, b0, b1, tb, bp, P.min_obs, d_scale, Qu);
-                kb_phase_mark(KB_PHASE_BOUND, st);
-                exact_queue_kernel<TP><<<n_sm * 4, EX_THREADS, smem2, st>>>(psiphi2, H, W, d_tab, P, Qu, d_keys, d_stats);
-                kb_phase_mark(KB_PHASE_EXACT, st);
-                launches += 2;
+                for (int g0 = 0; g0 < ng; g0 += groups_per_chunk) {
+                    const int g1 = std::min(ng, g0 + groups_per_chunk);
+                    KB_CUDA(cudaMemsetAsync(Qu.count, 0, sizeof(unsigned long long), st));
+                    bound_phase_kernel<<<std::min(grid, b1 - b0), PR_THREADS, smem1, st>>>(maps, T, H, W, b0, b1, g0, g1, tb, bp,
+                                                                                          P.min_obs, d_scale, Qu);
+                    kb_phase_mark(KB_PHASE_BOUND, st);
+                    exact_queue_kernel<TP><<<n_sm * 4, EX_THREADS, smem2, st>>>(psiphi2, H, W, d_tab, P, Qu, d_keys, d_stats);
+                    kb_phase_mark(KB_PHASE_EXACT, st);
+                    launches += 2;
+                }
             }
             exact_overflow_kernel<TP><<<n_sm * 4, EX_THREADS, smem2, st>>>(psiphi2, H, W, d_tab, P, Qu.overflow,
                                                                            L.overflow_words, d_gvel, ng, d_keys, d_stats);

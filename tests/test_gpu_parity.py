@@ -419,3 +419,26 @@ def test_config5_full_size_coadd_and_refilter(kb, oracle):
     few = has & ((hit & valid).sum(1) <= 5) & (valid.sum(1) >= 20)  # the 25/75 percentiles stay on clean epochs
     dropped = (hit & valid & ~kept)[few].sum() / max(1, (hit & valid)[few].sum())
     assert few.sum() > 10_000 and dropped >= 0.99, (int(few.sum()), float(dropped))
+
+
+def test_search_config4_full_size_sampled(kb, oracle):
+    """BASELINE configs[3] at full size (2048x4096x50, 256 x 128 velocities, K = 16, min_obs = 25) through the
+    AUTO -> pruned path at the paper's threshold: oracle on random pixels, the corners, and 3x3 windows on
+    injected mover starts (their fluxes are sub-threshold by construction: what is checked is parity)."""
+    st = synth.config4_heavy()
+    vx, vy = synth.config4_grid()
+    d = _prep(kb, st)
+    T, H, W = st.img.shape
+    rng = np.random.default_rng(4)
+    px = [rng.integers(0, W, 1200), np.array([0, W - 1, 0, W - 1])]
+    py = [rng.integers(0, H, 1200), np.array([0, 0, H - 1, H - 1])]
+    for m in st.movers[:40]:
+        wy, wx = np.mgrid[-1:2, -1:2]
+        px.append(np.clip(int(m["x0"]) + wx.reshape(-1), 0, W - 1))
+        py.append(np.clip(int(m["y0"]) + wy.reshape(-1), 0, H - 1))
+    px, py = np.concatenate(px).astype(np.int32), np.concatenate(py).astype(np.int32)
+    sp = kb.SearchParams(K=16, min_obs=25, min_lh=10.0, algo=kb.ALGO_AUTO)
+    r = _search_and_compare(kb, oracle, d, st.times, vx, vy, sp, pixels=(px, py))
+    ev, nominal, _, algo = kb.kbmod_search_stats(kb.kbmod_search.last_workspace)
+    assert algo == kb.ALGO_PRUNED and nominal == H * W * len(vx) and ev < 0.2 * nominal
+    assert r["n_pix"] == len(px)
