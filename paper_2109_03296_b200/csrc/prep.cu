@@ -7,6 +7,8 @@
 // 9 B per pixel, the algorithmic minimum, plus the halo overlap), then every thread produces
 // PREP_R vertically adjacent outputs, sliding a register window down each kernel column so that
 // one shared-memory read feeds up to PREP_R multiply-adds per plane.
+#include <math.h>
+
 #include "common.cuh"
 
 namespace {
@@ -89,6 +91,107 @@ prep_kernel(const float* __restrict__ img, const float* __restrict__ var, const 
     }
 }
 
+// Separable PSFs (P[j][i] = u[j] v[i], e.g. any Gaussian): a row pass into a second shared-memory array, then a
+// column pass with the same sliding register window: k + k (1 + (k-1)/64) multiply-adds per plane and output
+// instead of k^2 (29 instead of 169 for the 13x13 PSF of the DECam-shaped configs).
+struct SepParam {
+    float u[KBMOD_MAX_PSF], v[KBMOD_MAX_PSF];  // column (y) and row (x) factors
+};
+
+__global__ void __launch_bounds__(PREP_TX* PREP_WARPS)
+prep_sep_kernel(const float* __restrict__ img, const float* __restrict__ var, const uint8_t* __restrict__ mask, int H,
+                int W, int k, const __grid_constant__ SepParam psf, float2* __restrict__ out) {
+    const int r = k / 2;
+    extern __shared__ float2 tile[];  // [(PREP_TY + k - 1)][pitch], then the row-pass result [(PREP_TY + k - 1)][PREP_TX]
+    const int pitch = PREP_TX + k - 1;
+    const int rows = PREP_TY + k - 1;
+    float2* hp = tile + rows * pitch;
+    const int x_org = blockIdx.x * PREP_TX - r;
+    const int y_org = blockIdx.y * PREP_TY - r;
+    const int tid = threadIdx.y * PREP_TX + threadIdx.x;
+
+    for (int idx = tid; idx < rows * pitch; idx += PREP_TX * PREP_WARPS) {
+        const int ty = idx / pitch, tx = idx - ty * pitch;
+        const int x = x_org + tx, y = y_org + ty;
+        float2 v = make_float2(0.0f, 0.0f);
+        if (x >= 0 && x < W && y >= 0 && y < H) {
+            const size_t q = (size_t)y * W + x;
+            const float I = __ldg(img + q), V = __ldg(var + q);
+            const bool bad = (mask && __ldg(mask + q) != 0) || !(V > 0.0f) || !isfinite(V) || !isfinite(I);
+            if (!bad) {
+                const float w = 1.0f / V;
+                v = make_float2(I * w, w);
+            }
+        }
+        tile[idx] = v;
+    }
+    __syncthreads();
+    // row pass: hp[row][x] = sum_i v[i] tile[row][x + i]  (and v[i]^2 for the weight plane)
+    const int lx = threadIdx.x;
+    for (int row = threadIdx.y; row < rows; row += PREP_WARPS) {
+        const float2* src = tile + (size_t)row * pitch + lx;
+        float a = 0.0f, b = 0.0f;
+#pragma unroll 1
+        for (int i = 0; i < k; ++i) {
+            const float2 t = src[i];
+            const float vi = psf.v[i];
+            a = fmaf(vi, t.x, a);
+            b = fmaf(vi * vi, t.y, b);
+        }
+        hp[row * PREP_TX + lx] = make_float2(a, b);
+    }
+    __syncthreads();
+    // column pass: out(ly + a) = sum_j u[j] hp[ly + a + j]
+    float ps[PREP_R], ph[PREP_R];
+#pragma unroll
+    for (int a = 0; a < PREP_R; ++a) ps[a] = ph[a] = 0.0f;
+    const int ly = threadIdx.y * PREP_R;
+    const float2* col = hp + (size_t)ly * PREP_TX + lx;
+#pragma unroll 1
+    for (int jj = 0; jj < k + PREP_R - 1; ++jj) {
+        const float2 t = col[jj * PREP_TX];
+#pragma unroll
+        for (int a = 0; a < PREP_R; ++a) {
+            const int j = jj - a;
+            if (j >= 0 && j < k) {
+                const float uj = psf.u[j];
+                ps[a] = fmaf(uj, t.x, ps[a]);
+                ph[a] = fmaf(uj * uj, t.y, ph[a]);
+            }
+        }
+    }
+    const int x = blockIdx.x * PREP_TX + lx;
+    if (x < W) {
+#pragma unroll
+        for (int a = 0; a < PREP_R; ++a) {
+            const int y = blockIdx.y * PREP_TY + ly + a;
+            if (y < H) {
+                const float wc = tile[(size_t)(ly + a + r) * pitch + lx + r].y;
+                out[(size_t)y * W + x] = (wc > 0.0f) ? make_float2(ps[a], ph[a]) : make_float2(0.0f, 0.0f);
+            }
+        }
+    }
+}
+
+// P = u v^T to float32 precision per tap?  (u[j] = P[j][c] / P[c][c], v[i] = P[c][i], c = k/2)
+static bool separable(const float* P, int k, SepParam* sp) {
+    const int c = k / 2;
+    const double pc = (double)P[c * k + c];
+    if (!(fabs(pc) > 0.0)) return false;
+    double pmax = 0.0;
+    for (int i = 0; i < k * k; ++i) pmax = fmax(pmax, fabs((double)P[i]));
+    for (int j = 0; j < k; ++j)
+        for (int i = 0; i < k; ++i) {
+            const double want = (double)P[j * k + i], got = (double)P[j * k + c] / pc * (double)P[c * k + i];
+            if (!(fabs(want - got) <= 2e-7 * fabs(want) + 1e-12 * pmax)) return false;
+        }
+    for (int j = 0; j < KBMOD_MAX_PSF; ++j) {
+        sp->u[j] = j < k ? (float)((double)P[j * k + c] / pc) : 0.0f;
+        sp->v[j] = j < k ? P[c * k + j] : 0.0f;
+    }
+    return true;
+}
+
 }  // namespace
 
 int kb_launch_prep(const float* d_img, const float* d_var, const uint8_t* d_mask, int T, int H, int W,
@@ -98,8 +201,17 @@ int kb_launch_prep(const float* d_img, const float* d_var, const uint8_t* d_mask
     const size_t smem = (size_t)(PREP_TY + k - 1) * (PREP_TX + k - 1) * sizeof(float2);
     const size_t plane = (size_t)H * W;
     PsfParam psf;
+    SepParam sep;
+    const size_t smem_sep = smem + (size_t)(PREP_TY + k - 1) * PREP_TX * sizeof(float2);
+    KB_CUDA(cudaFuncSetAttribute(prep_sep_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_sep));
     for (int t = 0; t < T; ++t) {
         const float* src = h_psf + (n_psf > 1 ? (size_t)t * k * k : 0);
+        if (k > 1 && separable(src, k, &sep)) {
+            prep_sep_kernel<<<grid, block, smem_sep, st>>>(d_img + t * plane, d_var + t * plane,
+                                                           d_mask ? d_mask + t * plane : nullptr, H, W, k, sep,
+                                                           reinterpret_cast<float2*>(d_psiphi) + t * plane);
+            continue;
+        }
         for (int i = 0; i < k * k; ++i) psf.p[i] = src[i];
         for (int i = k * k; i < KBMOD_MAX_PSF * KBMOD_MAX_PSF; ++i) psf.p[i] = 0.0f;
         prep_kernel<0><<<grid, block, smem, st>>>(d_img + t * plane, d_var + t * plane,
