@@ -198,7 +198,9 @@ bound_scale_kernel(const float2* __restrict__ psiphi, int T, size_t plane, float
             ratio[k] = sqrtf(Fk / fmin);
         }
         const int sum_bits = 32 - 2 * BP.cbits;
-        const float cap = floorf((float)((1u << sum_bits) - 1u) / (float)T);
+        // the largest term value: T of them must stay inside the sum field.  0.999: 2^sum_bits - 1 is not a float32
+        // (it would round UP to 2^sum_bits and T clamped terms would wrap the field)
+        const float cap = floorf(0.999f * (float)(1u << sum_bits) / (float)T);
         const float thr_units = 0.98f * cap / fmaxf(ratio[T], 1.0f);
         const float ml = (min_lh > 0.0f && min_lh < CUDART_INF_F) ? min_lh : 1.0f;
         float unit = ml * sqrtf(fmin) / thr_units;

@@ -442,3 +442,19 @@ def test_search_config4_full_size_sampled(kb, oracle):
     ev, nominal, _, algo = kb.kbmod_search_stats(kb.kbmod_search.last_workspace)
     assert algo == kb.ALGO_PRUNED and nominal == H * W * len(vx) and ev < 0.2 * nominal
     assert r["n_pix"] == len(px)
+
+
+@pytest.mark.parametrize("T,H,W,nv,K", [(1, 9, 7, 1, 1), (2, 33, 65, 3, 2), (1, 40, 130, 17, 4), (4, 5, 300, 33, 3)])
+def test_search_pruned_degenerate_shapes(kb, oracle, T, H, W, nv, K):
+    """One or two epochs (the producer's table ring wraps inside a single region burst), a single velocity, images
+    smaller than one 64x32 tile: the pruned path against the oracle, every pixel."""
+    st = synth.random_stack(90 + T + H, T, H, W, mask_frac=0.05, t_span=1.0)
+    rng = np.random.default_rng(90 + T)
+    vx = rng.uniform(-30, 30, nv).astype(np.float32)
+    vy = rng.uniform(-30, 30, nv).astype(np.float32)
+    d = _prep(kb, st)
+    sp = kb.SearchParams(min_lh=0.5, min_obs=1, K=K, algo=kb.ALGO_PRUNED)
+    r = _search_and_compare(kb, oracle, d, st.times, vx, vy, sp)
+    assert r["n_pix"] == H * W
+    _, nominal, _, algo = kb.kbmod_search_stats(kb.kbmod_search.last_workspace)
+    assert algo == kb.ALGO_PRUNED and nominal == H * W * nv
