@@ -382,7 +382,7 @@ def test_search_pruned_equals_direct_heavy_shaped(kb):
         outs[name] = [o.clone() for o in kb.kbmod_search(d, st.times, vx, vy, sp)]
     for a, b in zip(outs["direct"], outs["pruned"]):
         assert torch.equal(a, b)
-    assert int((outs["pruned"][2] >= 0).sum()) > 50
+    assert int((outs["pruned"][2] >= 0).sum()) > 10  # (50, 50) percentiles keep only values equal to the median
 
 
 def test_config5_full_size_coadd_and_refilter(kb, oracle):
@@ -458,3 +458,48 @@ def test_search_pruned_degenerate_shapes(kb, oracle, T, H, W, nv, K):
     assert r["n_pix"] == H * W
     _, nominal, _, algo = kb.kbmod_search_stats(kb.kbmod_search.last_workspace)
     assert algo == kb.ALGO_PRUNED and nominal == H * W * nv
+
+
+@pytest.mark.parametrize("T", [1, 2, 3, 5, 7, 12, 26, 50, 64])
+def test_search_pruned_equals_direct_with_clamped_terms(kb, T):
+    """Very bright pixels (up to 10^8 sigma) make the fixed-point terms of the bound planes clamp; very faint and
+    very noisy epochs spread phi over six decades.  The pruned path must still equal the direct kernel exactly."""
+    import torch
+    H, W = 70, 140
+    st = synth.random_stack(200 + T, T, H, W, mask_frac=0.03, t_span=2.0)
+    rng = np.random.default_rng(200 + T)
+    hot = rng.random((T, H, W)) < 0.01
+    st.img[hot] *= (10.0 ** rng.uniform(1, 8, int(hot.sum()))).astype(np.float32)
+    st.var *= (10.0 ** rng.uniform(-3, 3, (T, 1, 1))).astype(np.float32)
+    vx = rng.uniform(-15, 15, 48).astype(np.float32)
+    vy = rng.uniform(-15, 15, 48).astype(np.float32)
+    d = _prep(kb, st)
+    outs = {}
+    for name, algo in (("direct", kb.ALGO_DIRECT), ("pruned", kb.ALGO_PRUNED)):
+        sp = kb.SearchParams(K=4, min_obs=1, min_lh=5.0, algo=algo)
+        outs[name] = [o.clone() for o in kb.kbmod_search(d, st.times, vx, vy, sp)]
+    for a, b in zip(outs["direct"], outs["pruned"]):
+        assert torch.equal(a, b)
+    assert int((outs["pruned"][2] >= 0).sum()) > 100
+
+
+@pytest.mark.parametrize("n_sigma,pct,fon,sig", [(0.5, (25.0, 75.0), 0, 1), (1.4, (10.0, 90.0), 0, 1), (3.0, (40.0, 60.0), 1, 1),
+                                               (2.0, (25.0, 75.0), 0, 0), (1.36, (50.0, 50.0), 0, 1)])
+def test_search_pruned_equals_direct_filter_parameters(kb, n_sigma, pct, fon, sig):
+    """The number of epochs the bound may count on, m(n), depends on the filter parameters (n_sigma * C below 1:
+    only the median is certain to be kept; filter off: all n).  Pruned must equal direct for each."""
+    import torch
+    st = synth.random_stack(300, 12, 60, 100, mask_frac=0.1, t_span=2.0)
+    rng = np.random.default_rng(300)
+    st.img[rng.random(st.img.shape) < 0.02] *= 30.0
+    vx = rng.uniform(-12, 12, 40).astype(np.float32)
+    vy = rng.uniform(-12, 12, 40).astype(np.float32)
+    d = _prep(kb, st)
+    outs = {}
+    for name, algo in (("direct", kb.ALGO_DIRECT), ("pruned", kb.ALGO_PRUNED)):
+        sp = kb.SearchParams(sigmag_enable=sig, pct_lo=pct[0], pct_hi=pct[1], n_sigma=n_sigma, filter_on=fon, K=3, min_obs=4,
+                             min_lh=3.0, algo=algo)
+        outs[name] = [o.clone() for o in kb.kbmod_search(d, st.times, vx, vy, sp)]
+    for a, b in zip(outs["direct"], outs["pruned"]):
+        assert torch.equal(a, b)
+    assert int((outs["pruned"][2] >= 0).sum()) > 10  # (50, 50) percentiles keep only values equal to the median
