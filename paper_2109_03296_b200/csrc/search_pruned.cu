@@ -79,6 +79,12 @@ __host__ __device__ inline int tbl_bytes(int T) { return T * (PR_G * 4 + (int)si
 struct PrunedTables {  // device pointers into the workspace
     const int32_t* gvel;          // [n_groups][PR_G]  velocity index or -1
     const unsigned char* gtbl;    // [n_groups] table blocks of tbl_bytes(T)
+    // bit t of maskx[g][tile column] & masky[g][tile row]: the staged region of (tile, group g, epoch t) touches the
+    // image.  Where it does not, every sample of the tile's trajectories is off-chip: the epoch is skipped, and the
+    // whole group when fewer than min_obs epochs are left
+    const unsigned long long* maskx;  // [n_groups][tiles_x]
+    const unsigned long long* masky;  // [n_groups][tiles_y]
+    const uint32_t* gfoot;        // [n_groups] ring bytes of all the regions of a group (charged when it is skipped)
     int n_groups;
     int ring_bytes;
 };
@@ -249,7 +255,8 @@ __device__ __forceinline__ void topk_insert(unsigned long long* keys, int K, uns
     }
 }
 
-__device__ __forceinline__ void tile_origin(int tile_lin, int tiles_x, int tiles_y, int& tile_x0, int& tile_y0) {
+__device__ __forceinline__ void tile_origin(int tile_lin, int tiles_x, int tiles_y, int& tile_x0, int& tile_y0, int& txi_out,
+                                            int& tyi_out) {
     // column-block order: 4 tile columns x all tile rows, then the next 4 columns, so that the CTAs
     // running at the same time work on a compact block of tiles and share their staged regions in L2
     const int cb = tile_lin / (4 * tiles_y), rem = tile_lin - cb * 4 * tiles_y;
@@ -257,6 +264,12 @@ __device__ __forceinline__ void tile_origin(int tile_lin, int tiles_x, int tiles
     const int tyi = rem / cols_here, txi = cb * 4 + rem - tyi * cols_here;
     tile_x0 = txi * PR_TW;
     tile_y0 = tyi * PR_TH;
+    txi_out = txi;
+    tyi_out = tyi;
+}
+__device__ __forceinline__ void tile_origin(int tile_lin, int tiles_x, int tiles_y, int& tile_x0, int& tile_y0) {
+    int a, b;
+    tile_origin(tile_lin, tiles_x, tiles_y, tile_x0, tile_y0, a, b);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -292,45 +305,70 @@ bound_phase_kernel(const __grid_constant__ TensorMaps maps, int T, int H, int W,
         // ------------------------------------------------------------------ producer (one thread)
         kb_reg_dec<PR_REGS_PRODUCER>();
         if (tid != PR_CONSUMERS) return;
-        uint32_t q = 0, oldest = 0, used = 0, gcount = 0;
+        uint32_t q = 0, oldest = 0, used = 0, gcount = 0, carry = 0;
         uint32_t qs0 = 0, qs1 = 0, qs2 = 0, qs3 = 0;  // first region of the last four groups
         const uint32_t ring = (uint32_t)tb.ring_bytes;
+        const int need = min_obs > 1 ? min_obs : 1;
         int4 nxt0 = make_int4(0, 0, 0, 0);
         uint32_t nxt_fp = 0;
-        if (g_begin < g_end) {
-            const GroupEpoch* nge = reinterpret_cast<const GroupEpoch*>(tb.gtbl + (size_t)g_begin * TBL + (size_t)T * PR_G * 4);
-            nxt0 = __ldg(reinterpret_cast<const int4*>(nge));
-            nxt_fp = __ldg(&nge->footprint);
-        }
+        int nxt_g = -1;  // the group nxt0 / nxt_fp belong to
         for (int tile_lin = tile_begin + blockIdx.x; tile_lin < tile_end; tile_lin += gridDim.x) {
-            int tile_x0, tile_y0;
-            tile_origin(tile_lin, tiles_x, tiles_y, tile_x0, tile_y0);
+            int tile_x0, tile_y0, txi, tyi;
+            tile_origin(tile_lin, tiles_x, tiles_y, tile_x0, tile_y0, txi, tyi);
             // the ring chain of the tables restarts at offset 0 for every tile: drain first
             while (oldest < q) {
                 kb_mbar_wait(&empty[oldest & (PR_NB - 1)], (oldest / PR_NB) & 1);
                 ++oldest;
             }
             used = 0;
-            for (int g = g_begin; g < g_end; ++g, ++gcount) {
+            carry = 0;
+            for (int g = g_begin; g < g_end; ++g) {
+                const unsigned long long on = __ldg(tb.maskx + (size_t)g * tiles_x + txi) & __ldg(tb.masky + (size_t)g * tiles_y + tyi);
+                if (__popcll(on) < need) {  // no trajectory of this tile and group can have min_obs valid epochs
+                    carry += __ldg(tb.gfoot + g);
+                    continue;
+                }
                 qs0 = qs1; qs1 = qs2; qs2 = qs3; qs3 = q;
                 const unsigned char* gt = tb.gtbl + (size_t)g * TBL;
+                const GroupEpoch* gge = reinterpret_cast<const GroupEpoch*>(gt + (size_t)T * PR_G * 4);
                 // the first epoch's entry was fetched from global memory one group ago (nxt0 / nxt_fp); the other
                 // epochs are read from the group's table in shared memory once it has landed: no global-memory
                 // latency on the producer's critical path
+                if (nxt_g != g) {
+                    nxt0 = __ldg(reinterpret_cast<const int4*>(gge));
+                    nxt_fp = __ldg(&gge->footprint);
+                }
                 int4 e0 = nxt0;
                 uint32_t fp = nxt_fp;
                 const unsigned char* tblp = tblbase + (gcount & (PR_NTBL - 1)) * TBL;
                 const GroupEpoch* sge = reinterpret_cast<const GroupEpoch*>(tblp + (size_t)T * PR_G * 4);
                 const uint32_t q_first = q;
-                for (int t = 0; t < T; ++t) {
-                    if (t == 1) {
-                        kb_mbar_wait(&full[q_first & (PR_NB - 1)], (q_first / PR_NB) & 1);  // the table is in
-                    }
+                bool tbl_landed = false;
+                for (int t = 0; t < T; ++t) {  // epoch 0 has no displacement: its region is the tile, always on the image
                     if (t >= 1) {
-                        e0 = *reinterpret_cast<const int4*>(sge + t);
+                        if (!tbl_landed) {
+                            kb_mbar_wait(&full[q_first & (PR_NB - 1)], (q_first / PR_NB) & 1);  // the table is in
+                            tbl_landed = true;
+                        }
                         fp = sge[t].footprint;
+                        if (!((on >> t) & 1ull)) {  // skipped: its ring bytes are charged to the next staged region
+                            carry += fp;
+                            continue;
+                        }
+                        e0 = *reinterpret_cast<const int4*>(sge + t);
                     }
                     const int pitch_k = e0.z & 0xFF, n_box = (unsigned)e0.z >> 16;
+                    if (carry + fp > ring / 2) {
+                        // a long run of skipped regions: rather than charge it, wait until nothing is in flight
+                        while (oldest < q) {
+                            kb_mbar_wait(&empty[oldest & (PR_NB - 1)], (oldest / PR_NB) & 1);
+                            ++oldest;
+                        }
+                        used = 0;
+                        carry = 0;
+                    }
+                    fp += carry;
+                    carry = 0;
                     // table slot gcount & 3 was last read by group gcount - 4: all its regions must be released
                     const bool tbl_busy_possible = (t == 0) && gcount >= PR_NTBL;
                     while (used + fp > ring || q - oldest >= PR_NB || (tbl_busy_possible && oldest < qs0)) {
@@ -358,12 +396,13 @@ bound_phase_kernel(const __grid_constant__ TensorMaps maps, int T, int H, int W,
                     }
                     ++q;
                     if (t == 0) {  // fetch the next group's first entry now: a whole group of time to arrive
-                        const int gn = (g + 1 < g_end) ? g + 1 : g_begin;
-                        const GroupEpoch* nge = reinterpret_cast<const GroupEpoch*>(tb.gtbl + (size_t)gn * TBL + (size_t)T * PR_G * 4);
+                        nxt_g = (g + 1 < g_end) ? g + 1 : g_begin;
+                        const GroupEpoch* nge = reinterpret_cast<const GroupEpoch*>(tb.gtbl + (size_t)nxt_g * TBL + (size_t)T * PR_G * 4);
                         nxt0 = __ldg(reinterpret_cast<const int4*>(nge));
                         nxt_fp = __ldg(&nge->footprint);
                     }
                 }
+                ++gcount;
             }
         }
         return;
@@ -374,12 +413,16 @@ bound_phase_kernel(const __grid_constant__ TensorMaps maps, int T, int H, int W,
     const int need = min_obs > 1 ? min_obs : 1;
     uint32_t q = 0, gcount = 0;
     for (int tile_lin = tile_begin + blockIdx.x; tile_lin < tile_end; tile_lin += gridDim.x) {
-        int tile_x0, tile_y0;
-        tile_origin(tile_lin, tiles_x, tiles_y, tile_x0, tile_y0);
-        const int px0 = tile_x0 + lane, py0 = tile_y0 + warp;  // this thread's pixels: (px0, py0), (px0+32, py0)
+        int tile_x0, tile_y0, txi, tyi;
+        tile_origin(tile_lin, tiles_x, tiles_y, tile_x0, tile_y0, txi, tyi);
+        const int px0 = tile_x0 + lane, py0 = tile_y0 + warp;  // this thread's pixels: (px0 + 32 h, py0 + 16 v)
 
-        for (int g = g_begin; g < g_end; ++g, ++gcount) {
+        for (int g = g_begin; g < g_end; ++g) {
+            // epochs whose staged region touches the image (the same test as the producer's)
+            const unsigned long long on = __ldg(tb.maskx + (size_t)g * tiles_x + txi) & __ldg(tb.masky + (size_t)g * tiles_y + tyi);
+            if (__popcll(on) < need) continue;
             const unsigned char* tblp = tblbase + (gcount & (PR_NTBL - 1)) * TBL;
+            ++gcount;
             const int4* offs4 = reinterpret_cast<const int4*>(tblp);
             const GroupEpoch* ge = reinterpret_cast<const GroupEpoch*>(tblp + (size_t)T * PR_G * 4);
             // per (pixel, velocity): fixed-point sum of psi_+ << 14 | low-phi samples << 7 | valid samples
@@ -394,13 +437,16 @@ bound_phase_kernel(const __grid_constant__ TensorMaps maps, int T, int H, int W,
 #pragma unroll
             for (int i = 0; i < PR_PIX; ++i) ANU[i] = 0u;
             uint2 gw = make_uint2(0u, 0u);  // {pitch_k | uniform << 8 | n_box << 16, smem_off} of the next epoch
+            unsigned long long rem = on;  // bit 0 is always set: epoch 0 has no displacement
 #pragma unroll 1
-            for (int t = 0; t < T; ++t) {
+            while (rem) {
+                const int t = __ffsll((long long)rem) - 1;
+                rem &= rem - 1;
                 const int slot = q & (PR_NB - 1);
                 kb_mbar_wait(&full[slot], (q / PR_NB) & 1);
                 if (t == 0) gw = *reinterpret_cast<const uint2*>(&ge[0].pitch_k);  // the tables came with this region
                 const uint2 cur = gw;
-                if (t + 1 < T) gw = *reinterpret_cast<const uint2*>(&ge[t + 1].pitch_k);
+                if (rem) gw = *reinterpret_cast<const uint2*>(&ge[__ffsll((long long)rem) - 1].pitch_k);
                 const int pitch = PR_TW + 16 * (int)(cur.x & 0xFFu);
                 const unsigned char* base = smem + cur.y + (size_t)(warp * pitch + lane) * sizeof(unsigned int);
                 const int rows16 = 16 * pitch * (int)sizeof(unsigned int);  // this thread's second row of pixels
@@ -743,7 +789,7 @@ size_t n_tiles_of(int H, int W) { return (size_t)((W + PR_TW - 1) / PR_TW) * ((H
 size_t al256(size_t x) { return (x + 255) & ~(size_t)255; }
 
 struct WsLayout {
-    size_t gvel, gtbl, B, keys, qentries, qcount, overflow, total, overflow_words;
+    size_t gvel, gtbl, maskx, masky, gfoot, B, keys, qentries, qcount, overflow, total, overflow_words;
 };
 WsLayout ws_layout(int T, int H, int W, int n_vel, int K) {
     WsLayout L;
@@ -751,6 +797,9 @@ WsLayout ws_layout(int T, int H, int W, int n_vel, int K) {
     size_t o = 0;
     L.gvel = o;     o += al256(ngm * PR_G * 4);
     L.gtbl = o;     o += al256(ngm * tbl_bytes(T));
+    L.maskx = o;    o += al256(ngm * (size_t)((W + PR_TW - 1) / PR_TW) * 8);
+    L.masky = o;    o += al256(ngm * (size_t)((H + PR_TH - 1) / PR_TH) * 8);
+    L.gfoot = o;    o += al256(ngm * 4);
     L.B = o;        o += al256((size_t)T * H * Wp * 4);
     L.keys = o;     o += al256((size_t)H * W * K * 8);
     L.qentries = o; o += al256(queue_cap(n_vel) * 8);
@@ -876,6 +925,27 @@ int kb_launch_search_pruned(const float* d_psiphi, int T, int TPv, int H, int W,
         }
         evals += (double)PR_TW * PR_TH * cnt * T;
     }
+    // on-image masks: region t of group g touches the image iff the tile column AND the tile row allow it
+    const int tiles_x = (W + PR_TW - 1) / PR_TW, tiles_y = (H + PR_TH - 1) / PR_TH;
+    std::vector<unsigned long long> maskx((size_t)ng * tiles_x, 0ull), masky((size_t)ng * tiles_y, 0ull);
+    std::vector<uint32_t> gfoot((size_t)ng, 0u);
+    for (int g = 0; g < ng; ++g) {
+        const GroupEpoch* ge = reinterpret_cast<const GroupEpoch*>(gtbl.data() + (size_t)g * TBL + (size_t)T * PR_G * 4);
+        unsigned long long foot = 0;
+        for (int t = 0; t < T; ++t) {
+            const long long pitch = PR_TW + 16 * (long long)(ge[t].pitch_k & 0xFF), rows = (long long)ge[t].n_box * PR_RB;
+            for (int c = 0; c < tiles_x; ++c) {
+                const long long x0 = (long long)c * PR_TW + ge[t].ox;
+                if (x0 < W && x0 + pitch > 0) maskx[(size_t)g * tiles_x + c] |= 1ull << t;
+            }
+            for (int r = 0; r < tiles_y; ++r) {
+                const long long y0 = (long long)r * PR_TH + ge[t].oy;
+                if (y0 < H && y0 + rows > 0) masky[(size_t)g * tiles_y + r] |= 1ull << t;
+            }
+            foot += ge[t].footprint;
+        }
+        gfoot[g] = (uint32_t)std::min<unsigned long long>(foot, 0xFFFFFFFFull);  // > ring / 2 is all that matters
+    }
     if (plan_stats) {
         plan_stats[0] = (size_t)ng > ngm ? 1.0 : 0.0;       // the velocity list is too scattered to group
         plan_stats[1] = evals > 0 ? staged / evals : 0.0;   // staged bytes per evaluation
@@ -905,6 +975,9 @@ int kb_launch_search_pruned(const float* d_psiphi, int T, int TPv, int H, int W,
     if (ng > 0) {
         KB_CUDA(cudaMemcpyAsync(d_gvel, gvel.data(), gvel.size() * 4, cudaMemcpyHostToDevice, st));
         KB_CUDA(cudaMemcpyAsync(d_gtbl, gtbl.data(), gtbl.size(), cudaMemcpyHostToDevice, st));
+        KB_CUDA(cudaMemcpyAsync(w + L.maskx, maskx.data(), maskx.size() * 8, cudaMemcpyHostToDevice, st));
+        KB_CUDA(cudaMemcpyAsync(w + L.masky, masky.data(), masky.size() * 8, cudaMemcpyHostToDevice, st));
+        KB_CUDA(cudaMemcpyAsync(w + L.gfoot, gfoot.data(), gfoot.size() * 4, cudaMemcpyHostToDevice, st));
     }
     KB_CUDA(cudaMemsetAsync(d_keys, 0, (size_t)H * W * P.K * 8, st));
     KB_CUDA(cudaMemsetAsync(Qu.overflow, 0, L.overflow_words * 4, st));
@@ -942,7 +1015,8 @@ int kb_launch_search_pruned(const float* d_psiphi, int T, int TPv, int H, int W,
     const int batch = (int)std::min<long long>((long long)n_tiles, waves * grid);
     const size_t smem1 = (size_t)pl.ring_bytes + (size_t)PR_NTBL * TBL + PR_SMEM_MISC;
     KB_CUDA(cudaFuncSetAttribute(bound_phase_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem1));
-    PrunedTables tb{d_gvel, d_gtbl, ng, pl.ring_bytes};
+    PrunedTables tb{d_gvel, d_gtbl, (const unsigned long long*)(w + L.maskx), (const unsigned long long*)(w + L.masky),
+                    (const uint32_t*)(w + L.gfoot), ng, pl.ring_bytes};
     const float2* psiphi2 = reinterpret_cast<const float2*>(d_psiphi);
     KB_DISPATCH_TP(TPv, {
         const size_t smem2 = (size_t)TP * EX_THREADS * sizeof(float);
