@@ -54,10 +54,11 @@ constexpr int PR_NTBL = 4;                 // group tables in flight
 constexpr int PR_SMEM_MAX = 232448;        // 227 KB: the opt-in maximum of dynamic shared memory per CTA
 constexpr int PR_SMEM_MISC = 512;          // barriers + producer bookkeeping
 constexpr int PR_WAVES_PER_BATCH = 7;
+constexpr int PR_SUB = 8;                  // groups per work unit: CTAs take (tile, PR_SUB groups) units dynamically
 // 20 warps = 5 per scheduler: 16384 registers / (5 x 32) = 102 -> 96 per thread at launch.  setmaxnreg moves
 // registers inside the CTA's own allocation (640 x 96 = 61440): the producer warp group drops to 24 and the
-// 16 consumer warps rise (512 x 104 + 128 x 40 = 58368 <= 61440)
-constexpr int PR_REGS_PRODUCER = 40, PR_REGS_CONSUMER = 104;      // tiles per batch = SMs x this (the queue is reused per batch)
+// 16 consumer warps rise (512 x 104 + 128 x 56 = 60416 <= 61440)
+constexpr int PR_REGS_PRODUCER = 56, PR_REGS_CONSUMER = 104;      // tiles per batch = SMs x this (the queue is reused per batch)
 
 // per (group, epoch): where the staged region comes from and where it goes in the ring
 struct __align__(16) GroupEpoch {
@@ -106,6 +107,7 @@ constexpr int SC_UNIT = 0, SC_INV_UNIT = 1, SC_CAP = 2, SC_FLOOR = 4, SC_THR = S
 struct Queue {
     uint2* entries;                  // (pixel index y0*W+x0, velocity index); v = 0xFFFFFFFF: hole
     unsigned long long* count;       // entries appended (may exceed cap: the excess overflowed)
+    unsigned long long* units;       // work units handed out to the CTAs of the running launch (count + 1)
     unsigned long long cap;
     unsigned int* overflow;          // bitmap over (tile, group, warp) items that did not fit
 };
@@ -284,7 +286,10 @@ bound_phase_kernel(const __grid_constant__ TensorMaps maps, int T, int H, int W,
     unsigned char* tblbase = smem + tb.ring_bytes;
     uint64_t* full = reinterpret_cast<uint64_t*>(tblbase + PR_NTBL * TBL);
     uint64_t* empty = full + PR_NB;
-    uint32_t* fpq = reinterpret_cast<uint32_t*>(empty + PR_NB);  // producer only: footprint of each region in flight
+    uint64_t* ufull = empty + PR_NB;   // work-unit mailbox: the producer takes a unit from the global counter and
+    uint64_t* uempty = ufull + 1;      // publishes its index here; the consumers acknowledge having read it
+    volatile uint32_t* mailbox = reinterpret_cast<volatile uint32_t*>(uempty + 1);
+    uint32_t* fpq = reinterpret_cast<uint32_t*>(uempty + 2);  // producer only: footprint of each region in flight
 
     const int tid = threadIdx.x;
     const int lane = tid & 31, warp = tid >> 5;
@@ -293,6 +298,8 @@ bound_phase_kernel(const __grid_constant__ TensorMaps maps, int T, int H, int W,
             kb_mbar_init(&full[i], 1);
             kb_mbar_init(&empty[i], PR_CONSUMERS / 32);
         }
+        kb_mbar_init(ufull, 1);
+        kb_mbar_init(uempty, PR_CONSUMERS / 32);
         kb_fence_barrier_init();
         for (int k = 0; k < PR_NHEIGHT * PR_NPITCH; ++k) kb_prefetch_tensormap(&maps.m[k]);
     }
@@ -300,6 +307,9 @@ bound_phase_kernel(const __grid_constant__ TensorMaps maps, int T, int H, int W,
 
     const int tiles_x = (W + PR_TW - 1) / PR_TW, tiles_y = (H + PR_TH - 1) / PR_TH;
     const int ng = tb.n_groups;
+    // work units: (tile of the batch) x (PR_SUB consecutive groups of the chunk), tile-major
+    const int n_sub = (g_end - g_begin + PR_SUB - 1) / PR_SUB;
+    const unsigned int n_units = (unsigned int)(tile_end - tile_begin) * (unsigned int)n_sub;
 
     if (warp >= PR_CONSUMERS / 32) {
         // ------------------------------------------------------------------ producer (one thread)
@@ -312,17 +322,24 @@ bound_phase_kernel(const __grid_constant__ TensorMaps maps, int T, int H, int W,
         int4 nxt0 = make_int4(0, 0, 0, 0);
         uint32_t nxt_fp = 0;
         int nxt_g = -1;  // the group nxt0 / nxt_fp belong to
-        for (int tile_lin = tile_begin + blockIdx.x; tile_lin < tile_end; tile_lin += gridDim.x) {
+        for (uint32_t uk = 0;; ++uk) {
+            if (uk > 0) kb_mbar_wait(uempty, (uk - 1) & 1);  // every consumer warp has read the previous unit
+            const unsigned int u = (unsigned int)atomicAdd(Qu.units, 1ull);
+            *mailbox = u;
+            kb_mbar_arrive(ufull);
+            if (u >= n_units) break;
+            const int tile_lin = tile_begin + (int)(u / (unsigned int)n_sub);
+            const int g_lo = g_begin + (int)(u % (unsigned int)n_sub) * PR_SUB, g_hi = min(g_end, g_lo + PR_SUB);
             int tile_x0, tile_y0, txi, tyi;
             tile_origin(tile_lin, tiles_x, tiles_y, tile_x0, tile_y0, txi, tyi);
-            // the ring chain of the tables restarts at offset 0 for every tile: drain first
+            // the ring chain of the tables restarts at offset 0 for every unit: drain first
             while (oldest < q) {
                 kb_mbar_wait(&empty[oldest & (PR_NB - 1)], (oldest / PR_NB) & 1);
                 ++oldest;
             }
             used = 0;
             carry = 0;
-            for (int g = g_begin; g < g_end; ++g) {
+            for (int g = g_lo; g < g_hi; ++g) {
                 const unsigned long long on = __ldg(tb.maskx + (size_t)g * tiles_x + txi) & __ldg(tb.masky + (size_t)g * tiles_y + tyi);
                 if (__popcll(on) < need) {  // no trajectory of this tile and group can have min_obs valid epochs
                     carry += __ldg(tb.gfoot + g);
@@ -396,10 +413,12 @@ bound_phase_kernel(const __grid_constant__ TensorMaps maps, int T, int H, int W,
                     }
                     ++q;
                     if (t == 0) {  // fetch the next group's first entry now: a whole group of time to arrive
-                        nxt_g = (g + 1 < g_end) ? g + 1 : g_begin;
-                        const GroupEpoch* nge = reinterpret_cast<const GroupEpoch*>(tb.gtbl + (size_t)nxt_g * TBL + (size_t)T * PR_G * 4);
-                        nxt0 = __ldg(reinterpret_cast<const int4*>(nge));
-                        nxt_fp = __ldg(&nge->footprint);
+                        nxt_g = (g + 1 < g_hi) ? g + 1 : -1;
+                        if (nxt_g >= 0) {
+                            const GroupEpoch* nge = reinterpret_cast<const GroupEpoch*>(tb.gtbl + (size_t)nxt_g * TBL + (size_t)T * PR_G * 4);
+                            nxt0 = __ldg(reinterpret_cast<const int4*>(nge));
+                            nxt_fp = __ldg(&nge->footprint);
+                        }
                     }
                 }
                 ++gcount;
@@ -412,12 +431,19 @@ bound_phase_kernel(const __grid_constant__ TensorMaps maps, int T, int H, int W,
     kb_reg_inc<PR_REGS_CONSUMER>();
     const int need = min_obs > 1 ? min_obs : 1;
     uint32_t q = 0, gcount = 0;
-    for (int tile_lin = tile_begin + blockIdx.x; tile_lin < tile_end; tile_lin += gridDim.x) {
+    for (uint32_t uk = 0;; ++uk) {
+        kb_mbar_wait(ufull, uk & 1);
+        const unsigned int u = *mailbox;
+        __syncwarp();
+        if (lane == 0) kb_mbar_arrive(uempty);
+        if (u >= n_units) break;
+        const int tile_lin = tile_begin + (int)(u / (unsigned int)n_sub);
+        const int g_lo = g_begin + (int)(u % (unsigned int)n_sub) * PR_SUB, g_hi = min(g_end, g_lo + PR_SUB);
         int tile_x0, tile_y0, txi, tyi;
         tile_origin(tile_lin, tiles_x, tiles_y, tile_x0, tile_y0, txi, tyi);
         const int px0 = tile_x0 + lane, py0 = tile_y0 + warp;  // this thread's pixels: (px0 + 32 h, py0 + 16 v)
 
-        for (int g = g_begin; g < g_end; ++g) {
+        for (int g = g_lo; g < g_hi; ++g) {
             // epochs whose staged region touches the image (the same test as the producer's)
             const unsigned long long on = __ldg(tb.maskx + (size_t)g * tiles_x + txi) & __ldg(tb.masky + (size_t)g * tiles_y + tyi);
             if (__popcll(on) < need) continue;
@@ -887,7 +913,7 @@ int kb_launch_search_pruned(const float* d_psiphi, int T, int TPv, int H, int W,
     const double budget = 4.0 * (double)queue_cap(n_vel);
     const double wave_nominal = (double)grid * PR_TW * PR_TH * (double)ng * PR_G;  // one wave, all groups
     const int n_chunks = std::max(1, std::min(std::max(ng, 1), (int)ceil(wave_nominal / budget)));
-    const int groups_per_chunk = std::max(1, (ng + n_chunks - 1) / n_chunks);
+    const int groups_per_chunk = ((std::max(1, (ng + n_chunks - 1) / n_chunks) + PR_SUB - 1) / PR_SUB) * PR_SUB;
 
     // ---- tables: gvel, per-group blocks {offs[T][G], ge[T]}, ring chain
     std::vector<int32_t> gvel((size_t)ng * PR_G, -1);
@@ -895,7 +921,7 @@ int kb_launch_search_pruned(const float* d_psiphi, int T, int TPv, int H, int W,
     double staged = 0.0, evals = 0.0;
     uint32_t ph = 0;
     for (int g = 0; g < ng; ++g) {
-        if (g % groups_per_chunk == 0) ph = 0;  // a launch starts its ring chain at offset 0
+        if (g % PR_SUB == 0) ph = 0;  // every work unit starts its ring chain at offset 0
         const int lo = pl.leaves[g].first, cnt = pl.leaves[g].second - pl.leaves[g].first;
         for (int j = 0; j < cnt; ++j) gvel[(size_t)g * PR_G + j] = pl.idx[lo + j];
         int32_t* offs = reinterpret_cast<int32_t*>(gtbl.data() + (size_t)g * TBL);
@@ -968,6 +994,7 @@ int kb_launch_search_pruned(const float* d_psiphi, int T, int TPv, int H, int W,
     Queue Qu;
     Qu.entries = (uint2*)(w + L.qentries);
     Qu.count = (unsigned long long*)(w + L.qcount);
+    Qu.units = Qu.count + 1;
     float* d_scale = (float*)(w + L.qcount + 256);  // unit, cap, floors and thresholds of the fixed-point bound planes
     Qu.cap = queue_cap(n_vel);
     Qu.overflow = (unsigned int*)(w + L.overflow);
@@ -1027,7 +1054,7 @@ int kb_launch_search_pruned(const float* d_psiphi, int T, int TPv, int H, int W,
                 const int b1 = std::min(n_tiles, b0 + batch);
                 for (int g0 = 0; g0 < ng; g0 += groups_per_chunk) {
                     const int g1 = std::min(ng, g0 + groups_per_chunk);
-                    KB_CUDA(cudaMemsetAsync(Qu.count, 0, sizeof(unsigned long long), st));
+                    KB_CUDA(cudaMemsetAsync(Qu.count, 0, 2 * sizeof(unsigned long long), st));  // queue and unit counters
                     bound_phase_kernel<<<std::min(grid, b1 - b0), PR_THREADS, smem1, st>>>(maps, T, H, W, b0, b1, g0, g1, tb, bp,
                                                                                           P.min_obs, d_scale, Qu);
                     kb_phase_mark(KB_PHASE_BOUND, st);
