@@ -188,7 +188,7 @@ def run_reference(args):
 #                    SURVEY 8(d) counted 8 B per evaluation (psi and phi as float32): reported beside it.
 # dram__bytes_read.sum + dram__bytes_write.sum per step of the dominant kernel from the committed ncu --set full
 # capture (profiles/); None = not captured for this kernel
-TRAFFIC = {"bound_phase_kernel": 21.3e9, "search_direct_kernel": None}  # bytes per step (10 launches): profiles/r1_launches_final.md
+TRAFFIC = {"bound_phase_kernel": 16.4e9, "search_direct_kernel": None}  # bytes per step (84 launches): profiles/r1_launches_final.md
 CE_COUNT = {4: 5, 5: 9, 8: 19, 10: 32, 12: 42, 16: 63, 20: 103, 24: 132, 26: 147, 28: 162, 32: 191, 40: 305,
             48: 384, 50: 403, 56: 464, 64: 543}
 N_SM = 148
