@@ -21,6 +21,7 @@
  *   O5 score                   PAPER.md L79  (nu = Psi_coadd / sqrt(Phi_coadd)), L123 (sum LH')
  *   O6 per-pixel top-K         PAPER.md L127-L137 (section 3.2)
  *   O7 coadded stamps          PAPER.md L141 (section 3.3), L131 (Fig. 5)
+ *   N2 stamp central moments   PAPER.md L141 (section 3.3): thresholds 0.5, 0.5, 1.5, 36.5, 36.5; reading R22
  *
  * Pins (tests/test_oracle_*.py): closed-form point source, all-zero psi, numpy brute force on
  * tiny stacks, sorted() percentiles, erf^-1 closed form of the 0.7413 coefficient, invariants.
@@ -318,5 +319,42 @@ void oracle_coadd_stamps(const float *img, const uint8_t *mask, int T, int H, in
                 if (mean) mean[o] = mu;
                 if (median) median[o] = med;
             }
+    }
+}
+
+/* ------------------------------------------------------------------ N2: central-moment stamp filter (L141) */
+/* PAPER.md L141 (section 3.3): "we computed the central moments of postage stamps ... Stamps were rejected if they
+ * did not have central moments that were consistent with a Gaussian ... we required that the x, y, xy, xx, and yy
+ * moments be strictly less than 0.5, 0.5, 1.5, 36.5, and 36.5 respectively."  Reading R22: the stamp
+ * is made non-negative by subtracting its minimum and normalised to unit sum, w = (I - min I) / sum(I - min I)
+ * (a constant stamp gets the uniform weights 1/N); the moments are taken about the CENTRE PIXEL in pixel units,
+ *     m_x = sum u w,  m_y = sum v w,  m_xy = sum u v w,  m_xx = sum u^2 w,  m_yy = sum v^2 w,   u, v in [-r, r];
+ * the first three are compared by absolute value.  Non-finite pixels make the stamp fail.
+ * Pin of the reading: a featureless stamp has m_xx = m_yy = r (r + 1) / 3 = 36.67 for the paper's 21x21 stamps,
+ * just above the paper's 36.5 -- the thresholds reject "no source at all" only under this normalisation.
+ * stamps [n][S][S] float (v rows, u columns), thr[5]; out: moments [n][5] double, pass [n] (1 = kept). */
+void oracle_stamp_moments(const float *stamps, int n, int radius, const double *thr, double *moments, uint8_t *pass) {
+    const int S = 2 * radius + 1, N = S * S;
+#pragma omp parallel for schedule(static)
+    for (int i = 0; i < n; ++i) {
+        const float *I = stamps + (size_t)i * N;
+        double *m = moments + (size_t)i * 5;
+        int finite = 1;
+        double mn = INFINITY;
+        for (int k = 0; k < N; ++k) {
+            if (!isfinite(I[k])) finite = 0;
+            else if ((double)I[k] < mn) mn = (double)I[k];
+        }
+        if (!finite) { for (int k = 0; k < 5; ++k) m[k] = NAN; pass[i] = 0; continue; }
+        double sum = 0.0;
+        for (int k = 0; k < N; ++k) sum += (double)I[k] - mn;
+        double mx = 0, my = 0, mxy = 0, mxx = 0, myy = 0;
+        for (int v = -radius; v <= radius; ++v)
+            for (int u = -radius; u <= radius; ++u) {
+                double w = sum > 0.0 ? ((double)I[(v + radius) * S + (u + radius)] - mn) / sum : 1.0 / (double)N;
+                mx += u * w; my += v * w; mxy += (double)(u * v) * w; mxx += (double)(u * u) * w; myy += (double)(v * v) * w;
+            }
+        m[0] = mx; m[1] = my; m[2] = mxy; m[3] = mxx; m[4] = myy;
+        pass[i] = (fabs(mx) < thr[0] && fabs(my) < thr[1] && fabs(mxy) < thr[2] && mxx < thr[3] && myy < thr[4]) ? 1 : 0;
     }
 }

@@ -168,3 +168,19 @@ def coadd_stamps(img, mask, times, x0, y0, vx, vy, radius: int, epoch_mask=None)
                               _p(x0, C.c_int32), _p(y0, C.c_int32), _p(vx, C.c_float), _p(vy, C.c_float),
                               _p(em, C.c_uint64), n, radius, _p(mean, C.c_double), _p(med, C.c_double))
     return mean, med
+
+
+PAPER_MOMENT_THRESHOLDS = (0.5, 0.5, 1.5, 36.5, 36.5)  # x, y, xy, xx, yy "strictly less than"
+
+
+def stamp_moments(stamps, thresholds=PAPER_MOMENT_THRESHOLDS):
+    """N2 (reading R22). stamps [n][S][S]. Returns moments float64 [n][5], keep uint8 [n]."""
+    stamps = _c(stamps, np.float32)
+    n, S, S2 = stamps.shape
+    assert S == S2 and S % 2 == 1
+    thr = np.ascontiguousarray(thresholds, dtype=np.float64)
+    mom, keep = np.empty((n, 5), np.float64), np.empty(n, np.uint8)
+    lib().oracle_stamp_moments(stamps.ctypes.data_as(C.c_void_p), C.c_int(n), C.c_int(S // 2),
+                               thr.ctypes.data_as(C.c_void_p), mom.ctypes.data_as(C.c_void_p),
+                               keep.ctypes.data_as(C.c_void_p))
+    return mom, keep

@@ -481,3 +481,73 @@ def test_config1_recovers_injected_mover_within_paper_window():
     assert abs(x - 20) <= g["recovery_window_px"] and abs(y - 30) <= g["recovery_window_px"]
     assert math.hypot(vx[v] - 20, vy[v] - 5) <= g["recovery_window_px_per_day"]
     assert 35 < lh[y, x, 0] < 70
+
+
+# ------------------------------------------------------------------ N2: central-moment stamp filter (L141; R22)
+def _gauss_stamp(r, sigma, cx=0.0, cy=0.0, amp=1.0, bg=0.0):
+    ax = np.arange(-r, r + 1, dtype=np.float64)
+    g = np.exp(-0.5 * ((ax[None, :] - cx) ** 2 + (ax[:, None] - cy) ** 2) / sigma**2)
+    return (amp * g + bg).astype(np.float32)
+
+
+def test_moment_thresholds_are_the_papers():
+    g = golden()
+    assert O.PAPER_MOMENT_THRESHOLDS == (g["moment_thr_x"], g["moment_thr_y"], g["moment_thr_xy"], g["moment_thr_xx"],
+                                         g["moment_thr_yy"])
+
+
+def test_moments_featureless_stamp_closed_form_and_rejection():
+    """A constant stamp has m_xx = m_yy = r (r + 1) / 3: 36.67 at the paper's 21x21, just above its 36.5 --
+    the pin of reading R22's normalisation (min-subtracted, unit sum, about the centre pixel, in pixels)."""
+    for r in (1, 3, 10, 12):
+        S = 2 * r + 1
+        mom, keep = O.stamp_moments(np.full((1, S, S), 7.5, np.float32))
+        assert np.allclose(mom[0], [0, 0, 0, r * (r + 1) / 3.0, r * (r + 1) / 3.0], atol=1e-12)
+    mom, keep = O.stamp_moments(np.full((1, 21, 21), -3.0, np.float32))
+    assert abs(mom[0, 3] - 110.0 / 3.0) < 1e-12 and keep[0] == 0  # 36.67 is not "strictly less than 36.5"
+    # noise-only stamps scatter around the featureless value: most of them are rejected
+    rng = np.random.default_rng(0)
+    mom, keep = O.stamp_moments(rng.standard_normal((200, 21, 21)).astype(np.float32))
+    assert abs(mom[:, 3:].mean() - 110.0 / 3.0) < 0.3 and keep.mean() < 0.3
+
+
+def test_moments_gaussian_closed_forms():
+    """Centred Gaussian: first and cross moments 0, second moments sigma^2; shifted by (dx, dy): first moments
+    (dx, dy), second moments sigma^2 + d^2 (parallel axes), cross moment dx dy.  Invariant to adding a constant
+    pedestal that the stamp's minimum absorbs, and to scaling."""
+    r, sig = 10, 1.4
+    mom, keep = O.stamp_moments(np.stack([_gauss_stamp(r, sig), _gauss_stamp(r, sig, amp=250.0),
+                                          _gauss_stamp(r, sig, 2.0, -1.0), _gauss_stamp(r, sig, 0.4, 0.3)]))
+    assert np.allclose(mom[0], [0, 0, 0, sig**2, sig**2], atol=1e-6) and keep[0] == 1
+    assert np.allclose(mom[1], mom[0], atol=1e-6)
+    assert np.allclose(mom[2], [2.0, -1.0, -2.0, sig**2 + 4.0, sig**2 + 1.0], atol=1e-5) and keep[2] == 0
+    assert np.allclose(mom[3], [0.4, 0.3, 0.12, sig**2 + 0.16, sig**2 + 0.09], atol=1e-5) and keep[3] == 1
+    # the minimum is subtracted: a pedestal changes nothing (float32 pedestal of a float32 stamp)
+    a = _gauss_stamp(r, sig, 0.4, 0.3)
+    m1, _ = O.stamp_moments((a + np.float32(8.0))[None])
+    assert np.allclose(m1[0], mom[3], atol=2e-5)
+
+
+def test_moments_equal_numpy_restatement_and_strict_thresholds():
+    rng = np.random.default_rng(3)
+    r = 10
+    st = np.stack([_gauss_stamp(r, rng.uniform(1, 2.5), rng.uniform(-1, 1), rng.uniform(-1, 1), rng.uniform(5, 50))
+                   + rng.standard_normal((21, 21)).astype(np.float32) for _ in range(300)])
+    mom, keep = O.stamp_moments(st)
+    u = np.arange(-r, r + 1, dtype=np.float64)[None, None, :]
+    v = np.arange(-r, r + 1, dtype=np.float64)[None, :, None]
+    w = st.astype(np.float64) - st.astype(np.float64).min(axis=(1, 2), keepdims=True)
+    w /= w.sum(axis=(1, 2), keepdims=True)
+    ref = np.stack([(u * w).sum((1, 2)), (v * w).sum((1, 2)), (u * v * w).sum((1, 2)), (u * u * w).sum((1, 2)),
+                    (v * v * w).sum((1, 2))], axis=1)
+    assert np.allclose(mom, ref, rtol=1e-12, atol=1e-12)
+    thr = np.array(O.PAPER_MOMENT_THRESHOLDS)
+    ref_keep = (np.abs(ref[:, :3]) < thr[:3]).all(1) & (ref[:, 3:] < thr[3:]).all(1)
+    assert np.array_equal(keep.astype(bool), ref_keep) and 0 < keep.sum() < 300
+    # "strictly less than": a moment equal to its threshold fails
+    m0, k0 = O.stamp_moments(_gauss_stamp(r, 1.4)[None], thresholds=(0.5, 0.5, 1.5, float(mom[0, 3]) * 0 + 1.0, 36.5))
+    m1, k1 = O.stamp_moments(_gauss_stamp(r, 1.4)[None], thresholds=(0.5, 0.5, 1.5, float(m0[0, 3]), 36.5))
+    assert k1[0] == 0
+    # non-finite pixels: the stamp fails
+    bad = _gauss_stamp(r, 1.4).copy(); bad[3, 4] = np.nan
+    assert O.stamp_moments(bad[None])[1][0] == 0
