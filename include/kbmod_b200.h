@@ -172,6 +172,22 @@ int kbmod_sigmag_filter(const float* d_psi_lc, const float* d_phi_lc, int n_lc, 
                         const kbmod_search_params* p, uint64_t* d_kept, float* d_lh, float* d_flux, void* stream);
 
 /* ---------------------------------------------------------------------------------------------
+ * Central-moment stamp filter, the step behind the coadd (s3.3): "we computed the central moments
+ * of postage stamps for candidate trajectories.  Stamps were rejected if they did not have central moments that
+ * were consistent with a Gaussian ... we required that the x, y, xy, xx, and yy moments be strictly less than
+ * 0.5, 0.5, 1.5, 36.5, and 36.5 respectively."  Reading R22: w = (I - min I) / sum(I - min I) (1/N for a constant
+ * stamp); about the centre pixel, u, v in [-radius, radius] pixels:
+ *     m_x = sum u w, m_y = sum v w, m_xy = sum u v w, m_xx = sum u^2 w, m_yy = sum v^2 w     (double precision)
+ * keep = |m_x| < t[0] && |m_y| < t[1] && |m_xy| < t[2] && m_xx < t[3] && m_yy < t[4]; a stamp with a non-finite
+ * pixel gets NaN moments and keep = 0.
+ *   d_stamps      [n_stamps][2r+1][2r+1] float32 (e.g. kbmod_coadd_stamps' d_median)
+ *   h_thresholds  [5] double on the HOST, or NULL for the paper's values
+ *   d_moments     out [n_stamps][5] float64 (x, y, xy, xx, yy); may be NULL
+ *   d_keep        out [n_stamps] uint8; may be NULL */
+int kbmod_stamp_moments(const float* d_stamps, int n_stamps, int radius, const double* h_thresholds, double* d_moments,
+                        uint8_t* d_keep, void* stream);
+
+/* ---------------------------------------------------------------------------------------------
  * Whole path from HOST buffers (what bench.py's end-to-end number times): H2D copies of the
  * image / variance / mask stacks, kbmod_prepare_psi_phi, kbmod_search, D2H copies of the four
  * result arrays, then synchronises `stream`.  h_mask may be NULL.  Host buffers should be pinned

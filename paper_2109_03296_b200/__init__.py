@@ -3,4 +3,4 @@ library libkbmod_b200.so (include/kbmod_b200.h) plus the seeded synthetic input 
 from .binding import (ALGO_AUTO, ALGO_DIRECT, ALGO_PRUNED, KbmodError, SearchParams, kbmod_coadd_stamps,  # noqa: F401
                       kbmod_default_params, kbmod_displacements, kbmod_eval_trajectories, kbmod_pipeline_host,
                       kbmod_pipeline_host_arena_bytes, kbmod_prepare_psi_phi, kbmod_search, kbmod_search_stats, kbmod_search_phase_ms, kbmod_search_phase_timing,
-                      kbmod_search_workspace_bytes, kbmod_sigmag_filter, kbmod_version)
+                      kbmod_search_workspace_bytes, kbmod_sigmag_filter, kbmod_stamp_moments, kbmod_version)

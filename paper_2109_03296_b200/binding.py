@@ -19,7 +19,7 @@ MAX_T, MAX_K, MAX_PSF, MAX_STAMP_RADIUS = 64, 32, 31, 15
 EXPORTS = ["kbmod_default_params", "kbmod_prepare_psi_phi", "kbmod_displacements",
            "kbmod_search_workspace_bytes", "kbmod_search", "kbmod_search_stats", "kbmod_search_phase_timing",
            "kbmod_search_phase_ms", "kbmod_coadd_stamps",
-           "kbmod_eval_trajectories", "kbmod_sigmag_filter", "kbmod_pipeline_host_arena_bytes",
+           "kbmod_eval_trajectories", "kbmod_sigmag_filter", "kbmod_stamp_moments", "kbmod_pipeline_host_arena_bytes",
            "kbmod_pipeline_host", "kbmod_last_error", "kbmod_version"]
 
 
@@ -241,6 +241,23 @@ def kbmod_sigmag_filter(psi_lc, phi_lc, params: SearchParams, stream=None):
     _check(lib().kbmod_sigmag_filter(_dev(psi_lc, torch.float32), _dev(phi_lc, torch.float32), n, T, C.byref(cp),
                                      _dev(r["kept"]), _dev(r["lh"]), _dev(r["flux"]), _stream(stream)))
     return r
+
+
+def kbmod_stamp_moments(stamps, thresholds=None, stream=None):
+    """Central moments (x, y, xy, xx, yy) of [n][S][S] stamps and the paper's keep / reject flag.
+    Returns (moments float64 [n][5], keep uint8 [n])."""
+    import torch
+    s = _dev(stamps, torch.float32)
+    n, S, S2 = stamps.shape
+    if S != S2 or S % 2 != 1:
+        raise KbmodError(-1, f"stamps must be [n][2r+1][2r+1], got {tuple(stamps.shape)}")
+    mom = torch.empty((n, 5), dtype=torch.float64, device=stamps.device)
+    keep = torch.empty((n,), dtype=torch.uint8, device=stamps.device)
+    thr_arr, thr_ptr = (None, C.c_void_p(0)) if thresholds is None else _host(thresholds, np.float64)
+    if thr_arr is not None and thr_arr.shape != (5,):
+        raise KbmodError(-1, "thresholds must be 5 numbers: x, y, xy, xx, yy")
+    _check(lib().kbmod_stamp_moments(s, C.c_int(n), C.c_int(S // 2), thr_ptr, _dev(mom), _dev(keep), _stream(stream)))
+    return mom, keep
 
 
 def kbmod_pipeline_host_arena_bytes(T, H, W, n_vel, params: SearchParams) -> int:

@@ -355,6 +355,21 @@ extern "C" int kbmod_sigmag_filter(const float* d_psi_lc, const float* d_phi_lc,
                                    d_flux, (cudaStream_t)stream);
 }
 
+extern "C" int kbmod_stamp_moments(const float* d_stamps, int n_stamps, int radius, const double* h_thresholds,
+                                   double* d_moments, uint8_t* d_keep, void* stream) {
+    KB_REQUIRE(n_stamps >= 0, KBMOD_ERR_INVALID_ARG, "n_stamps = %d", n_stamps);
+    KB_REQUIRE(radius >= 0, KBMOD_ERR_INVALID_ARG, "radius = %d", radius);
+    KB_REQUIRE(radius <= KBMOD_MAX_STAMP_RADIUS, KBMOD_ERR_UNSUPPORTED, "radius = %d exceeds %d", radius,
+               KBMOD_MAX_STAMP_RADIUS);
+    if (n_stamps == 0 || (!d_moments && !d_keep)) return KBMOD_OK;
+    KB_REQUIRE(d_stamps, KBMOD_ERR_INVALID_ARG, "NULL stamps");
+    static const double paper[5] = {0.5, 0.5, 1.5, 36.5, 36.5};
+    if (h_thresholds)
+        for (int k = 0; k < 5; ++k) KB_REQUIRE(!isnan(h_thresholds[k]), KBMOD_ERR_INVALID_ARG, "NaN threshold");
+    return kb_launch_stamp_moments(d_stamps, n_stamps, radius, h_thresholds ? h_thresholds : paper, d_moments, d_keep,
+                                   (cudaStream_t)stream);
+}
+
 // ---------------------------------------------------------------------------------------------
 // whole path from host buffers (bench.py's end-to-end number)
 struct ArenaPlan {

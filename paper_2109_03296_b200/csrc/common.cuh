@@ -171,6 +171,9 @@ int kb_launch_coadd(const float* d_img, const uint8_t* d_mask, int T, int TP, in
                     const unsigned long long* d_epoch_mask, int n_traj, int radius, float* d_mean, float* d_median,
                     cudaStream_t st);
 
+int kb_launch_stamp_moments(const float* d_stamps, int n, int radius, const double* thr5, double* d_moments,
+                            uint8_t* d_pass, cudaStream_t st);
+
 // pruned search (search_pruned.cu).  h_dx, h_dy: [n_vel][T] displacement table (a2).  plan_only: run the host
 // planner only and fill plan_stats = {fraction of velocity groups that cannot be staged, staged bytes per evaluation}.
 size_t kb_pruned_workspace_bytes(int T, int H, int W, int n_vel, int K);

@@ -503,3 +503,59 @@ def test_search_pruned_equals_direct_filter_parameters(kb, n_sigma, pct, fon, si
     for a, b in zip(outs["direct"], outs["pruned"]):
         assert torch.equal(a, b)
     assert int((outs["pruned"][2] >= 0).sum()) > 10  # (50, 50) percentiles keep only values equal to the median
+
+
+# ------------------------------------------------------------------------------------------- N2: stamp moments
+def _moments_agree(g_mom, g_keep, o_mom, o_keep, thr):
+    g_mom, g_keep = g_mom.cpu().numpy(), g_keep.cpu().numpy()
+    nan = np.isnan(o_mom).any(1)
+    assert np.array_equal(np.isnan(g_mom).any(1), nan)
+    assert np.allclose(g_mom[~nan], o_mom[~nan], rtol=1e-11, atol=1e-11)  # double on both sides, other summation order
+    # the flag is a threshold on a double: compare it except where a moment sits within 1e-9 of its threshold
+    t = np.asarray(thr)
+    dist = np.minimum(np.abs(np.abs(o_mom[:, :3]) - t[:3]).min(1), np.abs(o_mom[:, 3:] - t[3:]).min(1))
+    solid = ~nan & (dist > 1e-9)
+    assert np.array_equal(g_keep[solid], o_keep[solid]) and np.all(g_keep[nan] == 0)
+    return int(solid.sum())
+
+
+@pytest.mark.parametrize("radius", [0, 1, 3, 10, 15])
+def test_stamp_moments_random(kb, oracle, radius):
+    rng = np.random.default_rng(400 + radius)
+    S = 2 * radius + 1
+    n = 3000
+    ax = np.arange(-radius, radius + 1)
+    st = rng.standard_normal((n, S, S)).astype(np.float32)
+    amp = rng.uniform(0, 60, n)[:, None, None]
+    cx, cy = rng.uniform(-1.5, 1.5, n)[:, None, None], rng.uniform(-1.5, 1.5, n)[:, None, None]
+    st += (amp * np.exp(-0.5 * ((ax[None, None, :] - cx) ** 2 + (ax[None, :, None] - cy) ** 2) / 1.6**2)).astype(np.float32)
+    st[5] = 4.25                 # constant stamp
+    st[6, 0, 0] = np.nan         # non-finite pixel
+    st[7, S - 1, S - 1] = np.inf
+    thr = (0.5, 0.5, 1.5, 36.5, 36.5) if radius == 10 else (0.3, 0.3, 0.5, 0.3 * radius * radius + 0.5, 0.3 * radius * radius + 0.5)
+    g_mom, g_keep = kb.kbmod_stamp_moments(_cuda(st), None if radius == 10 else thr)
+    o_mom, o_keep = oracle.stamp_moments(st, thr)
+    assert _moments_agree(g_mom, g_keep, o_mom, o_keep, thr) > n - 20
+    if radius >= 3:
+        assert 0 < int(o_keep.sum()) < n
+
+
+def test_stamp_moments_on_coadded_stamps(kb, oracle):
+    """The step as the paper chains it (L141): median stamps of candidate trajectories, then the moment filter.
+    Candidates on injected movers (true velocity) must pass, candidates on empty sky mostly fail."""
+    st = synth.decam_stack(9, (7, 6, 7, 6), H=768, W=512, n_movers=60, n_stars=40)
+    T, H, W = st.img.shape
+    mv = [m for m in st.movers if m["flux"] > 1500]
+    n_sky = 2000
+    rng = np.random.default_rng(9)
+    x0 = np.concatenate([[int(m["x0"]) for m in mv], rng.integers(0, W, n_sky)]).astype(np.int32)
+    y0 = np.concatenate([[int(m["y0"]) for m in mv], rng.integers(0, H, n_sky)]).astype(np.int32)
+    vx = np.concatenate([[m["vx"] for m in mv], rng.uniform(-300, 300, n_sky)]).astype(np.float32)
+    vy = np.concatenate([[m["vy"] for m in mv], rng.uniform(-300, 300, n_sky)]).astype(np.float32)
+    _, med = kb.kbmod_coadd_stamps(_cuda(st.img), _cuda(st.mask), st.times, _cuda(x0), _cuda(y0), _cuda(vx), _cuda(vy), 10)
+    g_mom, g_keep = kb.kbmod_stamp_moments(med)
+    o_mom, o_keep = oracle.stamp_moments(med.cpu().numpy())
+    _moments_agree(g_mom, g_keep, o_mom, o_keep, oracle.PAPER_MOMENT_THRESHOLDS)
+    k = g_keep.cpu().numpy().astype(bool)
+    assert len(mv) >= 10 and k[:len(mv)].mean() > 0.8, (len(mv), k[:len(mv)].mean())
+    assert k[len(mv):].mean() < 0.5
