@@ -55,6 +55,10 @@ def make_workload(name: str, seed_shift: int = 0):
         st = synth.config4_heavy(seed=3 + seed_shift)
         vx, vy = synth.config4_grid()
         return st, vx, vy, dict(K=16, min_obs=25), "configs[3] heavy 2048x4096x50, 256x128 velocities, K=16"
+    if name == "paper":  # configs[2]'s stack searched with the paper's full 512 x 256 grid
+        st = synth.config3_decam(seed=2 + seed_shift)
+        vx, vy = synth.paper_grid()
+        return st, vx, vy, dict(K=8, min_obs=13), "configs[2] stack x the paper's 512x256 velocity grid (131072), K=8"
     if name == "c2":
         st = synth.config2_medium(seed=1 + seed_shift)
         vx, vy = synth.config2_grid()
@@ -384,7 +388,7 @@ def main():
     ap.add_argument("--steps", type=int, default=3)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="c3", choices=["c1", "c2", "c3", "c4"])
+    ap.add_argument("--workload", default="c3", choices=["c1", "c2", "c3", "c4", "paper"])
     ap.add_argument("--min-lh", type=float, default=10.0, dest="min_lh")
     ap.add_argument("--algo", default="auto", choices=["auto", "direct", "pruned"])
     ap.add_argument("--no-cpu-baseline", action="store_true")

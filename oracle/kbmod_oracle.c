@@ -25,8 +25,9 @@
  *
  * Pins (tests/test_oracle_*.py): closed-form point source, all-zero psi, numpy brute force on
  * tiny stacks, sorted() percentiles, erf^-1 closed form of the 0.7413 coefficient, invariants.
- * Unpinned against the original KBMOD code (not available): readings R3 (masked taps) and R10
- * (nearest-rank percentiles) -- "parity unpinned" with respect to that code; see DESIGN.md.
+ * Unpinned against the original KBMOD code (not available): readings R3 (masked taps), R10
+ * (nearest-rank percentiles) and R22 (moment normalisation) -- "parity unpinned" with respect to that
+ * code; see DESIGN.md.
  */
 #include <float.h>
 #include <math.h>

@@ -223,6 +223,12 @@ def config3_grid(n_ang: int = 128, n_spd: int = 64):
     return velocity_grid(n_ang, n_spd, THETA_ECLIPTIC - math.pi / 10, THETA_ECLIPTIC + math.pi / 10, 92.0, 526.0)
 
 
+def paper_grid():
+    """The paper's own search grid: 512 speed steps over 92-550 px/day x 256 angle steps within
+    +-pi/10 of the ecliptic angle = 131072 velocities (about 1.1e12 trajectories on a 2K x 4K CCD, L133)."""
+    return velocity_grid(256, 512, THETA_ECLIPTIC - math.pi / 10, THETA_ECLIPTIC + math.pi / 10, 92.0, 550.0)
+
+
 def config4_heavy(seed: int = 3, H: int = 4096, W: int = 2048, n_movers: int = 1000, **kw) -> Stack:
     return decam_stack(seed, (9, 8, 8, 9, 8, 8), H, W, n_movers=n_movers, flux_range=(10.0, 100.0),
                        flux_log=False, name="config4_heavy", **kw)

@@ -559,3 +559,26 @@ def test_stamp_moments_on_coadded_stamps(kb, oracle):
     k = g_keep.cpu().numpy().astype(bool)
     assert len(mv) >= 10 and k[:len(mv)].mean() > 0.8, (len(mv), k[:len(mv)].mean())
     assert k[len(mv):].mean() < 0.5
+
+
+def test_sigmag_refilter_one_million_candidates(kb, oracle):
+    """N1 (the CPU post-filter rejects ~10^6 trajectories in ~60 s on 30 cores): sigma-G on 10^6
+    candidate lightcurves of 26 epochs, both lightcurve choices (R9), every kept set against the oracle."""
+    rng = np.random.default_rng(77)
+    n, T = 1_000_000, 26
+    phi = rng.uniform(5e-5, 1.2e-4, (n, T)).astype(np.float32)
+    psi = (rng.standard_normal((n, T)).astype(np.float32) + np.float32(1.5)) * np.sqrt(phi)
+    phi[rng.random((n, T)) < 0.08] = 0.0
+    psi, _ = synth.outlier_lightcurves(8, psi, phi, 0.1, 8.0)
+    d_psi, d_phi = _cuda(psi), _cuda(phi)
+    for fon in (0, 1):
+        sp = kb.SearchParams(K=1, min_obs=13, filter_on=fon)
+        g = {k: v.cpu().numpy() for k, v in kb.kbmod_sigmag_filter(d_psi, d_phi, sp).items()}
+        o = oracle.sigmag_filter(psi, phi, parity.oracle_params(oracle, sp))
+        assert np.array_equal(g["kept"].view(np.uint64), o["kept"])
+        has = o["n_kept"] > 0
+        tl, tf = parity.score_tolerances(dict(o, psi_lc=psi, phi_lc=phi), T)
+        assert has.sum() > 900_000
+        assert np.all(np.abs(g["lh"][has] - o["lh"][has]) <= tl[has])
+        assert np.all(np.abs(g["flux"][has] - o["flux"][has]) <= tf[has])
+        assert np.all(np.isneginf(g["lh"][~has]))
