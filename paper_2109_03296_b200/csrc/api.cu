@@ -209,6 +209,9 @@ extern "C" int kbmod_search(const float* d_psiphi, int T, int H, int W, const do
                n_vel);
     int rc = check_stack(T, H, W);
     if (rc) return rc;
+    for (int t = 0; t < T; ++t) KB_REQUIRE(isfinite(h_times[t]), KBMOD_ERR_INVALID_ARG, "times[%d] is not finite", t);
+    for (int v = 0; v < n_vel; ++v)
+        KB_REQUIRE(isfinite(h_vx[v]) && isfinite(h_vy[v]), KBMOD_ERR_INVALID_ARG, "velocity %d is not finite", v);
     DevParams P;
     rc = kb_make_dev_params(p, T, &P);
     if (rc) return rc;

@@ -250,6 +250,10 @@ def test_error_codes(kb):
     assert e.value.code == -1
     with pytest.raises(TypeError):
         kb.kbmod_search(d.cpu(), t, v, v, kb.SearchParams(K=1))  # no CPU fallback
+    for bad_v, bad_t in ((np.array([np.inf], np.float32), t), (np.array([np.nan], np.float32), t), (v, np.array([0.0, np.nan]))):
+        with pytest.raises(kb.KbmodError) as e:
+            kb.kbmod_search(d, bad_t, bad_v, v, kb.SearchParams(K=1))
+        assert e.value.code == -1
 
 
 # ------------------------------------------------------------------------------------------- pruned search
