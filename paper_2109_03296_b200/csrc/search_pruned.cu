@@ -29,6 +29,7 @@
 #include <math.h>
 #include <stddef.h>
 #include <stdlib.h>
+#include <string.h>
 
 #include <algorithm>
 #include <vector>
@@ -797,6 +798,16 @@ struct Planner {
     }
 };
 
+struct PlanCache {
+    bool valid = false;
+    int T = 0, H = 0, W = 0, n_vel = 0, ng = 0;
+    double staged = 0.0, evals = 0.0;
+    std::vector<int32_t> kdx, kdy, gvel;
+    std::vector<unsigned char> gtbl;
+    std::vector<unsigned long long> maskx, masky;
+    std::vector<uint32_t> gfoot;
+};
+
 int ring_bytes_for(int T) { return ((PR_SMEM_MAX - PR_SMEM_MISC - PR_NTBL * tbl_bytes(T)) / 1024) * 1024; }
 size_t max_groups(int n_vel) {
     const size_t full = ((size_t)n_vel + PR_G - 1) / PR_G;
@@ -878,27 +889,109 @@ int kb_launch_search_pruned(const float* d_psiphi, int T, int TPv, int H, int W,
         cdx[i] = std::max(-40000, std::min(40000, h_dx[i]));
         cdy[i] = std::max(-40000, std::min(40000, h_dy[i]));
     }
-    Planner pl;
-    pl.T = T; pl.n_vel = n_vel; pl.ring_bytes = ring_bytes_for(T);
-    pl.max_region = (pl.ring_bytes / 2 / 1024) * 1024;
-    pl.dx = cdx.data(); pl.dy = cdy.data();
-    int t_far = 0;
-    {   // epoch with the largest displacement spread
-        long long best = -1;
-        for (int t = 0; t < T; ++t) {
-            long long s = 0;
-            for (int v = 0; v < n_vel; v += std::max(1, n_vel / 64)) s += llabs((long long)cdx[(size_t)v * T + t]) + llabs((long long)cdy[(size_t)v * T + t]);
-            if (s > best) { best = s; t_far = t; }
+    // ---- the plan depends only on the geometry (T, H, W and the displacement table): searching the CCDs of one
+    // pointing group, or the AUTO decision followed by the search itself, reuses it (one entry per host thread)
+    static thread_local PlanCache PC;
+    const bool plan_hit = PC.valid && PC.T == T && PC.H == H && PC.W == W && PC.n_vel == n_vel &&
+                          PC.kdx.size() == cdx.size() && (cdx.empty() || (memcmp(PC.kdx.data(), cdx.data(), cdx.size() * 4) == 0 &&
+                                                                        memcmp(PC.kdy.data(), cdy.data(), cdy.size() * 4) == 0));
+    const int tiles_x = (W + PR_TW - 1) / PR_TW, tiles_y = (H + PR_TH - 1) / PR_TH;
+    const int ring_bytes = ring_bytes_for(T);
+    if (!plan_hit) {
+        PC.valid = false;
+        Planner pl;
+        pl.T = T; pl.n_vel = n_vel; pl.ring_bytes = ring_bytes_for(T);
+        pl.max_region = (pl.ring_bytes / 2 / 1024) * 1024;
+        pl.dx = cdx.data(); pl.dy = cdy.data();
+        int t_far = 0;
+        {   // epoch with the largest displacement spread
+            long long best = -1;
+            for (int t = 0; t < T; ++t) {
+                long long s = 0;
+                for (int v = 0; v < n_vel; v += std::max(1, n_vel / 64)) s += llabs((long long)cdx[(size_t)v * T + t]) + llabs((long long)cdy[(size_t)v * T + t]);
+                if (s > best) { best = s; t_far = t; }
+            }
         }
+        pl.idx.resize(n_vel); pl.px.resize(n_vel); pl.py.resize(n_vel);
+        for (int v = 0; v < n_vel; ++v) {
+            pl.idx[v] = v;
+            pl.px[v] = cdx[(size_t)v * T + t_far];
+            pl.py[v] = cdy[(size_t)v * T + t_far];
+        }
+        if (n_vel > 0) pl.split(0, n_vel);
+        const int ng = (int)pl.leaves.size();
+        // ---- tables: gvel, per-group blocks {offs[T][G], ge[T]}, ring chain
+        std::vector<int32_t>& gvel = PC.gvel;
+        std::vector<unsigned char>& gtbl = PC.gtbl;
+        gvel.assign((size_t)ng * PR_G, -1);
+        gtbl.assign((size_t)ng * TBL, 0);
+        double staged = 0.0, evals = 0.0;
+        uint32_t ph = 0;
+        for (int g = 0; g < ng; ++g) {
+            if (g % PR_SUB == 0) ph = 0;  // every work unit starts its ring chain at offset 0
+            const int lo = pl.leaves[g].first, cnt = pl.leaves[g].second - pl.leaves[g].first;
+            for (int j = 0; j < cnt; ++j) gvel[(size_t)g * PR_G + j] = pl.idx[lo + j];
+            int32_t* offs = reinterpret_cast<int32_t*>(gtbl.data() + (size_t)g * TBL);
+            GroupEpoch* ge = reinterpret_cast<GroupEpoch*>(gtbl.data() + (size_t)g * TBL + (size_t)T * PR_G * 4);
+            for (int t = 0; t < T; ++t) {
+                GroupEpoch e;
+                memset(&e, 0, sizeof(e));
+                int x0, y0;
+                const long long bytes = pl.region(lo, lo + cnt, t, &e, &x0, &y0);
+                KB_REQUIRE(bytes > 0 && bytes <= pl.max_region, KBMOD_ERR_UNSUPPORTED, "planner: region of %lld bytes", bytes);
+                const int pitch = PR_TW + 16 * (int)(e.pitch_k & 0xFF);
+                for (int j = 0; j < cnt; ++j) {
+                    const int v = pl.idx[lo + j];
+                    offs[t * PR_G + j] = ((cdy[(size_t)v * T + t] - y0) * pitch + (cdx[(size_t)v * T + t] - x0)) * (int)sizeof(unsigned int);
+                }
+                uint32_t pad = 0;
+                if (ph + (uint32_t)bytes > (uint32_t)pl.ring_bytes) { pad = (uint32_t)pl.ring_bytes - ph; ph = 0; }
+                e.smem_off = ph;
+                e.footprint = (uint32_t)bytes + pad;
+                e.vmask = cnt >= 32 ? 0xFFFFFFFFu : ((1u << cnt) - 1u);
+                bool same = true;
+                for (int j = 1; j < cnt; ++j) same = same && offs[t * PR_G + j] == offs[t * PR_G];
+                if (same) e.pitch_k |= 0x100;
+                ph += (uint32_t)bytes;
+                ge[t] = e;
+                staged += (double)bytes;
+            }
+            evals += (double)PR_TW * PR_TH * cnt * T;
+        }
+        // on-image masks: region t of group g touches the image iff the tile column AND the tile row allow it
+        std::vector<unsigned long long>&maskx = PC.maskx, &masky = PC.masky;
+        std::vector<uint32_t>& gfoot = PC.gfoot;
+        maskx.assign((size_t)ng * tiles_x, 0ull);
+        masky.assign((size_t)ng * tiles_y, 0ull);
+        gfoot.assign((size_t)ng, 0u);
+        for (int g = 0; g < ng; ++g) {
+            const GroupEpoch* ge = reinterpret_cast<const GroupEpoch*>(gtbl.data() + (size_t)g * TBL + (size_t)T * PR_G * 4);
+            unsigned long long foot = 0;
+            for (int t = 0; t < T; ++t) {
+                const long long pitch = PR_TW + 16 * (long long)(ge[t].pitch_k & 0xFF), rows = (long long)ge[t].n_box * PR_RB;
+                for (int c = 0; c < tiles_x; ++c) {
+                    const long long x0 = (long long)c * PR_TW + ge[t].ox;
+                    if (x0 < W && x0 + pitch > 0) maskx[(size_t)g * tiles_x + c] |= 1ull << t;
+                }
+                for (int r = 0; r < tiles_y; ++r) {
+                    const long long y0 = (long long)r * PR_TH + ge[t].oy;
+                    if (y0 < H && y0 + rows > 0) masky[(size_t)g * tiles_y + r] |= 1ull << t;
+                }
+                foot += ge[t].footprint;
+            }
+            gfoot[g] = (uint32_t)std::min<unsigned long long>(foot, 0xFFFFFFFFull);  // > ring / 2 is all that matters
+        }
+        PC.T = T; PC.H = H; PC.W = W; PC.n_vel = n_vel;
+        PC.kdx = cdx; PC.kdy = cdy;
+        PC.ng = ng; PC.staged = staged; PC.evals = evals;
+        PC.valid = true;
     }
-    pl.idx.resize(n_vel); pl.px.resize(n_vel); pl.py.resize(n_vel);
-    for (int v = 0; v < n_vel; ++v) {
-        pl.idx[v] = v;
-        pl.px[v] = cdx[(size_t)v * T + t_far];
-        pl.py[v] = cdy[(size_t)v * T + t_far];
-    }
-    if (n_vel > 0) pl.split(0, n_vel);
-    const int ng = (int)pl.leaves.size();
+    const int ng = PC.ng;
+    const double staged = PC.staged, evals = PC.evals;
+    const std::vector<int32_t>& gvel = PC.gvel;
+    const std::vector<unsigned char>& gtbl = PC.gtbl;
+    const std::vector<unsigned long long>&maskx = PC.maskx, &masky = PC.masky;
+    const std::vector<uint32_t>& gfoot = PC.gfoot;
     const size_t ngm = max_groups(n_vel);
     // launches cover (a batch of whole waves of tiles) x (a chunk of the groups), sized so that 1/4 of the launch's
     // trajectories fit the survivor queue (what does not fit is evaluated wholesale by the overflow kernel)
@@ -915,63 +1008,6 @@ int kb_launch_search_pruned(const float* d_psiphi, int T, int TPv, int H, int W,
     const int n_chunks = std::max(1, std::min(std::max(ng, 1), (int)ceil(wave_nominal / budget)));
     const int groups_per_chunk = ((std::max(1, (ng + n_chunks - 1) / n_chunks) + PR_SUB - 1) / PR_SUB) * PR_SUB;
 
-    // ---- tables: gvel, per-group blocks {offs[T][G], ge[T]}, ring chain
-    std::vector<int32_t> gvel((size_t)ng * PR_G, -1);
-    std::vector<unsigned char> gtbl((size_t)ng * TBL, 0);
-    double staged = 0.0, evals = 0.0;
-    uint32_t ph = 0;
-    for (int g = 0; g < ng; ++g) {
-        if (g % PR_SUB == 0) ph = 0;  // every work unit starts its ring chain at offset 0
-        const int lo = pl.leaves[g].first, cnt = pl.leaves[g].second - pl.leaves[g].first;
-        for (int j = 0; j < cnt; ++j) gvel[(size_t)g * PR_G + j] = pl.idx[lo + j];
-        int32_t* offs = reinterpret_cast<int32_t*>(gtbl.data() + (size_t)g * TBL);
-        GroupEpoch* ge = reinterpret_cast<GroupEpoch*>(gtbl.data() + (size_t)g * TBL + (size_t)T * PR_G * 4);
-        for (int t = 0; t < T; ++t) {
-            GroupEpoch e;
-            memset(&e, 0, sizeof(e));
-            int x0, y0;
-            const long long bytes = pl.region(lo, lo + cnt, t, &e, &x0, &y0);
-            KB_REQUIRE(bytes > 0 && bytes <= pl.max_region, KBMOD_ERR_UNSUPPORTED, "planner: region of %lld bytes", bytes);
-            const int pitch = PR_TW + 16 * (int)(e.pitch_k & 0xFF);
-            for (int j = 0; j < cnt; ++j) {
-                const int v = pl.idx[lo + j];
-                offs[t * PR_G + j] = ((cdy[(size_t)v * T + t] - y0) * pitch + (cdx[(size_t)v * T + t] - x0)) * (int)sizeof(unsigned int);
-            }
-            uint32_t pad = 0;
-            if (ph + (uint32_t)bytes > (uint32_t)pl.ring_bytes) { pad = (uint32_t)pl.ring_bytes - ph; ph = 0; }
-            e.smem_off = ph;
-            e.footprint = (uint32_t)bytes + pad;
-            e.vmask = cnt >= 32 ? 0xFFFFFFFFu : ((1u << cnt) - 1u);
-            bool same = true;
-            for (int j = 1; j < cnt; ++j) same = same && offs[t * PR_G + j] == offs[t * PR_G];
-            if (same) e.pitch_k |= 0x100;
-            ph += (uint32_t)bytes;
-            ge[t] = e;
-            staged += (double)bytes;
-        }
-        evals += (double)PR_TW * PR_TH * cnt * T;
-    }
-    // on-image masks: region t of group g touches the image iff the tile column AND the tile row allow it
-    const int tiles_x = (W + PR_TW - 1) / PR_TW, tiles_y = (H + PR_TH - 1) / PR_TH;
-    std::vector<unsigned long long> maskx((size_t)ng * tiles_x, 0ull), masky((size_t)ng * tiles_y, 0ull);
-    std::vector<uint32_t> gfoot((size_t)ng, 0u);
-    for (int g = 0; g < ng; ++g) {
-        const GroupEpoch* ge = reinterpret_cast<const GroupEpoch*>(gtbl.data() + (size_t)g * TBL + (size_t)T * PR_G * 4);
-        unsigned long long foot = 0;
-        for (int t = 0; t < T; ++t) {
-            const long long pitch = PR_TW + 16 * (long long)(ge[t].pitch_k & 0xFF), rows = (long long)ge[t].n_box * PR_RB;
-            for (int c = 0; c < tiles_x; ++c) {
-                const long long x0 = (long long)c * PR_TW + ge[t].ox;
-                if (x0 < W && x0 + pitch > 0) maskx[(size_t)g * tiles_x + c] |= 1ull << t;
-            }
-            for (int r = 0; r < tiles_y; ++r) {
-                const long long y0 = (long long)r * PR_TH + ge[t].oy;
-                if (y0 < H && y0 + rows > 0) masky[(size_t)g * tiles_y + r] |= 1ull << t;
-            }
-            foot += ge[t].footprint;
-        }
-        gfoot[g] = (uint32_t)std::min<unsigned long long>(foot, 0xFFFFFFFFull);  // > ring / 2 is all that matters
-    }
     if (plan_stats) {
         plan_stats[0] = (size_t)ng > ngm ? 1.0 : 0.0;       // the velocity list is too scattered to group
         plan_stats[1] = evals > 0 ? staged / evals : 0.0;   // staged bytes per evaluation
@@ -1040,10 +1076,10 @@ int kb_launch_search_pruned(const float* d_psiphi, int T, int TPv, int H, int W,
     long long waves = (long long)(budget / std::max(1.0, wave_nominal / n_chunks));
     waves = std::max<long long>(1, std::min<long long>(PR_WAVES_PER_BATCH, waves));
     const int batch = (int)std::min<long long>((long long)n_tiles, waves * grid);
-    const size_t smem1 = (size_t)pl.ring_bytes + (size_t)PR_NTBL * TBL + PR_SMEM_MISC;
+    const size_t smem1 = (size_t)ring_bytes + (size_t)PR_NTBL * TBL + PR_SMEM_MISC;
     KB_CUDA(cudaFuncSetAttribute(bound_phase_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem1));
     PrunedTables tb{d_gvel, d_gtbl, (const unsigned long long*)(w + L.maskx), (const unsigned long long*)(w + L.masky),
-                    (const uint32_t*)(w + L.gfoot), ng, pl.ring_bytes};
+                    (const uint32_t*)(w + L.gfoot), ng, ring_bytes};
     const float2* psiphi2 = reinterpret_cast<const float2*>(d_psiphi);
     KB_DISPATCH_TP(TPv, {
         const size_t smem2 = (size_t)TP * EX_THREADS * sizeof(float);
