@@ -120,7 +120,10 @@ int kbmod_displacements(const double* h_times, int T, const float* h_vx, const f
  *   d_workspace caller-owned scratch of at least kbmod_search_workspace_bytes(...) bytes,
  *               256-byte aligned; contents undefined on entry and exit.
  * kbmod_search does host-side planning (the displacement table and the velocity grouping), copies
- * small tables to the workspace with cudaMemcpyAsync on `stream`, and enqueues the kernels. */
+ * small tables to the workspace with cudaMemcpyAsync on `stream`, and enqueues the kernels.  The
+ * geometry-only part of the plan is kept per host thread and reused while T, H, W and the displacement
+ * table are unchanged.  Test hook: the environment variable KBMOD_B200_QUEUE_CAP=<entries> shrinks the
+ * internal survivor queue of the pruned kernel (results are unaffected; it exercises the overflow path). */
 size_t kbmod_search_workspace_bytes(int T, int H, int W, int n_vel, const kbmod_search_params* p);
 int kbmod_search(const float* d_psiphi, int T, int H, int W, const double* h_times, const float* h_vx,
                  const float* h_vy, int n_vel, const kbmod_search_params* p, float* d_lh, float* d_flux,
