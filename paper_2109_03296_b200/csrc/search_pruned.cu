@@ -54,8 +54,13 @@ constexpr int PR_NB = KB_NB;               // regions in flight (mbarrier pairs)
 constexpr int PR_NTBL = 4;                 // group tables in flight
 constexpr int PR_SMEM_MAX = 232448;        // 227 KB: the opt-in maximum of dynamic shared memory per CTA
 constexpr int PR_SMEM_MISC = 512;          // barriers + producer bookkeeping
+static_assert(PR_NB * 16 + 16 + 8 + PR_NB * 4 <= PR_SMEM_MISC, "full/empty barriers, unit mailbox and footprints must fit");
+static_assert((PR_NB & (PR_NB - 1)) == 0, "PR_NB must be a power of two");
 constexpr int PR_WAVES_PER_BATCH = 7;
-constexpr int PR_SUB = 8;                  // groups per work unit: CTAs take (tile, PR_SUB groups) units dynamically
+#ifndef KB_SUB
+#define KB_SUB 8
+#endif
+constexpr int PR_SUB = KB_SUB;                  // groups per work unit: CTAs take (tile, PR_SUB groups) units dynamically
 // 20 warps = 5 per scheduler: 16384 registers / (5 x 32) = 102 -> 96 per thread at launch.  setmaxnreg moves
 // registers inside the CTA's own allocation (640 x 96 = 61440): the producer warp group drops to 24 and the
 // 16 consumer warps rise (512 x 104 + 128 x 56 = 60416 <= 61440)
