@@ -468,17 +468,14 @@ bound_phase_kernel(const __grid_constant__ TensorMaps maps, int T, int H, int W,
             unsigned int ANU[PR_PIX];
 #pragma unroll
             for (int i = 0; i < PR_PIX; ++i) ANU[i] = 0u;
-            uint2 gw = make_uint2(0u, 0u);  // {pitch_k | uniform << 8 | n_box << 16, smem_off} of the next epoch
             unsigned long long rem = on;  // bit 0 is always set: epoch 0 has no displacement
 #pragma unroll 1
             while (rem) {
                 const int t = __ffsll((long long)rem) - 1;
                 rem &= rem - 1;
                 const int slot = q & (PR_NB - 1);
-                kb_mbar_wait(&full[slot], (q / PR_NB) & 1);
-                if (t == 0) gw = *reinterpret_cast<const uint2*>(&ge[0].pitch_k);  // the tables came with this region
-                const uint2 cur = gw;
-                if (rem) gw = *reinterpret_cast<const uint2*>(&ge[__ffsll((long long)rem) - 1].pitch_k);
+                kb_mbar_wait(&full[slot], (q / PR_NB) & 1);  // (the group's tables came with the region of epoch 0)
+                const uint2 cur = *reinterpret_cast<const uint2*>(&ge[t].pitch_k);  // {pitch_k | uniform << 8 | n_box << 16, smem_off}
                 const int pitch = PR_TW + 16 * (int)(cur.x & 0xFFu);
                 const unsigned char* base = smem + cur.y + (size_t)(warp * pitch + lane) * sizeof(unsigned int);
                 const int rows16 = 16 * pitch * (int)sizeof(unsigned int);  // this thread's second row of pixels
@@ -491,6 +488,45 @@ bound_phase_kernel(const __grid_constant__ TensorMaps maps, int T, int H, int W,
                         ANU[2 * v + 1] += pv[32];
                     }
                 } else {
+                    // two non-uniform epochs at a time: one three-operand add takes both words
+                    const int t2 = rem ? __ffsll((long long)rem) - 1 : -1;
+                    const uint2 cur2 = (t2 >= 0) ? *reinterpret_cast<const uint2*>(&ge[t2].pitch_k) : make_uint2(0x100u, 0u);
+                    // ... if the second region has landed already: waiting for it while holding the first could
+                    // deadlock against the producer waiting for ring space (lane 0 decides for the warp)
+                    const int slot2 = (q + 1) & (PR_NB - 1);
+                    const bool both = !(cur2.x & 0x100u) &&
+                                      __shfl_sync(0xFFFFFFFFu, (int)kb_mbar_test(&full[slot2], ((q + 1) / PR_NB) & 1), 0) != 0;
+                    if (both) {
+                        rem &= rem - 1;
+                        kb_mbar_wait(&full[slot2], ((q + 1) / PR_NB) & 1);  // completed: acquires it for every lane
+                        const int pitch2 = PR_TW + 16 * (int)(cur2.x & 0xFFu);
+                        const unsigned char* base2 = smem + cur2.y + (size_t)(warp * pitch2 + lane) * sizeof(unsigned int);
+                        const int rows16b = 16 * pitch2 * (int)sizeof(unsigned int);
+#pragma unroll
+                        for (int k = 0; k < PR_G / 4; ++k) {
+                            const int4 o = offs4[t * (PR_G / 4) + k], o2 = offs4[t2 * (PR_G / 4) + k];
+                            const int oo[4] = {o.x, o.y, o.z, o.w}, oo2[4] = {o2.x, o2.y, o2.z, o2.w};
+#pragma unroll
+                            for (int i = 0; i < 4; ++i) {
+                                const unsigned char* p = base + oo[i];
+                                const unsigned char* p2 = base2 + oo2[i];
+#pragma unroll
+                                for (int v = 0; v < PR_TH / 16; ++v) {
+                                    const unsigned int* pv = reinterpret_cast<const unsigned int*>(p + v * rows16);
+                                    const unsigned int* pv2 = reinterpret_cast<const unsigned int*>(p2 + v * rows16b);
+                                    AN[2 * v][4 * k + i] += pv[0] + pv2[0];
+                                    AN[2 * v + 1][4 * k + i] += pv[32] + pv2[32];
+                                }
+                            }
+                        }
+                        __syncwarp();
+                        if (lane == 0) {
+                            kb_mbar_arrive(&empty[slot]);
+                            kb_mbar_arrive(&empty[slot2]);
+                        }
+                        q += 2;
+                        continue;
+                    }
 #pragma unroll
                     for (int k = 0; k < PR_G / 4; ++k) {
                         const int4 o = offs4[t * (PR_G / 4) + k];  // byte offsets inside the region

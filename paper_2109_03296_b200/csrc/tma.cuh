@@ -31,6 +31,17 @@ __device__ __forceinline__ void kb_mbar_wait(uint64_t* bar, uint32_t parity) {
         "KB_DONE_%=:\n\t"
         "}" ::"r"(kb_smem_u32(bar)), "r"(parity), "r"(2000u) : "memory");
 }
+// non-blocking test of a phase (acquire): true once the phase with this parity has completed
+__device__ __forceinline__ bool kb_mbar_test(uint64_t* bar, uint32_t parity) {
+    uint32_t ok;
+    asm volatile(
+        "{\n\t"
+        ".reg .pred p;\n\t"
+        "mbarrier.test_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+        "selp.u32 %0, 1, 0, p;\n\t"
+        "}" : "=r"(ok) : "r"(kb_smem_u32(bar)), "r"(parity) : "memory");
+    return ok != 0;
+}
 // generic-proxy writes to shared memory (st.shared) must be ordered before async-proxy (TMA) writes
 __device__ __forceinline__ void kb_fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 
