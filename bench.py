@@ -273,9 +273,10 @@ def run_ours(args):
         seg["prep"].append(e[0].elapsed_time(e[1])); seg["search"].append(e[1].elapsed_time(e[2]))
         seg["coadd"].append(e[2].elapsed_time(e[3]))
     stats = kb.kbmod_search_stats(ws)  # [evaluated, nominal, launches, algo]
+    smem_gbs = {b: kb.kbmod_measure_smem_gbs(b) for b in (4, 16)}  # after the timed region
     return dict(torch=torch, dist=dist, kb=kb, rank=rank, world=world, dev=dev, st=st, vx=vx, vy=vy, pd=pd, sp=sp,
                 desc=desc, evals=evals, total_ms=total_ms, seg=seg, stats=stats, clocks=clocks, peaks=peaks, phases=phases,
-                n_cand=n_cand, out=out)
+                n_cand=n_cand, out=out, smem_gbs=smem_gbs)
 
 
 def max_over_ranks(ms_local: float, dist, device, world: int) -> float:
@@ -347,10 +348,13 @@ def report(R, args):
                     peak_source="derived: 148 SMs x 128 FP32/ALU lanes x sm_max_mhz (DESIGN.md)")
     else:
         byts = R["evals"] * 4.0  # one packed 32-bit bound word per trajectory-epoch evaluation
-        peak = N_SM * 128 * f_max / 1e9
+        # denominator: the shared-memory load bandwidth measured live on this GPU (LDS.128 microbenchmark of the
+        # library: the highest of the three widths); the derived figure and the LDS.32 figure are quoted beside it
+        peak = R["smem_gbs"][16]
         roof = dict(bound="smem", achieved=byts / (kernel_ms * 1e-3) / 1e9, peak=peak,
                     unit="GB/s", kernel="bound_phase_kernel",
-                    peak_source="derived: 148 SMs x 128 B/clk shared-memory bandwidth x sm_max_mhz (DESIGN.md)",
+                    peak_source="measured live: kbmod_measure_smem_gbs(16), conflict-free LDS.128 on all SMs",
+                    peak_theoretical=N_SM * 128 * f_max / 1e9, peak_measured_lds32=R["smem_gbs"][4],
                     algorithmic_bytes_per_eval=4,
                     # SURVEY 8(d) counted 8 B (psi, phi as float32) per evaluation; against that figure:
                     frac_of_survey_8B_roofline=2.0 * byts / (kernel_ms * 1e-3) / 1e9 / peak,

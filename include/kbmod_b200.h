@@ -202,6 +202,11 @@ int kbmod_pipeline_host(const float* h_img, const float* h_var, const uint8_t* h
                         const float* h_vy, int n_vel, const kbmod_search_params* p, float* h_lh, float* h_flux,
                         int32_t* h_vel_idx, int32_t* h_n_obs, void* d_arena, size_t arena_bytes, void* stream);
 
+/* Measurement helper for the roofline denominator (not part of the search path; synchronises; allocates 4 bytes):
+ * streams conflict-free shared-memory loads of bytes_per_lane = 4, 8 or 16 on every SM and returns the best of three
+ * timed repetitions in GB/s.  The theoretical figure is SMs x 128 B/clk x SM clock. */
+int kbmod_measure_smem_gbs(int bytes_per_lane, double* h_gbs, void* stream);
+
 const char* kbmod_last_error(void); /* thread-local, never NULL */
 int kbmod_version(void);            /* 10000*major + 100*minor + patch */
 

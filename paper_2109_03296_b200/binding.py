@@ -20,7 +20,7 @@ EXPORTS = ["kbmod_default_params", "kbmod_prepare_psi_phi", "kbmod_displacements
            "kbmod_search_workspace_bytes", "kbmod_search", "kbmod_search_stats", "kbmod_search_phase_timing",
            "kbmod_search_phase_ms", "kbmod_coadd_stamps",
            "kbmod_eval_trajectories", "kbmod_sigmag_filter", "kbmod_stamp_moments", "kbmod_pipeline_host_arena_bytes",
-           "kbmod_pipeline_host", "kbmod_last_error", "kbmod_version"]
+           "kbmod_pipeline_host", "kbmod_measure_smem_gbs", "kbmod_last_error", "kbmod_version"]
 
 
 class KbmodError(RuntimeError):
@@ -258,6 +258,13 @@ def kbmod_stamp_moments(stamps, thresholds=None, stream=None):
         raise KbmodError(-1, "thresholds must be 5 numbers: x, y, xy, xx, yy")
     _check(lib().kbmod_stamp_moments(s, C.c_int(n), C.c_int(S // 2), thr_ptr, _dev(mom), _dev(keep), _stream(stream)))
     return mom, keep
+
+
+def kbmod_measure_smem_gbs(bytes_per_lane: int = 4, stream=None) -> float:
+    """Measured shared-memory load bandwidth of the whole GPU in GB/s (roofline denominator; synchronises)."""
+    out = C.c_double(0.0)
+    _check(lib().kbmod_measure_smem_gbs(C.c_int(bytes_per_lane), C.byref(out), _stream(stream)))
+    return float(out.value)
 
 
 def kbmod_pipeline_host_arena_bytes(T, H, W, n_vel, params: SearchParams) -> int:

@@ -1,0 +1,77 @@
+// Measurement helper for the roofline denominator ("re-measure the SMEM peak with an LDS microbenchmark
+// at the clocks the kernel actually holds"): every SM streams conflict-free shared-memory loads of 4, 8 or 16 bytes
+// per lane, many independent loads in flight per thread, nothing else in the loop.  Not part of the search path.
+#include "common.cuh"
+
+namespace {
+
+constexpr int SP_THREADS = 1024, SP_LOADS = 8;  // 8 distinct vectors per thread and iteration: 8 x 1024 x sizeof(V) bytes
+
+template <typename V>
+__global__ void __launch_bounds__(SP_THREADS) smem_peak_kernel(int iters, unsigned int* __restrict__ sink) {
+    extern __shared__ __align__(16) unsigned int buf[];
+    constexpr int PER = sizeof(V) / 4;                  // words per lane and load
+    constexpr int NV = SP_LOADS * SP_THREADS;           // vectors in the buffer
+    for (int i = threadIdx.x; i < NV * PER; i += SP_THREADS) buf[i] = i * 2654435761u;
+    __syncthreads();
+    const V* v = reinterpret_cast<const V*>(buf);
+    unsigned int acc = 0;
+    int idx = threadIdx.x;                              // consecutive lanes -> consecutive vectors: conflict-free
+#pragma unroll 1
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int u = 0; u < SP_LOADS; ++u) {
+            const V x = v[(idx + u * SP_THREADS) & (NV - 1)];
+            const unsigned int* w = reinterpret_cast<const unsigned int*>(&x);
+#pragma unroll
+            for (int k = 0; k < PER; ++k) acc += w[k];
+        }
+        idx = (idx + 32) & (NV - 1);                    // another warp's vectors next time: nothing to hoist
+    }
+    if (acc == 0x12345678u) sink[0] = acc;              // keeps the loads alive
+}
+
+template <typename V>
+int run_peak(int iters, int grid, unsigned int* sink, cudaStream_t st) {
+    const int smem = SP_LOADS * SP_THREADS * (int)sizeof(V);
+    KB_CUDA(cudaFuncSetAttribute(smem_peak_kernel<V>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+    smem_peak_kernel<V><<<grid, SP_THREADS, smem, st>>>(iters, sink);
+    return KBMOD_OK;
+}
+
+}  // namespace
+
+extern "C" int kbmod_measure_smem_gbs(int bytes_per_lane, double* h_gbs, void* stream) {
+    KB_REQUIRE(h_gbs, KBMOD_ERR_INVALID_ARG, "NULL argument");
+    KB_REQUIRE(bytes_per_lane == 4 || bytes_per_lane == 8 || bytes_per_lane == 16, KBMOD_ERR_INVALID_ARG,
+               "bytes_per_lane = %d must be 4, 8 or 16", bytes_per_lane);
+    cudaStream_t st = (cudaStream_t)stream;
+    int dev = 0, n_sm = 0;
+    KB_CUDA(cudaGetDevice(&dev));
+    KB_CUDA(cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev));
+    unsigned int* sink = nullptr;
+    KB_CUDA(cudaMalloc(&sink, 4));  // measurement helper only: the search path never allocates
+    cudaEvent_t e0, e1;
+    KB_CUDA(cudaEventCreate(&e0));
+    KB_CUDA(cudaEventCreate(&e1));
+    const int iters = 8000, grid = n_sm;
+    double best = 0.0;
+    for (int rep = 0; rep < 4; ++rep) {  // first repetition warms up
+        KB_CUDA(cudaEventRecord(e0, st));
+        int rc = bytes_per_lane == 4 ? run_peak<unsigned int>(iters, grid, sink, st)
+                 : bytes_per_lane == 8 ? run_peak<uint2>(iters, grid, sink, st) : run_peak<uint4>(iters, grid, sink, st);
+        if (rc) return rc;
+        KB_CUDA(cudaEventRecord(e1, st));
+        KB_CUDA(cudaEventSynchronize(e1));
+        float ms = 0.0f;
+        KB_CUDA(cudaEventElapsedTime(&ms, e0, e1));
+        const double bytes = (double)grid * SP_THREADS * (double)iters * SP_LOADS * bytes_per_lane;
+        if (rep > 0) best = fmax(best, bytes / (ms * 1e-3) / 1e9);
+    }
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    cudaFree(sink);
+    KB_CUDA(cudaGetLastError());
+    *h_gbs = best;
+    return KBMOD_OK;
+}

@@ -591,3 +591,13 @@ def test_sigmag_refilter_one_million_candidates(kb, oracle):
         assert np.all(np.abs(g["lh"][has] - o["lh"][has]) <= tl[has])
         assert np.all(np.abs(g["flux"][has] - o["flux"][has]) <= tf[has])
         assert np.all(np.isneginf(g["lh"][~has]))
+
+
+def test_measured_smem_peak_is_plausible(kb):
+    """The roofline denominator bench.py measures live: within 25 % of SMs x 128 B/clk x max SM clock."""
+    import torch
+    props = torch.cuda.get_device_properties(0)
+    theo = props.multi_processor_count * 128 * 1.965  # GB/s at 1965 MHz
+    for width in (4, 8, 16):
+        gbs = kb.kbmod_measure_smem_gbs(width)
+        assert 0.6 * theo < gbs < 1.1 * theo, (width, gbs, theo)
