@@ -374,7 +374,8 @@ def report(R, args):
                 data="synthetic",
                 config=dict(workload=R["desc"], min_lh=args.min_lh, min_obs=sp.min_obs, sigma_g="on",
                             algo={1: "direct", 2: "pruned"}.get(algo_used, "?"), coadd_candidates=R["n_cand"],
-                            l2="inputs larger than L2 (psi/phi stack %.2f GB)" % (T * H * W * 8 / 1e9),
+                            l2=("inputs larger than L2 (psi/phi stack %.2f GB)" % (T * H * W * 8 / 1e9)) if T * H * W * 8 > 2.6e8 else
+                               "inputs SMALLER than L2 and no flush: a parity-test configuration, not a cold-cache measurement",
                             multi_gpu="one independent CCD stack per rank, no collective" if world > 1 else "single GPU",
                             host_plan="velocity grouping / staging geometry cached after the first (warm-up) step: same grid and times"),
                 segments_ms={k: float(np.mean(v)) for k, v in R["seg"].items()},
