@@ -202,6 +202,18 @@ int kbmod_pipeline_host(const float* h_img, const float* h_var, const uint8_t* h
                         const float* h_vy, int n_vel, const kbmod_search_params* p, float* h_lh, float* h_flux,
                         int32_t* h_vel_idx, int32_t* h_n_obs, void* d_arena, size_t arena_bytes, void* stream);
 
+/* The same for n_stacks stacks of one shape searched with one grid (the 60 CCDs of a pointing group):
+ * h_img[i], h_var[i], h_mask[i] (h_mask may be NULL) and the four result pointers per stack.  The copies of stack
+ * i + 1 and of the results of stack i - 1 overlap the search of stack i (two internal copy streams, created once
+ * per host thread; kernels run on `stream`).  d_arena: at least 2 x kbmod_pipeline_host_arena_bytes(...) bytes
+ * (1 x for a single stack).  Synchronises `stream` (which then also waits for the last results) before returning. */
+int kbmod_pipeline_host_batch(int n_stacks, const float* const* h_img, const float* const* h_var,
+                              const uint8_t* const* h_mask, int T, int H, int W, const float* h_psf, int n_psf, int k,
+                              const double* h_times, const float* h_vx, const float* h_vy, int n_vel,
+                              const kbmod_search_params* p, float* const* h_lh, float* const* h_flux,
+                              int32_t* const* h_vel_idx, int32_t* const* h_n_obs, void* d_arena, size_t arena_bytes,
+                              void* stream);
+
 /* Measurement helper for the roofline denominator (not part of the search path; synchronises; allocates 4 bytes):
  * streams conflict-free shared-memory loads of bytes_per_lane = 4, 8 or 16 on every SM and returns the best of three
  * timed repetitions in GB/s.  The theoretical figure is SMs x 128 B/clk x SM clock. */

@@ -20,7 +20,7 @@ EXPORTS = ["kbmod_default_params", "kbmod_prepare_psi_phi", "kbmod_displacements
            "kbmod_search_workspace_bytes", "kbmod_search", "kbmod_search_stats", "kbmod_search_phase_timing",
            "kbmod_search_phase_ms", "kbmod_coadd_stamps",
            "kbmod_eval_trajectories", "kbmod_sigmag_filter", "kbmod_stamp_moments", "kbmod_pipeline_host_arena_bytes",
-           "kbmod_pipeline_host", "kbmod_measure_smem_gbs", "kbmod_last_error", "kbmod_version"]
+           "kbmod_pipeline_host", "kbmod_pipeline_host_batch", "kbmod_measure_smem_gbs", "kbmod_last_error", "kbmod_version"]
 
 
 class KbmodError(RuntimeError):
@@ -258,6 +258,33 @@ def kbmod_stamp_moments(stamps, thresholds=None, stream=None):
         raise KbmodError(-1, "thresholds must be 5 numbers: x, y, xy, xx, yy")
     _check(lib().kbmod_stamp_moments(s, C.c_int(n), C.c_int(S // 2), thr_ptr, _dev(mom), _dev(keep), _stream(stream)))
     return mom, keep
+
+
+def kbmod_pipeline_host_batch(stacks, psf, times, vx, vy, params: SearchParams, outs, arena, stream=None):
+    """`stacks`: list of (img, var, mask-or-None) CPU tensors of one shape; `outs`: list of 4-tuples of CPU tensors
+    [H][W][K]; `arena`: uint8 CUDA tensor of at least 2 x kbmod_pipeline_host_arena_bytes (1 x for one stack).
+    Copies overlap the searches; synchronises before returning."""
+    n = len(stacks)
+    T, H, W = stacks[0][0].shape
+    p, pp = _host(psf, np.float32)
+    n_psf = 1 if p.ndim == 2 else p.shape[0]
+    t, tp = _host(times, np.float64)
+    x, xp = _host(vx, np.float32)
+    y, yp = _host(vy, np.float32)
+    has_mask = stacks[0][2] is not None
+    for st_ in stacks:
+        assert tuple(st_[0].shape) == (T, H, W) and (st_[2] is not None) == has_mask
+        for a in st_:
+            assert a is None or (not a.is_cuda and a.is_contiguous())
+    arr = lambda items: (C.c_void_p * n)(*[C.c_void_p(a.data_ptr()) for a in items])
+    imgs, vars_ = arr([s_[0] for s_ in stacks]), arr([s_[1] for s_ in stacks])
+    masks = arr([s_[2] for s_ in stacks]) if has_mask else None
+    o = [arr([o_[j] for o_ in outs]) for j in range(4)]
+    cp = params.c()
+    _check(lib().kbmod_pipeline_host_batch(C.c_int(n), imgs, vars_, masks, T, H, W, pp, n_psf, p.shape[-1], tp, xp, yp, len(x),
+                                           C.byref(cp), o[0], o[1], o[2], o[3], _dev(arena), C.c_size_t(arena.numel()),
+                                           _stream(stream)))
+    return outs
 
 
 def kbmod_measure_smem_gbs(bytes_per_lane: int = 4, stream=None) -> float:

@@ -438,3 +438,84 @@ extern "C" int kbmod_pipeline_host(const float* h_img, const float* h_var, const
     KB_CUDA(cudaStreamSynchronize(st));
     return KBMOD_OK;
 }
+
+// ---------------------------------------------------------------------------------------------
+// a batch of stacks of one shape (the CCDs of a pointing group): copies overlap the searches
+struct BatchStreams {
+    cudaStream_t s_in = nullptr, s_out = nullptr;
+    cudaEvent_t in_done[2] = {nullptr, nullptr}, comp_done[2] = {nullptr, nullptr}, out_done[2] = {nullptr, nullptr};
+    bool ready = false;
+};
+static thread_local BatchStreams g_bs;
+
+extern "C" int kbmod_pipeline_host_batch(int n_stacks, const float* const* h_img, const float* const* h_var,
+                                         const uint8_t* const* h_mask, int T, int H, int W, const float* h_psf, int n_psf,
+                                         int k, const double* h_times, const float* h_vx, const float* h_vy, int n_vel,
+                                         const kbmod_search_params* p, float* const* h_lh, float* const* h_flux,
+                                         int32_t* const* h_vel_idx, int32_t* const* h_n_obs, void* d_arena,
+                                         size_t arena_bytes, void* stream) {
+    KB_REQUIRE(n_stacks >= 0, KBMOD_ERR_INVALID_ARG, "n_stacks = %d", n_stacks);
+    if (n_stacks == 0) return KBMOD_OK;
+    KB_REQUIRE(h_img && h_var && h_lh && h_flux && h_vel_idx && h_n_obs && p && d_arena, KBMOD_ERR_INVALID_ARG, "NULL argument");
+    int rc = check_stack(T, H, W);
+    if (rc) return rc;
+    KB_REQUIRE(p->K >= 1 && p->K <= KBMOD_MAX_K, KBMOD_ERR_INVALID_ARG, "K = %d", p->K);
+    KB_REQUIRE(((uintptr_t)d_arena & 255) == 0, KBMOD_ERR_INVALID_ARG, "arena must be 256-byte aligned");
+    ArenaPlan a;
+    plan_arena(T, H, W, n_vel, p, &a);
+    const int n_buf = n_stacks > 1 ? 2 : 1;
+    KB_REQUIRE(arena_bytes >= (size_t)n_buf * a.total, KBMOD_ERR_WORKSPACE,
+               "arena of %zu bytes is smaller than the %d x %zu needed", arena_bytes, n_buf, a.total);
+    for (int i = 0; i < n_stacks; ++i)
+        KB_REQUIRE(h_img[i] && h_var[i] && h_lh[i] && h_flux[i] && h_vel_idx[i] && h_n_obs[i], KBMOD_ERR_INVALID_ARG,
+                   "NULL buffer of stack %d", i);
+    if (!g_bs.ready) {
+        KB_CUDA(cudaStreamCreateWithFlags(&g_bs.s_in, cudaStreamNonBlocking));
+        KB_CUDA(cudaStreamCreateWithFlags(&g_bs.s_out, cudaStreamNonBlocking));
+        for (int b = 0; b < 2; ++b) {
+            KB_CUDA(cudaEventCreateWithFlags(&g_bs.in_done[b], cudaEventDisableTiming));
+            KB_CUDA(cudaEventCreateWithFlags(&g_bs.comp_done[b], cudaEventDisableTiming));
+            KB_CUDA(cudaEventCreateWithFlags(&g_bs.out_done[b], cudaEventDisableTiming));
+        }
+        g_bs.ready = true;
+    }
+    cudaStream_t st = (cudaStream_t)stream;
+    const size_t px = (size_t)T * H * W, res = (size_t)H * W * p->K;
+    // everything enqueued on `stream` before this call happens-before the first copy
+    KB_CUDA(cudaEventRecord(g_bs.comp_done[1], st));
+    KB_CUDA(cudaStreamWaitEvent(g_bs.s_in, g_bs.comp_done[1], 0));
+    for (int i = 0; i < n_stacks; ++i) {
+        const int b = i & 1;
+        char* A = (char*)d_arena + (size_t)b * a.total;
+        const uint8_t* hm = h_mask ? h_mask[i] : nullptr;
+        // inputs of buffer b are free once the search of stack i - 2 is done
+        if (i >= 2) KB_CUDA(cudaStreamWaitEvent(g_bs.s_in, g_bs.comp_done[b], 0));
+        KB_CUDA(cudaMemcpyAsync(A + a.off_img, h_img[i], px * 4, cudaMemcpyHostToDevice, g_bs.s_in));
+        KB_CUDA(cudaMemcpyAsync(A + a.off_var, h_var[i], px * 4, cudaMemcpyHostToDevice, g_bs.s_in));
+        if (hm) KB_CUDA(cudaMemcpyAsync(A + a.off_mask, hm, px, cudaMemcpyHostToDevice, g_bs.s_in));
+        KB_CUDA(cudaEventRecord(g_bs.in_done[b], g_bs.s_in));
+        // the search waits for its inputs and for the results of stack i - 2 to have left buffer b
+        KB_CUDA(cudaStreamWaitEvent(st, g_bs.in_done[b], 0));
+        if (i >= 2) KB_CUDA(cudaStreamWaitEvent(st, g_bs.out_done[b], 0));
+        rc = kbmod_prepare_psi_phi((const float*)(A + a.off_img), (const float*)(A + a.off_var),
+                                   hm ? (const uint8_t*)(A + a.off_mask) : nullptr, T, H, W, h_psf, n_psf, k,
+                                   (float*)(A + a.off_psiphi), stream);
+        if (rc) return rc;
+        rc = kbmod_search((const float*)(A + a.off_psiphi), T, H, W, h_times, h_vx, h_vy, n_vel, p, (float*)(A + a.off_lh),
+                          (float*)(A + a.off_flux), (int32_t*)(A + a.off_vel), (int32_t*)(A + a.off_nobs), A + a.off_ws,
+                          a.ws_bytes, stream);
+        if (rc) return rc;
+        KB_CUDA(cudaEventRecord(g_bs.comp_done[b], st));
+        KB_CUDA(cudaStreamWaitEvent(g_bs.s_out, g_bs.comp_done[b], 0));
+        KB_CUDA(cudaMemcpyAsync(h_lh[i], A + a.off_lh, res * 4, cudaMemcpyDeviceToHost, g_bs.s_out));
+        KB_CUDA(cudaMemcpyAsync(h_flux[i], A + a.off_flux, res * 4, cudaMemcpyDeviceToHost, g_bs.s_out));
+        KB_CUDA(cudaMemcpyAsync(h_vel_idx[i], A + a.off_vel, res * 4, cudaMemcpyDeviceToHost, g_bs.s_out));
+        KB_CUDA(cudaMemcpyAsync(h_n_obs[i], A + a.off_nobs, res * 4, cudaMemcpyDeviceToHost, g_bs.s_out));
+        KB_CUDA(cudaEventRecord(g_bs.out_done[b], g_bs.s_out));
+    }
+    // the caller's stream finishes after the last result has landed
+    KB_CUDA(cudaStreamWaitEvent(st, g_bs.out_done[(n_stacks - 1) & 1], 0));
+    if (n_stacks > 1) KB_CUDA(cudaStreamWaitEvent(st, g_bs.out_done[(n_stacks - 2) & 1], 0));
+    KB_CUDA(cudaStreamSynchronize(st));
+    return KBMOD_OK;
+}

@@ -601,3 +601,35 @@ def test_measured_smem_peak_is_plausible(kb):
     for width in (4, 8, 16):
         gbs = kb.kbmod_measure_smem_gbs(width)
         assert 0.6 * theo < gbs < 1.1 * theo, (width, gbs, theo)
+
+
+def test_pipeline_host_batch_equals_single_calls(kb):
+    """Five stacks of one shape through kbmod_pipeline_host_batch (copies overlapped with the searches, two arena
+    halves reused) must give exactly what five kbmod_pipeline_host calls give."""
+    import torch
+    T, H, W, K = 8, 96, 130, 4
+    rng = np.random.default_rng(500)
+    vx = rng.uniform(-20, 20, 50).astype(np.float32)
+    vy = rng.uniform(-20, 20, 50).astype(np.float32)
+    sts = [synth.random_stack(500 + i, T, H, W, mask_frac=0.05, t_span=1.5) for i in range(5)]
+    for s_ in sts:
+        s_.img[rng.random(s_.img.shape) < 0.02] *= 20.0
+        s_.times = sts[0].times
+    sp = kb.SearchParams(K=K, min_obs=3, min_lh=4.0)
+    pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
+    stacks = [(pin(s_.img), pin(s_.var), pin(s_.mask)) for s_ in sts]
+    mk_out = lambda: tuple(torch.empty((H, W, K), dtype=dt).pin_memory() for dt in (torch.float32, torch.float32, torch.int32, torch.int32))
+    per = kb.kbmod_pipeline_host_arena_bytes(T, H, W, len(vx), sp)
+    arena = torch.empty(2 * per, dtype=torch.uint8, device="cuda")
+    singles = []
+    for stk in stacks:
+        o = mk_out()
+        kb.kbmod_pipeline_host(*stk, sts[0].psf, sts[0].times, vx, vy, sp, o, arena)
+        singles.append([t.clone() for t in o])
+    outs = [mk_out() for _ in stacks]
+    kb.kbmod_pipeline_host_batch(stacks, sts[0].psf, sts[0].times, vx, vy, sp, outs, arena)
+    for a, b in zip(singles, outs):
+        for x, y in zip(a, b):
+            assert torch.equal(x, y)
+    assert any(int((o[2] >= 0).sum()) > 0 for o in outs)
+    assert not torch.equal(outs[0][2], outs[1][2])  # different stacks, different results
