@@ -279,6 +279,15 @@ def run_ours(args):
                 n_cand=n_cand, out=out, smem_gbs=smem_gbs)
 
 
+def in_bounds_fraction(times, vx, vy, H, W) -> float:
+    """Share of the nominal trajectory-epoch evaluations whose position is on the image (reported beside
+    the nominal count).  Positions follow reading R5: start + floor(v dt + 1/2)."""
+    dt = np.asarray(times, np.float64) - float(times[0])
+    dx = np.floor(np.asarray(vx, np.float64)[:, None] * dt[None, :] + 0.5)
+    dy = np.floor(np.asarray(vy, np.float64)[:, None] * dt[None, :] + 0.5)
+    return float((np.clip(W - np.abs(dx), 0, None) * np.clip(H - np.abs(dy), 0, None)).mean() / (float(W) * H))
+
+
 def max_over_ranks(ms_local: float, dist, device, world: int) -> float:
     """Device time of the timed region: the MAX over ranks (every rank gets it)."""
     import torch
@@ -380,6 +389,7 @@ def report(R, args):
                             host_plan="velocity grouping / staging geometry cached after the first (warm-up) step: same grid and times"),
                 segments_ms={k: float(np.mean(v)) for k, v in R["seg"].items()},
                 evaluated_fraction=evaluated / max(1, nominal),
+                in_bounds_fraction=in_bounds_fraction(st.times, R["vx"], R["vy"], H, W),
                 roofline=roof, cpu_baseline=cpu,
                 e2e=dict(value=whole_job_value(R["evals"], world, e2e_max), unit=UNIT, h2d_bytes_per_step=h2d,
                          d2h_bytes_per_step=d2h, ms_per_step=e2e_max, steps=e2e_steps,
