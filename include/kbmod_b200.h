@@ -129,6 +129,13 @@ int kbmod_search(const float* d_psiphi, int T, int H, int W, const double* h_tim
                  const float* h_vy, int n_vel, const kbmod_search_params* p, float* d_lh, float* d_flux,
                  int32_t* d_vel_idx, int32_t* d_n_obs, void* d_workspace, size_t workspace_bytes, void* stream);
 
+/* Host-only view of the pruned kernel's plan for a geometry (no GPU needed; what `-m "not gpu"` tests check):
+ * h_out[0] = 1 if the velocity list is too scattered for the pruned kernel (AUTO then runs the direct one), h_out[1] =
+ * bytes staged into shared memory per trajectory-epoch evaluation, h_out[2] = number of velocity groups, h_out[3] =
+ * share of the (tile, group, epoch) region loads that lie off the image and are skipped. */
+int kbmod_plan_stats(int T, int H, int W, const double* h_times, const float* h_vx, const float* h_vy, int n_vel,
+                     const kbmod_search_params* p, double* h_out);
+
 /* Counters of the last kbmod_search on this thread (read after synchronising the stream).
  * h_out[0] = trajectories fully evaluated (sigma-G run), h_out[1] = trajectories nominally
  * searched (H*W*n_vel), h_out[2] = kernels launched by the call, h_out[3] = algo actually used. */

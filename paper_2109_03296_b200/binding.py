@@ -17,7 +17,7 @@ ALGO_AUTO, ALGO_DIRECT, ALGO_PRUNED = 0, 1, 2
 MAX_T, MAX_K, MAX_PSF, MAX_STAMP_RADIUS = 64, 32, 31, 15
 
 EXPORTS = ["kbmod_default_params", "kbmod_prepare_psi_phi", "kbmod_displacements",
-           "kbmod_search_workspace_bytes", "kbmod_search", "kbmod_search_stats", "kbmod_search_phase_timing",
+           "kbmod_search_workspace_bytes", "kbmod_search", "kbmod_plan_stats", "kbmod_search_stats", "kbmod_search_phase_timing",
            "kbmod_search_phase_ms", "kbmod_coadd_stamps",
            "kbmod_eval_trajectories", "kbmod_sigmag_filter", "kbmod_stamp_moments", "kbmod_pipeline_host_arena_bytes",
            "kbmod_pipeline_host", "kbmod_pipeline_host_batch", "kbmod_measure_smem_gbs", "kbmod_last_error", "kbmod_version"]
@@ -174,6 +174,18 @@ def kbmod_search(psiphi, times, vx, vy, params: SearchParams, out=None, workspac
                               C.c_size_t(workspace.numel()), _stream(stream)))
     kbmod_search.last_workspace = workspace
     return out
+
+
+def kbmod_plan_stats(T, H, W, times, vx, vy, params: SearchParams):
+    """Host-only: dict(too_scattered, staged_bytes_per_eval, n_groups, off_image_fraction) of the pruned kernel's plan."""
+    t, tp = _host(times, np.float64)
+    x, xp = _host(vx, np.float32)
+    y, yp = _host(vy, np.float32)
+    cp = params.c()
+    out = (C.c_double * 4)()
+    _check(lib().kbmod_plan_stats(T, H, W, tp, xp, yp, len(x), C.byref(cp), out))
+    return dict(too_scattered=bool(out[0]), staged_bytes_per_eval=float(out[1]), n_groups=int(out[2]),
+                off_image_fraction=float(out[3]))
 
 
 def kbmod_search_stats(workspace):

@@ -255,7 +255,7 @@ extern "C" int kbmod_search(const float* d_psiphi, int T, int H, int W, const do
     // groups can be staged
     int algo = p->algo;
     if (algo != KBMOD_ALGO_DIRECT && n_vel > 0) {
-        double ps[2] = {0, 0};
+        double ps[4] = {0, 0, 0, 0};
         rc = kb_launch_search_pruned(nullptr, T, TP, H, W, nullptr, hdx.data(), hdy.data(), n_vel, p, P, nullptr, nullptr,
                                      nullptr, nullptr, nullptr, 0, nullptr, st, /*plan_only=*/1, ps, nullptr);
         if (algo == KBMOD_ALGO_AUTO) {
@@ -288,6 +288,27 @@ extern "C" int kbmod_search(const float* d_psiphi, int T, int H, int W, const do
     if (rc) return rc;
     const unsigned long long nl = (unsigned long long)launches;  // kernels this call enqueued
     KB_CUDA(cudaMemcpyAsync(ws + pl.off_stats + 2 * sizeof(unsigned long long), &nl, sizeof(nl), cudaMemcpyHostToDevice, st));
+    return KBMOD_OK;
+}
+
+// host-only view of the pruned search's plan (no GPU needed): what the planner would stage for this geometry
+extern "C" int kbmod_plan_stats(int T, int H, int W, const double* h_times, const float* h_vx, const float* h_vy, int n_vel,
+                                const kbmod_search_params* p, double* h_out) {
+    KB_REQUIRE(h_times && h_out && p && (n_vel == 0 || (h_vx && h_vy)), KBMOD_ERR_INVALID_ARG, "NULL argument");
+    KB_REQUIRE(n_vel >= 0, KBMOD_ERR_INVALID_ARG, "n_vel = %d", n_vel);
+    int rc = check_stack(T, H, W);
+    if (rc) return rc;
+    DevParams P;
+    rc = kb_make_dev_params(p, T, &P);
+    if (rc) return rc;
+    std::vector<int32_t> hdx((size_t)n_vel * T), hdy((size_t)n_vel * T);
+    rc = kbmod_displacements(h_times, T, h_vx, h_vy, n_vel, hdx.data(), hdy.data());
+    if (rc) return rc;
+    double ps[4] = {0, 0, 0, 0};
+    rc = kb_launch_search_pruned(nullptr, T, kb_padded_T(T), H, W, nullptr, hdx.data(), hdy.data(), n_vel, p, P, nullptr,
+                                 nullptr, nullptr, nullptr, nullptr, 0, nullptr, nullptr, /*plan_only=*/1, ps, nullptr);
+    if (rc) return rc;
+    for (int i = 0; i < 4; ++i) h_out[i] = ps[i];
     return KBMOD_OK;
 }
 

@@ -1051,7 +1051,17 @@ int kb_launch_search_pruned(const float* d_psiphi, int T, int TPv, int H, int W,
 
     if (plan_stats) {
         plan_stats[0] = (size_t)ng > ngm ? 1.0 : 0.0;       // the velocity list is too scattered to group
-        plan_stats[1] = evals > 0 ? staged / evals : 0.0;   // staged bytes per evaluation
+        plan_stats[1] = evals > 0 ? staged / evals : 0.0;   // staged bytes per evaluation (before off-image skipping)
+        plan_stats[2] = (double)ng;                         // velocity groups
+        // share of the (tile, group, epoch) region loads that lie off the image and are skipped
+        double on = 0.0, all = 0.0;
+        for (int g = 0; g < ng; ++g)
+            for (int c = 0; c < tiles_x; ++c)
+                for (int r = 0; r < tiles_y; ++r) {
+                    on += (double)__builtin_popcountll(maskx[(size_t)g * tiles_x + c] & masky[(size_t)g * tiles_y + r]);
+                    all += (double)T;
+                }
+        plan_stats[3] = all > 0 ? 1.0 - on / all : 0.0;
     }
     if (plan_only) return KBMOD_OK;
     KB_REQUIRE((size_t)ng <= ngm, KBMOD_ERR_UNSUPPORTED,

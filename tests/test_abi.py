@@ -89,3 +89,27 @@ def test_binding_refuses_cpu_tensors(lib):
     import torch
     with pytest.raises(TypeError):
         binding.kbmod_prepare_psi_phi(torch.zeros(1, 4, 4), torch.ones(1, 4, 4), None, np.ones((1, 1), np.float32))
+
+
+def test_planner_host_logic_without_gpu(lib):
+    """The pruned kernel's host planner (k-d velocity grouping, staging geometry, on-image masks) runs without a GPU
+    through kbmod_plan_stats: the numbers DESIGN.md quotes for the benchmark configurations."""
+    import math
+    import paper_2109_03296_b200 as kb
+    from paper_2109_03296_b200 import synth
+    sp = kb.SearchParams()
+    c3 = kb.kbmod_plan_stats(26, 4096, 2048, synth.night_times((7, 6, 7, 6)), *synth.config3_grid(), sp)
+    assert not c3["too_scattered"] and c3["n_groups"] == 512
+    assert 0.5 < c3["staged_bytes_per_eval"] < 0.65 and 0.10 < c3["off_image_fraction"] < 0.18
+    c4 = kb.kbmod_plan_stats(50, 4096, 2048, synth.night_times((9, 8, 8, 9, 8, 8)), *synth.config4_grid(), sp)
+    assert c4["n_groups"] == 2048 and 0.2 < c4["off_image_fraction"] < 0.3
+    c1 = kb.kbmod_plan_stats(5, 64, 64, synth.config1_tiny().times, *synth.config1_grid(), sp)
+    assert c1["n_groups"] == 16 and c1["off_image_fraction"] == 0.0  # 40 px/day x 2 d stays inside one 64x64 tile's regions
+    # velocities all over the sky at a long baseline: groups are bisected until every staged region fits the ring
+    rng = np.random.default_rng(0)
+    vx, vy = rng.uniform(-3000, 3000, 200).astype(np.float32), rng.uniform(-3000, 3000, 200).astype(np.float32)
+    sc = kb.kbmod_plan_stats(10, 512, 512, np.linspace(0, 5, 10), vx, vy, sp)
+    assert sc["n_groups"] > math.ceil(200 / 16) and sc["off_image_fraction"] > 0.5
+    # bad arguments are refused on the host
+    with pytest.raises(kb.KbmodError):
+        kb.kbmod_plan_stats(65, 64, 64, np.zeros(65), vx, vy, sp)
