@@ -25,6 +25,8 @@
  *
  * Pins (tests/test_oracle_*.py): closed-form point source, all-zero psi, numpy brute force on
  * tiny stacks, sorted() percentiles, erf^-1 closed form of the 0.7413 coefficient, invariants.
+ * Interpolated percentiles (R23) are pinned against numpy.percentile(method="linear"); the unfiltered sum-LH
+ * against the sigma-G-off evaluation; the post-filter's reject flag against the paper's threshold (L123).
  * Unpinned against the original KBMOD code (not available): readings R3 (masked taps), R10
  * (nearest-rank percentiles) and R22 (moment normalisation) -- "parity unpinned" with respect to that
  * code; see DESIGN.md.
@@ -127,6 +129,7 @@ typedef struct {
     int filter_on; /* 0: flux psi/phi, 1: likelihood psi/sqrt(phi)  (L123 "likelihood and/or flux") */
     float min_lh;
     int min_obs, K;
+    int pct_interp; /* 0: nearest-rank order statistics (R10); 1: linear interpolation between them (R23) */
 } oparams;
 
 /* nearest-rank percentile index: ceil(q n / 100) - 1, clamped to [0, n-1]  (R10) */
@@ -138,6 +141,27 @@ static int pct_rank(float q, int n) {
 }
 
 int oracle_pct_rank(float q, int n) { return pct_rank(q, n); }
+
+/* The q-th percentile of the ascending array s[0..m).  PAPER.md L117: "selecting the 25th and 75th percentile
+ * values ... from the data".  interp = 0 (reading R10, the default): the nearest-rank order statistic.
+ * interp = 1 (reading R23, the alternative SURVEY 8c-R10 names): linear interpolation between the two order
+ * statistics that bracket the fractional position h = (m - 1) q / 100,
+ *     v = s[k] + g (s[k+1] - s[k]),   k = floor(h),  g = h - k,
+ * h and g in double, g rounded to single, then the three single-precision operations separately rounded
+ * (the decision precision).  This is numpy.percentile(method="linear") up to single-precision rounding. */
+static float pct_value(const float *s, int m, float q, int interp) {
+    if (!interp) return s[pct_rank(q, m)];
+    double h = (double)(m - 1) * (double)q / 100.0;
+    if (h <= 0.0) return s[0];
+    if (h >= (double)(m - 1)) return s[m - 1];
+    int k = (int)floor(h);
+    float g = (float)(h - (double)k);
+    float d = s[k + 1] - s[k];
+    float e = g * d;
+    return s[k] + e;
+}
+
+float oracle_pct_value(const float *s, int m, float q, int interp) { return pct_value(s, m, q, interp); }
 
 /* psi_t, phi_t: the T gathered samples; valid: bit t set iff epoch t contributes.
  * Returns n_kept (0 = "no result": fewer than max(1, min_obs) valid epochs). */
@@ -165,9 +189,9 @@ static int filter_and_score(const float *psi_t, const float *phi_t, int T, uint6
             while (j >= 0 && s[j] > key) { s[j + 1] = s[j]; --j; }
             s[j + 1] = key;
         }
-        float p_lo = s[pct_rank(p->pct_lo, m)];
-        float p_50 = s[pct_rank(50.0f, m)];
-        float p_hi = s[pct_rank(p->pct_hi, m)];
+        float p_lo = pct_value(s, m, p->pct_lo, p->pct_interp);
+        float p_50 = pct_value(s, m, 50.0f, p->pct_interp);
+        float p_hi = pct_value(s, m, p->pct_hi, p->pct_interp);
         float d = p_hi - p_lo;       /* Eq. 5: sigma_G = C (x_j - x_i) */
         float sg = p->coeff * d;
         float w = p->n_sigma * sg;   /* L117: +- n sigma_G about the median */
@@ -213,9 +237,9 @@ static uint64_t gather(const float *psiphi, int T, int H, int W, int x0, int y0,
 void oracle_search_pixels(const float *psiphi, int T, int H, int W, const double *times, const float *vx,
                           const float *vy, int n_vel, const int32_t *px, const int32_t *py, int n_pix,
                           int sigmag_enable, float pct_lo, float pct_hi, float coeff, float n_sigma,
-                          int filter_on, float min_lh, int min_obs, int K, double *lh, double *flux,
+                          int filter_on, float min_lh, int min_obs, int K, int pct_interp, double *lh, double *flux,
                           int32_t *vel_idx, int32_t *n_obs) {
-    oparams p = {sigmag_enable, pct_lo, pct_hi, coeff, n_sigma, filter_on, min_lh, min_obs, K};
+    oparams p = {sigmag_enable, pct_lo, pct_hi, coeff, n_sigma, filter_on, min_lh, min_obs, K, pct_interp};
     int32_t *dx = (int32_t *)malloc(sizeof(int32_t) * (size_t)n_vel * T);
     int32_t *dy = (int32_t *)malloc(sizeof(int32_t) * (size_t)n_vel * T);
     oracle_displacements(times, T, vx, vy, n_vel, dx, dy);
@@ -248,9 +272,9 @@ void oracle_search_pixels(const float *psiphi, int T, int H, int W, const double
 void oracle_eval_trajectories(const float *psiphi, int T, int H, int W, const double *times, const int32_t *x0,
                               const int32_t *y0, const float *vx, const float *vy, int n_traj,
                               int sigmag_enable, float pct_lo, float pct_hi, float coeff, float n_sigma,
-                              int filter_on, int min_obs, float *psi_lc, float *phi_lc, uint64_t *valid_out,
-                              uint64_t *kept_out, double *lh, double *flux, int32_t *n_kept) {
-    oparams p = {sigmag_enable, pct_lo, pct_hi, coeff, n_sigma, filter_on, -INFINITY, min_obs, 1};
+                              int filter_on, int min_obs, int pct_interp, float *psi_lc, float *phi_lc,
+                              uint64_t *valid_out, uint64_t *kept_out, double *lh, double *flux, int32_t *n_kept) {
+    oparams p = {sigmag_enable, pct_lo, pct_hi, coeff, n_sigma, filter_on, -INFINITY, min_obs, 1, pct_interp};
 #pragma omp parallel for schedule(dynamic, 64)
     for (int i = 0; i < n_traj; ++i) {
         int32_t dx[ORACLE_MAX_T], dy[ORACLE_MAX_T];
@@ -262,11 +286,15 @@ void oracle_eval_trajectories(const float *psiphi, int T, int H, int W, const do
     }
 }
 
-/* sigma-G on given lightcurves [n_lc][T] (config 5's "rerun sigma-G"); valid iff phi > 0. */
+/* sigma-G on given lightcurves [n_lc][T] (config 5's "rerun sigma-G"); valid iff phi > 0.
+ * The paper's post-filter: "reject the trajectory if the recomputed likelihood (sum LH') is
+ * less than 10": pass[i] = 1 iff the lightcurve has a result (n_valid >= max(1, min_obs)) and L' >= min_lh
+ * (reading R14: the comparison is >=; min_lh = -inf keeps every lightcurve that has a result). */
 void oracle_sigmag_filter(const float *psi_lc, const float *phi_lc, int n_lc, int T, int sigmag_enable,
                           float pct_lo, float pct_hi, float coeff, float n_sigma, int filter_on, int min_obs,
-                          uint64_t *kept_out, double *lh, double *flux, int32_t *n_kept) {
-    oparams p = {sigmag_enable, pct_lo, pct_hi, coeff, n_sigma, filter_on, -INFINITY, min_obs, 1};
+                          int pct_interp, float min_lh, uint64_t *kept_out, double *lh, double *flux,
+                          int32_t *n_kept, uint8_t *pass) {
+    oparams p = {sigmag_enable, pct_lo, pct_hi, coeff, n_sigma, filter_on, -INFINITY, min_obs, 1, pct_interp};
 #pragma omp parallel for schedule(static)
     for (int i = 0; i < n_lc; ++i) {
         const float *ps = psi_lc + (size_t)i * T, *ph = phi_lc + (size_t)i * T;
@@ -274,7 +302,34 @@ void oracle_sigmag_filter(const float *psi_lc, const float *phi_lc, int n_lc, in
         for (int t = 0; t < T; ++t)
             if (ph[t] > 0.0f) valid |= (uint64_t)1 << t;
         n_kept[i] = filter_and_score(ps, ph, T, valid, &p, &kept_out[i], &lh[i], &flux[i]);
+        if (pass) pass[i] = (n_kept[i] > 0 && lh[i] >= (double)min_lh) ? 1 : 0;
     }
+}
+
+/* ------------------------------------------------------------------ unfiltered sum-LH beside sum-LH' (L175, L181) */
+/* PAPER.md L175 (section 4.1): the single-trajectory variant "computes the likelihoods along a single trajectory
+ * then runs the ... filtering"; L181 quotes the unfiltered sum-LH next to the filtered sum-LH' of recovered objects.
+ * For every result slot (pixel i, slot k) with vel_idx >= 0: L = sum_valid psi / sqrt(sum_valid phi) over ALL
+ * valid epochs of that trajectory (no sigma-G clip, no threshold), double precision; empty slots get -inf. */
+void oracle_unfiltered_lh(const float *psiphi, int T, int H, int W, const double *times, const float *vx,
+                          const float *vy, int n_vel, const int32_t *px, const int32_t *py, int n_pix, int K,
+                          const int32_t *vel_idx, double *lh_raw) {
+#pragma omp parallel for schedule(dynamic, 64)
+    for (int i = 0; i < n_pix; ++i)
+        for (int k = 0; k < K; ++k) {
+            int v = vel_idx[(size_t)i * K + k];
+            double *out = lh_raw + (size_t)i * K + k;
+            *out = -INFINITY;
+            if (v < 0 || v >= n_vel) continue;
+            int32_t dx[ORACLE_MAX_T], dy[ORACLE_MAX_T];
+            float psi_t[ORACLE_MAX_T], phi_t[ORACLE_MAX_T];
+            oracle_displacements(times, T, vx + v, vy + v, 1, dx, dy);
+            uint64_t valid = gather(psiphi, T, H, W, px[i], py[i], dx, dy, psi_t, phi_t);
+            double sp = 0.0, sf = 0.0;
+            for (int t = 0; t < T; ++t)
+                if ((valid >> t) & 1u) { sp += (double)psi_t[t]; sf += (double)phi_t[t]; }
+            if (valid) *out = sp / sqrt(sf);
+        }
 }
 
 /* ------------------------------------------------------------------ O7: coadded stamps (L141; R17) */

@@ -35,6 +35,8 @@ def lib():
         _lib.oracle_num_threads.restype = C.c_int
         _lib.oracle_pct_rank.restype = C.c_int
         _lib.oracle_pct_rank.argtypes = [C.c_float, C.c_int]
+        _lib.oracle_pct_value.restype = C.c_float
+        _lib.oracle_pct_value.argtypes = [C.POINTER(C.c_float), C.c_int, C.c_float, C.c_int]
     return _lib
 
 
@@ -51,6 +53,7 @@ class Params:
     min_lh: float = -np.inf
     min_obs: int = 1
     K: int = 8
+    pct_interp: int = 0  # 0 nearest-rank order statistics (R10), 1 linear interpolation (R23)
 
 
 def _p(a, ct):
@@ -67,6 +70,12 @@ def num_threads() -> int:
 
 def pct_rank(q: float, n: int) -> int:
     return int(lib().oracle_pct_rank(C.c_float(q), n))
+
+
+def pct_value(sorted_values, q: float, interp: int) -> float:
+    """The q-th percentile of an ascending float32 array: nearest rank (interp=0, R10) or linear (interp=1, R23)."""
+    s = np.ascontiguousarray(sorted_values, dtype=np.float32)
+    return float(lib().oracle_pct_value(_p(s, C.c_float), len(s), C.c_float(q), interp))
 
 
 def prepare_psi_phi(img, var, mask, psf):
@@ -112,7 +121,7 @@ def search_pixels(psiphi, times, vx, vy, px, py, p: Params):
     lib().oracle_search_pixels(_p(psiphi, C.c_float), T, H, W, _p(times, C.c_double), _p(vx, C.c_float),
                                _p(vy, C.c_float), len(vx), _p(px, C.c_int32), _p(py, C.c_int32), n,
                                p.sigmag_enable, C.c_float(p.pct_lo), C.c_float(p.pct_hi), C.c_float(p.coeff),
-                               C.c_float(p.n_sigma), p.filter_on, C.c_float(p.min_lh), p.min_obs, p.K,
+                               C.c_float(p.n_sigma), p.filter_on, C.c_float(p.min_lh), p.min_obs, p.K, p.pct_interp,
                                _p(lh, C.c_double), _p(flux, C.c_double), _p(vel, C.c_int32), _p(nobs, C.c_int32))
     return lh, flux, vel, nobs
 
@@ -138,21 +147,37 @@ def eval_trajectories(psiphi, times, x0, y0, vx, vy, p: Params):
     lib().oracle_eval_trajectories(_p(psiphi, C.c_float), T, H, W, _p(times, C.c_double), _p(x0, C.c_int32),
                                    _p(y0, C.c_int32), _p(vx, C.c_float), _p(vy, C.c_float), n, p.sigmag_enable,
                                    C.c_float(p.pct_lo), C.c_float(p.pct_hi), C.c_float(p.coeff),
-                                   C.c_float(p.n_sigma), p.filter_on, p.min_obs, _p(psi_lc, C.c_float),
+                                   C.c_float(p.n_sigma), p.filter_on, p.min_obs, p.pct_interp, _p(psi_lc, C.c_float),
                                    _p(phi_lc, C.c_float), _p(valid, C.c_uint64), _p(kept, C.c_uint64),
                                    _p(lh, C.c_double), _p(flux, C.c_double), _p(nk, C.c_int32))
     return dict(psi_lc=psi_lc, phi_lc=phi_lc, valid=valid, kept=kept, lh=lh, flux=flux, n_kept=nk)
 
 
 def sigmag_filter(psi_lc, phi_lc, p: Params):
+    """The post-filter on given lightcurves. `passed` = has a result and L' >= p.min_lh."""
     psi_lc, phi_lc = _c(psi_lc, np.float32), _c(phi_lc, np.float32)
     n, T = psi_lc.shape
     kept, lh, flux, nk = np.empty(n, np.uint64), np.empty(n), np.empty(n), np.empty(n, np.int32)
+    passed = np.empty(n, np.uint8)
     lib().oracle_sigmag_filter(_p(psi_lc, C.c_float), _p(phi_lc, C.c_float), n, T, p.sigmag_enable,
                                C.c_float(p.pct_lo), C.c_float(p.pct_hi), C.c_float(p.coeff), C.c_float(p.n_sigma),
-                               p.filter_on, p.min_obs, _p(kept, C.c_uint64), _p(lh, C.c_double),
-                               _p(flux, C.c_double), _p(nk, C.c_int32))
-    return dict(kept=kept, lh=lh, flux=flux, n_kept=nk)
+                               p.filter_on, p.min_obs, p.pct_interp, C.c_float(p.min_lh), _p(kept, C.c_uint64),
+                               _p(lh, C.c_double), _p(flux, C.c_double), _p(nk, C.c_int32), _p(passed, C.c_uint8))
+    return dict(kept=kept, lh=lh, flux=flux, n_kept=nk, passed=passed)
+
+
+def unfiltered_lh(psiphi, times, vx, vy, px, py, vel_idx):
+    """Unfiltered sum-LH of every result slot: vel_idx int32 [n][K] -> float64 [n][K]."""
+    psiphi = _c(psiphi, np.float32)
+    T, H, W, _ = psiphi.shape
+    times, vx, vy = _c(times, np.float64), _c(vx, np.float32), _c(vy, np.float32)
+    px, py, vel_idx = _c(px, np.int32), _c(py, np.int32), _c(vel_idx, np.int32)
+    n, K = vel_idx.shape
+    out = np.empty((n, K))
+    lib().oracle_unfiltered_lh(_p(psiphi, C.c_float), T, H, W, _p(times, C.c_double), _p(vx, C.c_float),
+                               _p(vy, C.c_float), len(vx), _p(px, C.c_int32), _p(py, C.c_int32), n, K,
+                               _p(vel_idx, C.c_int32), _p(out, C.c_double))
+    return out
 
 
 def coadd_stamps(img, mask, times, x0, y0, vx, vy, radius: int, epoch_mask=None):

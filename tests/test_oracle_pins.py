@@ -551,3 +551,148 @@ def test_moments_equal_numpy_restatement_and_strict_thresholds():
     # non-finite pixels: the stamp fails
     bad = _gauss_stamp(r, 1.4).copy(); bad[3, 4] = np.nan
     assert O.stamp_moments(bad[None])[1][0] == 0
+
+
+# ------------------------------------------------------------------ N4: interpolated percentiles (reading R23)
+def test_interpolated_percentiles_match_numpy_linear():
+    """R23: pct_interp = 1 is numpy.percentile(method="linear") up to float32 rounding (PAPER.md L117 leaves the
+    percentile definition open; SURVEY 8c-R10 names linear interpolation as the alternative)."""
+    rng = np.random.default_rng(11)
+    for n in list(range(1, 30)) + [50, 64]:
+        s = np.sort(rng.standard_normal(n).astype(np.float32) * 5)
+        for q in (25.0, 50.0, 75.0, 10.0, 90.0, 0.0, 100.0, 33.3):
+            ref = np.percentile(s.astype(np.float64), q, method="linear")
+            got = O.pct_value(s, q, 1)
+            assert abs(got - ref) <= 4e-7 * max(1.0, np.abs(s).max()), (n, q, got, ref)
+            assert O.pct_value(s, q, 0) == s[O.pct_rank(q, n)]  # interp = 0 is the nearest-rank order statistic
+    # exact cases: small integers, dyadic weights -- no rounding anywhere, so equality is exact
+    s = np.array([1, 2, 4, 8, 16], np.float32)
+    assert [O.pct_value(s, q, 1) for q in (25, 50, 75)] == [2.0, 4.0, 8.0]          # h = 1, 2, 3: order statistics
+    s = np.array([0, 4, 12], np.float32)
+    assert [O.pct_value(s, q, 1) for q in (25, 50, 75)] == [2.0, 4.0, 8.0]          # h = .5, 1, 1.5
+    assert O.pct_value(np.array([3, 7], np.float32), 50, 1) == 5.0                   # even n: mean of the two middles
+
+
+def test_interpolated_filter_matches_numpy_chain():
+    """The kept set with pct_interp = 1 is {|f - P50| <= 2 * 0.7413 * (P75 - P25)} with numpy's linear percentiles;
+    epochs within float32 rounding of a clip bound are exempt (they are decided in float32, R20)."""
+    rng = np.random.default_rng(12)
+    n_lc, compared, total = 4000, 0, 0
+    for T in (3, 4, 7, 10, 26, 50):
+        phi = rng.uniform(0.5, 2.0, (n_lc, T)).astype(np.float32)
+        psi = (rng.standard_normal((n_lc, T)) * np.sqrt(phi)).astype(np.float32)
+        psi[rng.random((n_lc, T)) < 0.1] *= 8.0
+        phi[rng.random((n_lc, T)) < 0.08] = 0.0
+        r = O.sigmag_filter(psi, phi, P(pct_interp=1))
+        for i in range(0, n_lc, 7):
+            v = phi[i] > 0
+            if v.sum() == 0:
+                continue
+            f = psi[i, v].astype(np.float64) / phi[i, v].astype(np.float64)
+            p25, p50, p75 = np.percentile(f, [25, 50, 75], method="linear")
+            w = 2.0 * 0.7413 * (p75 - p25)
+            keep = np.abs(f - p50) <= w
+            near = np.abs(np.abs(f - p50) - w) <= 1e-5 * max(abs(p50), w, 1e-30)
+            got = ((int(r["kept"][i]) >> np.nonzero(v)[0]) & 1).astype(bool)
+            assert np.array_equal(got[~near], keep[~near]), (T, i)
+            compared += int((~near).sum()); total += len(f)
+    assert compared > 0.999 * total
+
+
+def test_interpolation_is_a_no_op_where_positions_are_integers():
+    """n = 5 and n = 9 put h = (n-1) q / 100 on integers for q = 25, 50, 75, which are also the nearest ranks: both
+    percentile definitions must then give the same results."""
+    rng = np.random.default_rng(13)
+    for T in (5, 9):
+        assert [O.pct_rank(q, T) for q in (25, 50, 75)] == [(T - 1) * q // 100 for q in (25, 50, 75)]
+        phi = rng.uniform(0.5, 2.0, (3000, T)).astype(np.float32)
+        psi = (rng.standard_normal((3000, T)) * 3).astype(np.float32)
+        a, b = O.sigmag_filter(psi, phi, P(pct_interp=0)), O.sigmag_filter(psi, phi, P(pct_interp=1))
+        assert np.array_equal(a["kept"], b["kept"]) and np.array_equal(a["lh"], b["lh"])
+    # ... and differs where they are not (n = 26: ranks 6, 12, 19 against h = 6.25, 12.5, 18.75)
+    phi = rng.uniform(0.5, 2.0, (3000, 26)).astype(np.float32)
+    psi = (rng.standard_normal((3000, 26)) * 3).astype(np.float32)
+    a, b = O.sigmag_filter(psi, phi, P(pct_interp=0)), O.sigmag_filter(psi, phi, P(pct_interp=1))
+    assert (a["kept"] != b["kept"]).mean() > 0.05
+
+
+# ------------------------------------------------------------------ N4: unfiltered sum-LH beside sum-LH' (L175, L181)
+def test_unfiltered_lh_equals_sigma_g_off_evaluation():
+    st = synth.random_stack(71, 9, 30, 41, mask_frac=0.1, t_span=2.0)
+    psi, phi, _, _ = O.prepare_psi_phi(st.img, st.var, st.mask, st.psf)
+    pp = O.interleave(psi, phi)
+    rng = np.random.default_rng(3)
+    vx, vy = rng.uniform(-12, 12, 25).astype(np.float32), rng.uniform(-12, 12, 25).astype(np.float32)
+    yy, xx = np.mgrid[0:30, 0:41]
+    px, py = xx.reshape(-1).astype(np.int32), yy.reshape(-1).astype(np.int32)
+    lh, flux, vel, nobs = O.search_pixels(pp, st.times, vx, vy, px, py, P(K=4, min_obs=3))
+    raw = O.unfiltered_lh(pp, st.times, vx, vy, px, py, vel)
+    filled = vel >= 0
+    assert filled.sum() > 1000 and np.all(np.isneginf(raw[~filled]))
+    ii, kk = np.nonzero(filled)
+    ev = O.eval_trajectories(pp, st.times, px[ii], py[ii], vx[vel[ii, kk]], vy[vel[ii, kk]], P(sigmag_enable=0, min_obs=1))
+    assert np.array_equal(raw[ii, kk], ev["lh"])           # = the sigma-G-off evaluation of the same trajectory
+    # ... which is the plain sum of PAPER.md L79 over the valid epochs (numpy, from the lightcurves)
+    sp = ev["psi_lc"].astype(np.float64).sum(1); sf = ev["phi_lc"].astype(np.float64).sum(1)
+    assert np.allclose(raw[ii, kk], sp / np.sqrt(sf), rtol=1e-14)
+    # the filter can only remove epochs: where nothing was clipped the two likelihoods coincide
+    same = nobs[ii, kk] == np.array([bin(int(v)).count("1") for v in ev["valid"]])
+    assert same.any() and np.allclose(raw[ii, kk][same], lh[ii, kk][same], rtol=1e-12)
+
+
+# ------------------------------------------------------------------ N1: the post-filter's decision (L123)
+def test_postfilter_rejects_below_the_papers_threshold():
+    g = golden()
+    rng = np.random.default_rng(17)
+    n, T = 20000, 20
+    phi = rng.uniform(0.5, 2.0, (n, T)).astype(np.float32)
+    psi = ((rng.standard_normal((n, T)) + rng.uniform(0, 4, (n, 1))) * np.sqrt(phi)).astype(np.float32)
+    phi[rng.random((n, T)) < 0.3] = 0.0
+    r = O.sigmag_filter(psi, phi, P(min_lh=g["min_lh"], min_obs=12))
+    has = r["n_kept"] > 0
+    assert has.any() and (~has).any()
+    want = has & (r["lh"] >= g["min_lh"])                     # "reject ... if the recomputed likelihood is less than 10"
+    assert np.array_equal(r["passed"].astype(bool), want) and 0.05 < want.mean() < 0.95
+    assert np.all(O.sigmag_filter(psi, phi, P(min_lh=-np.inf, min_obs=12))["passed"].astype(bool) == has)
+
+
+# ------------------------------------------------------------------ R20: float32 decision chain vs the double chain
+def test_float32_decision_chain_against_double_precision_definition():
+    """Reading R20 takes the keep / drop decision in float32.  Here the same decision is taken in DOUBLE (numpy, the
+    definition north_star names) on 10^6 configs[2]-like lightcurves: every epoch the two chains disagree on must
+    sit within float32 rounding of a clip bound (or the chains picked different but equal-to-rounding order
+    statistics); the disagreement rate is printed and recorded in DESIGN.md."""
+    rng = np.random.default_rng(20)
+    n, T = 1_000_000, 26
+    # configs[2]: phi ~ sum(P^2) / var, var = 300 (1 + 0.1 g_t) (1 + 0.05 u); psi ~ sqrt(phi) N(0,1); movers, cosmic rays,
+    # 2 % invalid epochs
+    gt = np.clip(rng.standard_normal(T), -2, 2)
+    var = 300.0 * (1 + 0.1 * gt)[None, :] * (1 + 0.05 * rng.uniform(-1, 1, (n, 1)))
+    phi = (0.024586 / var).astype(np.float32)
+    z = rng.standard_normal((n, T))
+    z += np.where(rng.random((n, 1)) < 0.1, rng.uniform(1, 8, (n, 1)), 0.0)            # movers
+    z += np.where(rng.random((n, T)) < 0.02, rng.uniform(5, 50, (n, T)), 0.0)          # single-epoch spikes
+    psi = (z * np.sqrt(phi)).astype(np.float32)
+    phi[rng.random((n, T)) < 0.02] = 0.0
+    r = O.sigmag_filter(psi, phi, P())
+    kept32 = ((r["kept"][:, None] >> np.arange(T, dtype=np.uint64)[None, :]) & np.uint64(1)).astype(bool)
+    valid = phi > 0
+    f = np.where(valid, psi.astype(np.float64) / np.where(valid, phi, 1).astype(np.float64), np.inf)
+    s = np.sort(f, axis=1)
+    nv = valid.sum(1)
+    rows = np.arange(n)
+    rk = lambda q: np.clip(np.ceil(q * nv / 100.0).astype(int) - 1, 0, np.maximum(nv - 1, 0))
+    p25, p50, p75 = s[rows, rk(25.0)], s[rows, rk(50.0)], s[rows, rk(75.0)]
+    w = 2.0 * np.float64(np.float32(0.7413)) * (p75 - p25)
+    kept64 = valid & (f >= (p50 - w)[:, None]) & (f <= (p50 + w)[:, None]) & (nv > 0)[:, None]
+    diff = kept32 != kept64
+    n_diff = int(diff.sum())
+    ii, tt = np.nonzero(diff)
+    if n_diff:
+        scale = np.maximum(np.maximum(np.abs(p50[ii]), np.abs(w[ii])), np.abs(f[ii, tt]))
+        dist = np.minimum(np.abs(f[ii, tt] - (p50[ii] - w[ii])), np.abs(f[ii, tt] - (p50[ii] + w[ii])))
+        assert np.all(dist <= 16 * 2.0 ** -24 * scale), float((dist / scale).max())
+    rate = n_diff / float(valid.sum())
+    print(f"R20: {n_diff} of {int(valid.sum())} epoch decisions differ between the float32 and the double chain "
+          f"({rate:.2e}); lightcurves affected: {len(set(ii.tolist()))} of {n}")
+    assert rate < 1e-5
