@@ -227,7 +227,7 @@ def run_ours(args):
     psiphi = torch.empty((T, H, W, 2), dtype=torch.float32, device=dev)
     out = tuple(torch.empty((H, W, sp.K), dtype=dt, device=dev)
                 for dt in (torch.float32, torch.float32, torch.int32, torch.int32))
-    ws = torch.empty(max(256, kb.kbmod_search_workspace_bytes(T, H, W, n_vel, sp)), dtype=torch.uint8, device=dev)
+    ws = torch.empty(max(256, kb.kbmod_search_workspace_bytes_for(T, H, W, st.times, vx, vy, sp)), dtype=torch.uint8, device=dev)
     n_cand = min(100_000, H * W)  # (a6) candidate list: configs[4]'s recipe
     cx0, cy0, cvx, cvy = (torch.from_numpy(a).to(dev) for a in synth.config5_trajectories(4 + rank, H, W, n_cand))
 
@@ -312,7 +312,8 @@ def run_e2e(R, steps):
     h_in = tuple(torch.from_numpy(a).pin_memory() for a in (st.img, st.var, st.mask))
     h_out = tuple(torch.empty((H, W, sp.K), dtype=dt).pin_memory()
                   for dt in (torch.float32, torch.float32, torch.int32, torch.int32))
-    arena = torch.empty(2 * kb.kbmod_pipeline_host_arena_bytes(T, H, W, len(R["vx"]), sp), dtype=torch.uint8, device=R["dev"])
+    arena = torch.empty(2 * kb.kbmod_pipeline_host_arena_bytes_for(T, H, W, st.times, R["vx"], R["vy"], sp), dtype=torch.uint8,
+                        device=R["dev"])
     h2d = sum(a.numel() * a.element_size() for a in h_in)
     d2h = sum(a.numel() * a.element_size() for a in h_out)
     kb.kbmod_pipeline_host_batch([h_in], st.psf, st.times, R["vx"], R["vy"], sp, [h_out], arena)  # warm-up

@@ -16,11 +16,45 @@ LIB_PATH = os.path.join(_HERE, "libkbmod_b200.so")
 ALGO_AUTO, ALGO_DIRECT, ALGO_PRUNED = 0, 1, 2
 MAX_T, MAX_K, MAX_PSF, MAX_STAMP_RADIUS = 64, 32, 31, 15
 
-EXPORTS = ["kbmod_default_params", "kbmod_prepare_psi_phi", "kbmod_displacements",
-           "kbmod_search_workspace_bytes", "kbmod_search", "kbmod_plan_stats", "kbmod_search_stats", "kbmod_search_phase_timing",
-           "kbmod_search_phase_ms", "kbmod_coadd_stamps",
-           "kbmod_eval_trajectories", "kbmod_sigmag_filter", "kbmod_stamp_moments", "kbmod_pipeline_host_arena_bytes",
-           "kbmod_pipeline_host", "kbmod_pipeline_host_batch", "kbmod_measure_smem_gbs", "kbmod_last_error", "kbmod_version"]
+# every symbol include/kbmod_b200.h declares, with its C signature (restype, argtypes): ctypes then converts and
+# range-checks every argument itself (a Python int for a size_t can no longer be truncated to a C int)
+_P, _I, _Z, _D = C.c_void_p, C.c_int, C.c_size_t, C.c_double
+SIGNATURES = {
+    "kbmod_default_params": (None, [_P]),
+    "kbmod_percentile_ranks": (_I, [_P, _I, _P, _P]),
+    "kbmod_prepare_psi_phi": (_I, [_P, _P, _P, _I, _I, _I, _P, _I, _I, _P, _P]),
+    "kbmod_displacements": (_I, [_P, _I, _P, _P, _I, _P, _P]),
+    "kbmod_search_workspace_bytes": (_Z, [_I, _I, _I, _I, _P]),
+    "kbmod_search_workspace_bytes_for": (_Z, [_I, _I, _I, _P, _P, _P, _I, _P, _I, _I]),
+    "kbmod_search": (_I, [_P, _I, _I, _I, _P, _P, _P, _I, _P, _P, _P, _P, _P, _P, _Z, _P]),
+    "kbmod_search_rows": (_I, [_P, _I, _I, _I, _P, _P, _P, _I, _P, _I, _I, _P, _P, _P, _P, _P, _Z, _P]),
+    "kbmod_search_unfiltered_lh": (_I, [_P, _P, _P, _P]),
+    "kbmod_plan_create": (_I, [_I, _I, _I, _P, _P, _P, _I, _P, _I, _I, C.POINTER(_P)]),
+    "kbmod_plan_workspace_bytes": (_Z, [_P]),
+    "kbmod_plan_info": (_I, [_P, _P]),
+    "kbmod_plan_search": (_I, [_P, _P, _P, _P, _P, _P, _P, _Z, _P]),
+    "kbmod_plan_unfiltered_lh": (_I, [_P, _P, _P, _P, _P]),
+    "kbmod_plan_destroy": (None, [_P]),
+    "kbmod_release_thread_state": (_I, []),
+    "kbmod_plan_stats": (_I, [_I, _I, _I, _P, _P, _P, _I, _P, _P]),
+    "kbmod_search_stats": (_I, [_P, _P]),
+    "kbmod_search_phase_timing": (_I, [_I]),
+    "kbmod_search_phase_ms": (_I, [_P]),
+    "kbmod_coadd_stamps": (_I, [_P, _P, _I, _I, _I, _P, _P, _P, _P, _P, _P, _I, _I, _P, _P, _P]),
+    "kbmod_coadd_stamps_filtered": (_I, [_P, _P, _I, _I, _I, _P, _P, _P, _P, _P, _P, _I, _I, _P, _P, _P, _P, _P, _P]),
+    "kbmod_eval_trajectories": (_I, [_P, _I, _I, _I, _P, _P, _P, _P, _P, _I, _P, _P, _P, _P, _P, _P, _P, _P]),
+    "kbmod_sigmag_filter": (_I, [_P, _P, _I, _I, _P, _P, _P, _P, _P]),
+    "kbmod_sigmag_postfilter": (_I, [_P, _P, _I, _I, _P, _P, _P, _P, _P, _P, _P, _P]),
+    "kbmod_stamp_moments": (_I, [_P, _I, _I, _P, _P, _P, _P]),
+    "kbmod_pipeline_host_arena_bytes": (_Z, [_I, _I, _I, _I, _P]),
+    "kbmod_pipeline_host_arena_bytes_for": (_Z, [_I, _I, _I, _P, _P, _P, _I, _P]),
+    "kbmod_pipeline_host": (_I, [_P, _P, _P, _I, _I, _I, _P, _I, _I, _P, _P, _P, _I, _P, _P, _P, _P, _P, _P, _Z, _P]),
+    "kbmod_pipeline_host_batch": (_I, [_I, _P, _P, _P, _I, _I, _I, _P, _I, _I, _P, _P, _P, _I, _P, _P, _P, _P, _P, _P, _Z, _P]),
+    "kbmod_measure_smem_gbs": (_I, [_I, _P, _P, _P]),
+    "kbmod_last_error": (C.c_char_p, []),
+    "kbmod_version": (_I, []),
+}
+EXPORTS = list(SIGNATURES)
 
 
 class KbmodError(RuntimeError):
@@ -32,7 +66,8 @@ class KbmodError(RuntimeError):
 class CParams(C.Structure):
     _fields_ = [("sigmag_enable", C.c_int), ("pct_lo", C.c_float), ("pct_hi", C.c_float),
                 ("sigmag_coeff", C.c_float), ("n_sigma", C.c_float), ("filter_on", C.c_int),
-                ("min_lh", C.c_float), ("min_obs", C.c_int), ("K", C.c_int), ("algo", C.c_int)]
+                ("min_lh", C.c_float), ("min_obs", C.c_int), ("K", C.c_int), ("algo", C.c_int),
+                ("pct_interp", C.c_int)]
 
 
 @dataclass
@@ -48,10 +83,11 @@ class SearchParams:
     min_obs: int = 1
     K: int = 8
     algo: int = ALGO_AUTO
+    pct_interp: int = 0
 
     def c(self) -> CParams:
         return CParams(self.sigmag_enable, self.pct_lo, self.pct_hi, self.sigmag_coeff, self.n_sigma,
-                       self.filter_on, self.min_lh, self.min_obs, self.K, self.algo)
+                       self.filter_on, self.min_lh, self.min_obs, self.K, self.algo, self.pct_interp)
 
 
 _lib = None
@@ -64,11 +100,9 @@ def lib():
         if not os.path.exists(LIB_PATH):
             raise KbmodError(-4, f"{LIB_PATH} is missing: run `python -m paper_2109_03296_b200.build`")
         L = C.CDLL(LIB_PATH)
-        L.kbmod_last_error.restype = C.c_char_p
-        L.kbmod_version.restype = C.c_int
-        L.kbmod_search_workspace_bytes.restype = C.c_size_t
-        L.kbmod_pipeline_host_arena_bytes.restype = C.c_size_t
-        L.kbmod_default_params.restype = None
+        for name, (res, args) in SIGNATURES.items():
+            fn = getattr(L, name)  # AttributeError if the library does not export what the header declares
+            fn.restype, fn.argtypes = res, args
         _lib = L
     return _lib
 
@@ -99,6 +133,28 @@ def _host(a, dtype):
     return a, a.ctypes.data_as(C.c_void_p)
 
 
+def _grid(times, vx, vy, T):
+    """Host arrays of a search: times float64 [T], vx, vy float32 [n_vel]; shapes checked here."""
+    t, tp = _host(times, np.float64)
+    x, xp = _host(vx, np.float32)
+    y, yp = _host(vy, np.float32)
+    if t.ndim != 1 or len(t) != T:
+        raise ValueError(f"times must be [T] = [{T}], got {t.shape}")
+    if x.ndim != 1 or x.shape != y.shape:
+        raise ValueError(f"vx, vy must be 1-D arrays of one length, got {x.shape}, {y.shape}")
+    return (t, x, y), (tp, xp, yp)
+
+
+def _check_out(out, shape):
+    import torch
+    want = (torch.float32, torch.float32, torch.int32, torch.int32)
+    if len(out) != 4:
+        raise ValueError("out must be (lh, flux, vel_idx, n_obs)")
+    for o, dt in zip(out, want):
+        if tuple(o.shape) != tuple(shape) or o.dtype != dt:
+            raise ValueError(f"output tensors must be {tuple(shape)} {want}, got {tuple(o.shape)} {o.dtype}")
+
+
 def _stream(stream=None):
     import torch
     s = torch.cuda.current_stream() if stream is None else stream
@@ -113,6 +169,14 @@ def kbmod_default_params() -> SearchParams:
     cp = CParams()
     lib().kbmod_default_params(C.byref(cp))
     return SearchParams(*[getattr(cp, f) for f, _ in CParams._fields_])
+
+
+def kbmod_percentile_ranks(params: SearchParams, n: int):
+    """Host-only: [(k, g)] for (pct_lo, 50, pct_hi) of n valid samples; g < 0 means "take s[k]"."""
+    cp = params.c()
+    k, g = (C.c_int * 3)(), (C.c_float * 3)()
+    _check(lib().kbmod_percentile_ranks(C.byref(cp), n, k, g))
+    return [(int(k[i]), float(g[i])) for i in range(3)]
 
 
 def kbmod_displacements(times, vx, vy):
@@ -133,10 +197,16 @@ def kbmod_prepare_psi_phi(img, var, mask, psf, out=None, stream=None):
     import torch
     T, H, W = img.shape
     p, pp = _host(psf, np.float32)
+    if p.ndim not in (2, 3) or p.shape[-1] != p.shape[-2]:
+        raise ValueError(f"psf must be [k][k] or [T][k][k], got {p.shape}")
     n_psf = 1 if p.ndim == 2 else p.shape[0]
     k = p.shape[-1]
+    if tuple(var.shape) != (T, H, W) or (mask is not None and tuple(mask.shape) != (T, H, W)):
+        raise ValueError("img, var and mask must have one shape [T][H][W]")
     if out is None:
         out = torch.empty((T, H, W, 2), dtype=torch.float32, device=img.device)
+    elif tuple(out.shape) != (T, H, W, 2):
+        raise ValueError(f"out must be [T][H][W][2], got {tuple(out.shape)}")
     _check(lib().kbmod_prepare_psi_phi(_dev(img, torch.float32), _dev(var, torch.float32),
                                        _dev(mask, torch.uint8, allow_none=True), T, H, W, pp, n_psf, k,
                                        _dev(out, torch.float32), _stream(stream)))
@@ -144,36 +214,154 @@ def kbmod_prepare_psi_phi(img, var, mask, psf, out=None, stream=None):
 
 
 def kbmod_search_workspace_bytes(T, H, W, n_vel, params: SearchParams) -> int:
+    """Upper bound for any list of n_vel velocities (the stack padded by the image size on every side)."""
     cp = params.c()
     return int(lib().kbmod_search_workspace_bytes(T, H, W, n_vel, C.byref(cp)))
 
 
-def kbmod_search(psiphi, times, vx, vy, params: SearchParams, out=None, workspace=None, stream=None):
-    """(a3)-(a5).  psiphi float32 CUDA [T][H][W][2].  Returns (lh, flux, vel_idx, n_obs), each [H][W][K]."""
+def kbmod_search_workspace_bytes_for(T, H, W, times, vx, vy, params: SearchParams, rows=None) -> int:
+    """Exact workspace need of kbmod_search / kbmod_search_rows for this grid."""
+    (t, x, y), (tp, xp, yp) = _grid(times, vx, vy, T)
+    r0, r1 = (0, H) if rows is None else rows
+    cp = params.c()
+    n = int(lib().kbmod_search_workspace_bytes_for(T, H, W, tp, xp, yp, len(x), C.byref(cp), r0, r1))
+    if n == 0:
+        raise KbmodError(-1, lib().kbmod_last_error().decode())
+    return n
+
+
+def kbmod_search(psiphi, times, vx, vy, params: SearchParams, out=None, workspace=None, stream=None, rows=None):
+    """(a3)-(a5).  psiphi float32 CUDA [T][H][W][2].  Returns (lh, flux, vel_idx, n_obs), each [H][W][K]; with
+    rows=(row_begin, row_end) the search is restricted to that band of start rows and the outputs are
+    [row_end - row_begin][W][K] (kbmod_search_rows)."""
     import torch
     T, H, W, two = psiphi.shape
-    assert two == 2
-    t, tp = _host(times, np.float64)
-    x, xp = _host(vx, np.float32)
-    y, yp = _host(vy, np.float32)
-    assert len(t) == T and len(x) == len(y)
+    if two != 2:
+        raise ValueError("psiphi must be [T][H][W][2]")
+    (t, x, y), (tp, xp, yp) = _grid(times, vx, vy, T)
     K = params.K
     dev = psiphi.device
+    r0, r1 = (0, H) if rows is None else (int(rows[0]), int(rows[1]))
+    shape = (max(r1 - r0, 0), W, K)
     if out is None:
-        out = (torch.empty((H, W, K), dtype=torch.float32, device=dev),
-               torch.empty((H, W, K), dtype=torch.float32, device=dev),
-               torch.empty((H, W, K), dtype=torch.int32, device=dev),
-               torch.empty((H, W, K), dtype=torch.int32, device=dev))
-    nbytes = kbmod_search_workspace_bytes(T, H, W, len(x), params)
-    if workspace is None:
-        workspace = torch.empty(max(nbytes, 256), dtype=torch.uint8, device=dev)
+        out = (torch.empty(shape, dtype=torch.float32, device=dev), torch.empty(shape, dtype=torch.float32, device=dev),
+               torch.empty(shape, dtype=torch.int32, device=dev), torch.empty(shape, dtype=torch.int32, device=dev))
+    else:
+        _check_out(out, shape)
     cp = params.c()
-    _check(lib().kbmod_search(_dev(psiphi, torch.float32), T, H, W, tp, xp, yp, len(x), C.byref(cp),
-                              _dev(out[0], torch.float32), _dev(out[1], torch.float32),
-                              _dev(out[2], torch.int32), _dev(out[3], torch.int32), _dev(workspace),
-                              C.c_size_t(workspace.numel()), _stream(stream)))
+    if workspace is None:
+        nbytes = int(lib().kbmod_search_workspace_bytes_for(T, H, W, tp, xp, yp, len(x), C.byref(cp), r0, r1))
+        workspace = torch.empty(max(nbytes, 256), dtype=torch.uint8, device=dev)
+    args = [_dev(psiphi, torch.float32), T, H, W, tp, xp, yp, len(x), C.byref(cp)]
+    tail = [_dev(out[0], torch.float32), _dev(out[1], torch.float32), _dev(out[2], torch.int32),
+            _dev(out[3], torch.int32), _dev(workspace), workspace.numel(), _stream(stream)]
+    if rows is None:
+        _check(lib().kbmod_search(*args, *tail))
+    else:
+        _check(lib().kbmod_search_rows(*args, r0, r1, *tail))
     kbmod_search.last_workspace = workspace
     return out
+
+
+def kbmod_search_unfiltered_lh(workspace, vel_idx, stream=None):
+    """Unfiltered sum-LH of the result slots of the last kbmod_search of this thread that used
+    `workspace`.  vel_idx int32 CUDA [rows][W][K] -> float32 CUDA of the same shape."""
+    import torch
+    out = torch.empty(vel_idx.shape, dtype=torch.float32, device=vel_idx.device)
+    _check(lib().kbmod_search_unfiltered_lh(_dev(workspace), _dev(vel_idx, torch.int32), _dev(out), _stream(stream)))
+    return out
+
+
+class Plan:
+    """kbmod_plan: the geometry-only part of a search (host memory), shared by any number of searches / streams."""
+
+    def __init__(self, T, H, W, times, vx, vy, params: SearchParams, rows=None):
+        (t, x, y), (tp, xp, yp) = _grid(times, vx, vy, T)
+        self.T, self.H, self.W, self.K, self.n_vel = T, H, W, params.K, len(x)
+        self.rows = (0, H) if rows is None else (int(rows[0]), int(rows[1]))
+        self._h = C.c_void_p(0)
+        cp = params.c()
+        _check(lib().kbmod_plan_create(T, H, W, tp, xp, yp, len(x), C.byref(cp), self.rows[0], self.rows[1], C.byref(self._h)))
+
+    def workspace_bytes(self) -> int:
+        return int(lib().kbmod_plan_workspace_bytes(self._h))
+
+    def info(self):
+        out = (C.c_double * 8)()
+        _check(lib().kbmod_plan_info(self._h, out))
+        return dict(algo=int(out[0]), n_groups=int(out[1]), staged_bytes_per_eval=float(out[2]),
+                    off_image_fraction=float(out[3]), canvas=(int(out[4]), int(out[5])), too_scattered=bool(out[6]),
+                    table_bytes=int(out[7]))
+
+    def search(self, psiphi, out=None, workspace=None, stream=None):
+        import torch
+        if tuple(psiphi.shape) != (self.T, self.H, self.W, 2):
+            raise ValueError("psiphi does not have the plan's shape")
+        dev = psiphi.device
+        shape = (self.rows[1] - self.rows[0], self.W, self.K)
+        if out is None:
+            out = tuple(torch.empty(shape, dtype=dt, device=dev)
+                        for dt in (torch.float32, torch.float32, torch.int32, torch.int32))
+        else:
+            _check_out(out, shape)
+        if workspace is None:
+            workspace = torch.empty(max(self.workspace_bytes(), 256), dtype=torch.uint8, device=dev)
+        _check(lib().kbmod_plan_search(self._h, _dev(psiphi, torch.float32), _dev(out[0]), _dev(out[1]), _dev(out[2]),
+                                       _dev(out[3]), _dev(workspace), workspace.numel(), _stream(stream)))
+        self.last_workspace = workspace
+        return out
+
+    def unfiltered_lh(self, workspace, vel_idx, stream=None):
+        import torch
+        out = torch.empty(vel_idx.shape, dtype=torch.float32, device=vel_idx.device)
+        _check(lib().kbmod_plan_unfiltered_lh(self._h, _dev(workspace), _dev(vel_idx, torch.int32), _dev(out),
+                                              _stream(stream)))
+        return out
+
+    def destroy(self):
+        if self._h:
+            lib().kbmod_plan_destroy(self._h)
+            self._h = C.c_void_p(0)
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass
+
+
+# the plan entry points under their C names (thin aliases of the Plan class)
+def kbmod_plan_create(T, H, W, times, vx, vy, params: SearchParams, rows=None) -> Plan:
+    return Plan(T, H, W, times, vx, vy, params, rows)
+
+
+def kbmod_plan_workspace_bytes(plan: Plan) -> int:
+    return plan.workspace_bytes()
+
+
+def kbmod_plan_info(plan: Plan):
+    return plan.info()
+
+
+def kbmod_plan_search(plan: Plan, psiphi, out=None, workspace=None, stream=None):
+    return plan.search(psiphi, out=out, workspace=workspace, stream=stream)
+
+
+def kbmod_plan_unfiltered_lh(plan: Plan, workspace, vel_idx, stream=None):
+    return plan.unfiltered_lh(workspace, vel_idx, stream=stream)
+
+
+def kbmod_plan_destroy(plan: Plan):
+    plan.destroy()
+
+
+def kbmod_search_rows(psiphi, times, vx, vy, params: SearchParams, rows, out=None, workspace=None, stream=None):
+    return kbmod_search(psiphi, times, vx, vy, params, out=out, workspace=workspace, stream=stream, rows=rows)
+
+
+def kbmod_release_thread_state():
+    """Frees the per-thread conveniences of the library (cached plan, timing events, batch copy streams)."""
+    _check(lib().kbmod_release_thread_state())
 
 
 def kbmod_plan_stats(T, H, W, times, vx, vy, params: SearchParams):
@@ -197,7 +385,7 @@ def kbmod_search_stats(workspace):
 
 def kbmod_search_phase_timing(enable: bool):
     """Switches the per-phase CUDA-event timing of kbmod_search on or off for this host thread."""
-    _check(lib().kbmod_search_phase_timing(C.c_int(1 if enable else 0)))
+    _check(lib().kbmod_search_phase_timing(1 if enable else 0))
 
 
 def kbmod_search_phase_ms():
@@ -222,6 +410,33 @@ def kbmod_coadd_stamps(img, mask, times, x0, y0, vx, vy, radius, epoch_mask=None
                                     _dev(vy, torch.float32), _dev(epoch_mask, allow_none=True), n, radius,
                                     _dev(mean, allow_none=True), _dev(med, allow_none=True), _stream(stream)))
     return mean, med
+
+
+def kbmod_coadd_stamps_filtered(img, mask, times, x0, y0, vx, vy, radius, epoch_mask=None, thresholds=None,
+                                want_mean=True, want_median=True, stream=None):
+    """(a6) + the central-moment filter in one kernel.  Returns (mean, median, moments float64 [n][5],
+    keep uint8 [n]); the moments are those of the median stamp, bit-identical to kbmod_stamp_moments(median)."""
+    import torch
+    T, H, W = img.shape
+    t, tp = _host(times, np.float64)
+    n, S = x0.numel(), 2 * radius + 1
+    dev = img.device
+    mean = torch.empty((n, S, S), dtype=torch.float32, device=dev) if want_mean else None
+    med = torch.empty((n, S, S), dtype=torch.float32, device=dev) if want_median else None
+    mom = torch.empty((n, 5), dtype=torch.float64, device=dev)
+    keep = torch.empty((n,), dtype=torch.uint8, device=dev)
+    thr_arr, thr_ptr = (None, C.c_void_p(0)) if thresholds is None else _host(thresholds, np.float64)
+    if thr_arr is not None and thr_arr.shape != (5,):
+        raise KbmodError(-1, "thresholds must be 5 numbers: x, y, xy, xx, yy")
+    for a in (x0, y0, vx, vy):
+        if a.numel() != n:
+            raise ValueError("x0, y0, vx, vy must have one length")
+    _check(lib().kbmod_coadd_stamps_filtered(_dev(img, torch.float32), _dev(mask, torch.uint8, allow_none=True), T, H, W,
+                                             tp, _dev(x0, torch.int32), _dev(y0, torch.int32), _dev(vx, torch.float32),
+                                             _dev(vy, torch.float32), _dev(epoch_mask, allow_none=True), n, radius,
+                                             _dev(mean, allow_none=True), _dev(med, allow_none=True), thr_ptr, _dev(mom),
+                                             _dev(keep), _stream(stream)))
+    return mean, med, mom, keep
 
 
 def kbmod_eval_trajectories(psiphi, times, x0, y0, vx, vy, params: SearchParams, stream=None):
@@ -255,6 +470,28 @@ def kbmod_sigmag_filter(psi_lc, phi_lc, params: SearchParams, stream=None):
     return r
 
 
+def kbmod_sigmag_postfilter(psi_lc, phi_lc, params: SearchParams, compact=True, stream=None):
+    """The paper's post-filter: sigma-G on given lightcurves, then reject L' < min_lh.  Returns
+    dict(kept, lh, flux, passed uint8 [n], survivors int32 [n] (first n_pass entries valid, ascending), n_pass
+    uint64 [4] device counter ([0] = number of survivors))."""
+    import torch
+    n, T = psi_lc.shape
+    if tuple(phi_lc.shape) != (n, T):
+        raise ValueError("psi_lc and phi_lc must have one shape [n][T]")
+    dev = psi_lc.device
+    r = dict(kept=torch.empty(n, dtype=torch.int64, device=dev), lh=torch.empty(n, dtype=torch.float32, device=dev),
+             flux=torch.empty(n, dtype=torch.float32, device=dev), passed=torch.empty(n, dtype=torch.uint8, device=dev))
+    if compact:
+        r["survivors"] = torch.empty(n, dtype=torch.int32, device=dev)
+        r["n_pass"] = torch.empty(4, dtype=torch.int64, device=dev)
+    cp = params.c()
+    _check(lib().kbmod_sigmag_postfilter(_dev(psi_lc, torch.float32), _dev(phi_lc, torch.float32), n, T, C.byref(cp),
+                                         _dev(r["kept"]), _dev(r["lh"]), _dev(r["flux"]), _dev(r["passed"]),
+                                         _dev(r.get("survivors"), allow_none=True), _dev(r.get("n_pass"), allow_none=True),
+                                         _stream(stream)))
+    return r
+
+
 def kbmod_stamp_moments(stamps, thresholds=None, stream=None):
     """Central moments (x, y, xy, xx, yy) of [n][S][S] stamps and the paper's keep / reject flag.
     Returns (moments float64 [n][5], keep uint8 [n])."""
@@ -268,7 +505,7 @@ def kbmod_stamp_moments(stamps, thresholds=None, stream=None):
     thr_arr, thr_ptr = (None, C.c_void_p(0)) if thresholds is None else _host(thresholds, np.float64)
     if thr_arr is not None and thr_arr.shape != (5,):
         raise KbmodError(-1, "thresholds must be 5 numbers: x, y, xy, xx, yy")
-    _check(lib().kbmod_stamp_moments(s, C.c_int(n), C.c_int(S // 2), thr_ptr, _dev(mom), _dev(keep), _stream(stream)))
+    _check(lib().kbmod_stamp_moments(s, n, S // 2, thr_ptr, _dev(mom), _dev(keep), _stream(stream)))
     return mom, keep
 
 
@@ -293,22 +530,40 @@ def kbmod_pipeline_host_batch(stacks, psf, times, vx, vy, params: SearchParams, 
     masks = arr([s_[2] for s_ in stacks]) if has_mask else None
     o = [arr([o_[j] for o_ in outs]) for j in range(4)]
     cp = params.c()
-    _check(lib().kbmod_pipeline_host_batch(C.c_int(n), imgs, vars_, masks, T, H, W, pp, n_psf, p.shape[-1], tp, xp, yp, len(x),
-                                           C.byref(cp), o[0], o[1], o[2], o[3], _dev(arena), C.c_size_t(arena.numel()),
-                                           _stream(stream)))
+    for o_ in outs:
+        for a in o_:
+            assert tuple(a.shape) == (H, W, params.K) and not a.is_cuda and a.is_contiguous()
+    _check(lib().kbmod_pipeline_host_batch(n, C.cast(imgs, C.c_void_p), C.cast(vars_, C.c_void_p),
+                                           C.cast(masks, C.c_void_p) if masks is not None else None, T, H, W, pp, n_psf,
+                                           p.shape[-1], tp, xp, yp, len(x), C.byref(cp), C.cast(o[0], C.c_void_p),
+                                           C.cast(o[1], C.c_void_p), C.cast(o[2], C.c_void_p), C.cast(o[3], C.c_void_p),
+                                           _dev(arena), arena.numel(), _stream(stream)))
     return outs
 
 
 def kbmod_measure_smem_gbs(bytes_per_lane: int = 4, stream=None) -> float:
     """Measured shared-memory load bandwidth of the whole GPU in GB/s (roofline denominator; synchronises)."""
+    import torch
     out = C.c_double(0.0)
-    _check(lib().kbmod_measure_smem_gbs(C.c_int(bytes_per_lane), C.byref(out), _stream(stream)))
+    scratch = torch.zeros(4, dtype=torch.uint8, device="cuda")
+    _check(lib().kbmod_measure_smem_gbs(bytes_per_lane, _dev(scratch), C.byref(out), _stream(stream)))
     return float(out.value)
 
 
 def kbmod_pipeline_host_arena_bytes(T, H, W, n_vel, params: SearchParams) -> int:
+    """Upper bound for any list of n_vel velocities."""
     cp = params.c()
     return int(lib().kbmod_pipeline_host_arena_bytes(T, H, W, n_vel, C.byref(cp)))
+
+
+def kbmod_pipeline_host_arena_bytes_for(T, H, W, times, vx, vy, params: SearchParams) -> int:
+    """Exact arena need of kbmod_pipeline_host / one buffer of kbmod_pipeline_host_batch for this grid."""
+    (t, x, y), (tp, xp, yp) = _grid(times, vx, vy, T)
+    cp = params.c()
+    n = int(lib().kbmod_pipeline_host_arena_bytes_for(T, H, W, tp, xp, yp, len(x), C.byref(cp)))
+    if n == 0:
+        raise KbmodError(-1, lib().kbmod_last_error().decode())
+    return n
 
 
 def kbmod_pipeline_host(img, var, mask, psf, times, vx, vy, params: SearchParams, out, arena, stream=None):
@@ -328,5 +583,5 @@ def kbmod_pipeline_host(img, var, mask, psf, times, vx, vy, params: SearchParams
     hp = lambda a: C.c_void_p(a.data_ptr()) if a is not None else C.c_void_p(0)
     _check(lib().kbmod_pipeline_host(hp(img), hp(var), hp(mask), T, H, W, pp, n_psf, p.shape[-1], tp, xp, yp, len(x),
                                      C.byref(cp), hp(out[0]), hp(out[1]), hp(out[2]), hp(out[3]), _dev(arena),
-                                     C.c_size_t(arena.numel()), _stream(stream)))
+                                     arena.numel(), _stream(stream)))
     return out

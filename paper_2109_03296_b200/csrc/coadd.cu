@@ -3,8 +3,11 @@
 // One block per trajectory, one thread per stamp pixel: for each epoch the block reads a
 // (2r+1)-wide row segment per stamp row (coalesced within the row), the T samples of a pixel
 // stay in registers, and the median comes from the same compare-exchange network as sigma-G
-// (with two-sided +-inf padding so that its position is fixed; see below).
-#include "common.cuh"
+// (with two-sided +-inf padding so that its position is fixed; see below).  Optionally the block goes on to the step
+// behind the coadd (L141: "we computed the central moments of postage stamps ..."): the medians are parked in shared
+// memory and one warp computes the five moments and the keep flag with the same device function as
+// kbmod_stamp_moments -- no second pass over the stamps in global memory.
+#include "moments.cuh"
 
 namespace {
 
@@ -13,8 +16,11 @@ __global__ void __launch_bounds__(448) coadd_kernel(const float* __restrict__ im
                              const __grid_constant__ DevTimes times, const int32_t* __restrict__ x0s,
                              const int32_t* __restrict__ y0s, const float* __restrict__ vxs,
                              const float* __restrict__ vys, const unsigned long long* __restrict__ epoch_mask,
-                             int radius, float* __restrict__ mean_out, float* __restrict__ median_out) {
+                             int radius, float* __restrict__ mean_out, float* __restrict__ median_out, int want_moments,
+                             const __grid_constant__ MomentThr thr, double* __restrict__ moments_out,
+                             uint8_t* __restrict__ keep_out) {
     __shared__ int sdx[KBMOD_MAX_T], sdy[KBMOD_MAX_T];
+    __shared__ float smed[(2 * KBMOD_MAX_STAMP_RADIUS + 1) * (2 * KBMOD_MAX_STAMP_RADIUS + 1)];
     const int i = blockIdx.x;
     const int S = 2 * radius + 1;
     const int x0 = x0s[i], y0 = y0s[i];
@@ -73,6 +79,20 @@ __global__ void __launch_bounds__(448) coadd_kernel(const float* __restrict__ im
     const size_t o = (size_t)i * S * S + p;
     if (mean_out) mean_out[o] = mean;
     if (median_out) median_out[o] = med;
+    if (want_moments) smed[p] = med;
+    }
+    if (want_moments) {  // block-uniform
+        __syncthreads();
+        if (threadIdx.x < 32) {
+            double m[5];
+            bool keep;
+            kb_moments_warp(smed, radius, thr, m, keep);
+            if (threadIdx.x == 0) {
+                if (moments_out)
+                    for (int k = 0; k < 5; ++k) moments_out[(size_t)i * 5 + k] = m[k];
+                if (keep_out) keep_out[i] = keep ? 1 : 0;
+            }
+        }
     }
 }
 
@@ -81,14 +101,18 @@ __global__ void __launch_bounds__(448) coadd_kernel(const float* __restrict__ im
 int kb_launch_coadd(const float* d_img, const uint8_t* d_mask, int T, int TPv, int H, int W, const DevTimes& times,
                     const int32_t* d_x0, const int32_t* d_y0, const float* d_vx, const float* d_vy,
                     const unsigned long long* d_epoch_mask, int n_traj, int radius, float* d_mean, float* d_median,
-                    cudaStream_t st) {
+                    const double* thr5, double* d_moments, uint8_t* d_keep, cudaStream_t st) {
+    MomentThr thr;
+    for (int k = 0; k < 5; ++k) thr.t[k] = thr5 ? thr5[k] : 0.0;
+    const int want_moments = (d_moments || d_keep) ? 1 : 0;
     const int S = 2 * radius + 1;
     int threads = ((S * S + 31) / 32) * 32;  // one stamp pixel per thread up to 21x21, a loop above that
     if (threads < 64) threads = 64;          // the first T threads compute the displacements
     if (threads > 448) threads = 256;
     KB_DISPATCH_TP(TPv, {
         coadd_kernel<TP><<<n_traj, threads, 0, st>>>(d_img, d_mask, T, H, W, times, d_x0, d_y0, d_vx, d_vy,
-                                                        d_epoch_mask, radius, d_mean, d_median);
+                                                        d_epoch_mask, radius, d_mean, d_median, want_moments, thr,
+                                                        d_moments, d_keep);
     });
     KB_CUDA(cudaGetLastError());
     return KBMOD_OK;

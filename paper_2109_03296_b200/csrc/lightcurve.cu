@@ -1,6 +1,8 @@
 // Single-trajectory variant (s4.1) and the sigma-G post-filter on given lightcurves
 // (s3.1; BASELINE configs[4]).  One thread per trajectory / lightcurve; the filter is
 // the same device function the search kernels use (common.cuh: kb_score_lightcurve).
+#include <algorithm>
+
 #include "common.cuh"
 
 namespace {
@@ -62,7 +64,7 @@ template <int TP>
 __global__ void __launch_bounds__(LC_THREADS)
 sigmag_filter_kernel(const float* __restrict__ psi_lc, const float* __restrict__ phi_lc, int n_lc, int T,
                      const __grid_constant__ DevParams P, unsigned long long* __restrict__ kept_out,
-                     float* __restrict__ lh_out, float* __restrict__ flux_out) {
+                     float* __restrict__ lh_out, float* __restrict__ flux_out, uint8_t* __restrict__ pass_out) {
     extern __shared__ float scratch_all[];
     float* scratch = scratch_all + threadIdx.x;
     const int i = blockIdx.x * LC_THREADS + threadIdx.x;
@@ -81,10 +83,66 @@ sigmag_filter_kernel(const float* __restrict__ psi_lc, const float* __restrict__
     }
     float lh, flux;
     unsigned long long kept;
-    kb_score_lightcurve<TP>(psi, phi, P, scratch, LC_THREADS, lh, flux, kept);
+    const int nk = kb_score_lightcurve<TP>(psi, phi, P, scratch, LC_THREADS, lh, flux, kept);
     if (kept_out) kept_out[i] = kept;
     if (lh_out) lh_out[i] = lh;
     if (flux_out) flux_out[i] = flux;
+    // "reject the trajectory if the recomputed likelihood (sum LH') is less than 10"
+    if (pass_out) pass_out[i] = (nk > 0 && lh >= P.min_lh) ? 1 : 0;
+}
+
+// Ordered compaction of the pass flags into a list of surviving lightcurve indices.  Blocks take contiguous chunks
+// in ticket order (a block's ticket is its arrival order, so the block it waits for has always started: no
+// co-residency assumption), count their survivors, chain the running total through ctr[0] and write their indices
+// at the offset they were handed.  ctr: [0] running total (= the number of survivors at the end), [1] tickets
+// issued, [2] chunks that have published their total; all zero on entry.
+constexpr int CP_THREADS = 256;
+__global__ void __launch_bounds__(CP_THREADS)
+compact_pass_kernel(const uint8_t* __restrict__ pass, int n, int chunk, int32_t* __restrict__ survivors,
+                    unsigned long long* __restrict__ ctr) {
+    __shared__ unsigned int s_warp[CP_THREADS / 32];
+    __shared__ unsigned long long s_base;
+    __shared__ unsigned int s_ticket;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    if (threadIdx.x == 0) s_ticket = (unsigned int)atomicAdd(ctr + 1, 1ull);
+    __syncthreads();
+    const unsigned int ticket = s_ticket;
+    const long long lo = (long long)ticket * chunk, hi = lo + chunk < n ? lo + chunk : n;
+    // pass 1: count
+    unsigned int cnt = 0;
+    for (long long i = lo + threadIdx.x; i < hi; i += CP_THREADS) cnt += pass[i] ? 1u : 0u;
+    cnt = __reduce_add_sync(0xFFFFFFFFu, cnt);
+    if (lane == 0) s_warp[warp] = cnt;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        unsigned int total = 0;
+        for (int w = 0; w < CP_THREADS / 32; ++w) total += s_warp[w];
+        volatile unsigned long long* done = ctr + 2;
+        while (*done != (unsigned long long)ticket) __nanosleep(64);
+        __threadfence();
+        s_base = atomicAdd(ctr, (unsigned long long)total);  // only this block touches ctr[0] now: the old value is its offset
+        __threadfence();
+        *done = (unsigned long long)ticket + 1ull;
+    }
+    __syncthreads();
+    unsigned long long base = s_base;
+    // pass 2: ordered write, one tile of CP_THREADS flags at a time
+    for (long long t0 = lo; t0 < hi; t0 += CP_THREADS) {
+        const long long i = t0 + threadIdx.x;
+        const bool f = i < hi && pass[i];
+        const unsigned int bal = __ballot_sync(0xFFFFFFFFu, f);
+        __syncthreads();  // s_warp of the previous tile has been read
+        if (lane == 0) s_warp[warp] = __popc(bal);
+        __syncthreads();
+        unsigned int before = 0, total = 0;
+        for (int w = 0; w < CP_THREADS / 32; ++w) {
+            const unsigned int c = s_warp[w];
+            before += w < warp ? c : 0u;
+            total += c;
+        }
+        if (f && survivors) survivors[base + before + __popc(bal & ((1u << lane) - 1u))] = (int32_t)i;
+        base += total;
+    }
 }
 
 }  // namespace
@@ -106,12 +164,20 @@ int kb_launch_eval_trajectories(const float* d_psiphi, int T, int TPv, int H, in
 }
 
 int kb_launch_sigmag_filter(const float* d_psi_lc, const float* d_phi_lc, int n_lc, int T, int TPv, const DevParams& P,
-                            unsigned long long* d_kept, float* d_lh, float* d_flux, cudaStream_t st) {
+                            unsigned long long* d_kept, float* d_lh, float* d_flux, uint8_t* d_pass,
+                            unsigned long long* d_n_pass, int32_t* d_survivors, cudaStream_t st) {
     const int grid = (n_lc + LC_THREADS - 1) / LC_THREADS;
     KB_DISPATCH_TP(TPv, {
         const size_t smem = (size_t)TP * LC_THREADS * sizeof(float);
-        sigmag_filter_kernel<TP><<<grid, LC_THREADS, smem, st>>>(d_psi_lc, d_phi_lc, n_lc, T, P, d_kept, d_lh, d_flux);
+        sigmag_filter_kernel<TP><<<grid, LC_THREADS, smem, st>>>(d_psi_lc, d_phi_lc, n_lc, T, P, d_kept, d_lh, d_flux, d_pass);
     });
     KB_CUDA(cudaGetLastError());
+    if (d_n_pass) {
+        KB_CUDA(cudaMemsetAsync(d_n_pass, 0, 4 * sizeof(unsigned long long), st));
+        const int chunk = std::max(CP_THREADS * 16, (n_lc + 1023) / 1024);  // at most 1024 chunks in the chain
+        const int blocks = (n_lc + chunk - 1) / chunk;
+        compact_pass_kernel<<<blocks, CP_THREADS, 0, st>>>(d_pass, n_lc, chunk, d_survivors, d_n_pass);
+        KB_CUDA(cudaGetLastError());
+    }
     return KBMOD_OK;
 }

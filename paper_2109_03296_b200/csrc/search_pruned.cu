@@ -2,30 +2,32 @@
 // for trajectories whose EXACT upper bound reaches the threshold min_lh (trajectories
 // with a recomputed likelihood below 10 are rejected; L115: only sum-LH > 10 leave the GPU).
 //
-// Bound.  For any kept set S produced by the sigma-G filter,
-//     L' = sum_S psi / sqrt(sum_S phi)  <=  sum_valid max(psi,0) / sqrt(m(n) * min_valid phi)  =: U
-// because sum_S psi <= sum_valid psi_+, and S always contains every epoch whose value lies between
-// the two percentiles (the clip window is the median +- n_sigma*C*(P_hi-P_lo) with n_sigma*C >= 1 and
-// P_lo <= P_50 <= P_hi), so |S| >= m(n) = rank_hi(n) - rank_lo(n) + 1 and sum_S phi >= m(n) min phi.
-// U needs one float2 per trajectory-epoch: (a, q) = (psi_+, -1/sqrt(phi)), zero where invalid:
-//     A += a;  qmin = min(qmin, q);  n += (q < 0)        U = A * (-qmin) / sqrt(m(n))
+// Bound.  For any kept set S the sigma-G filter can produce,
+//     L' = sum_S psi / sqrt(sum_S phi)  <=  sum_valid max(psi, 0) / sqrt(F(m(n) - n_low))  =: U
+// because sum_S psi <= sum_valid psi_+, and S always contains every sample between the two percentiles (the clip
+// window is the median +- n_sigma*C*(P_hi - P_lo) with n_sigma*C >= 1 and P_lo <= P_50 <= P_hi), so |S| >= m(n);
+// at most n_low members of S have phi below their epoch's floor f_t, the others have phi >= f_t, and F(k) is the
+// sum of the k smallest floors.  U needs ONE packed 32-bit word per trajectory-epoch evaluation:
+//     word = ceil(psi_+ / unit) << 2c  |  (phi < f_t) << c  |  1        (c = bits of an epoch count; 0 = invalid)
+// so a single integer add per evaluation accumulates the fixed-point sum (rounded up), n_low and n.
 //
 // Kernels (all on the caller's stream, per batch of tiles):
-//   bound_plane_kernel   once: the (a, q) planes, row pitch even so that TMA boxes start 16-byte aligned
-//   bound_phase_kernel   where the time goes.  Persistent, one CTA per SM = 16 consumer warps + 1
-//                        producer warp.  A CTA owns a 64x16 tile of start pixels and walks the velocity
-//                        groups (<= 16 neighbouring velocities); for each epoch the tile (+) the group's
-//                        displacement bounding box is staged by TMA (zero fill outside the image = the
-//                        off-chip rule) into a byte ring in shared memory, several epochs ahead, and
-//                        every consumer thread gathers its 2 pixels x 16 velocities from it (8 B per
-//                        trajectory-epoch evaluation, conflict-free LDS.64).  full/empty mbarriers per
-//                        in-flight region; no CTA-wide barrier anywhere in the loop.  (pixel, velocity)
-//                        pairs whose bound reaches min_lh are appended to a global queue.
-//   exact_queue_kernel   the queued pairs get the same device function as the direct kernel (gather from
-//                        the psi/phi stack in L2, register sorting network); results enter the per-pixel
-//                        top-K through a cascade of 64-bit atomicMax on (orderable L', ~vel_idx) keys.
-//   exact_overflow_kernel  pairs of (tile, group, warp) items that did not fit the queue, all evaluated.
-//   finalize_kernel      keys -> the four output arrays.
+//   bound_scale_kernel   once: per-epoch floors, the fixed-point unit and the thresholds thr[k]
+//   bound_plane_kernel   once: the packed planes, row pitch a multiple of 4 so that TMA boxes start 16-byte aligned
+//   bound_phase_kernel   where the time goes.  Persistent, one CTA per SM = 16 consumer warps + 1 producer warp
+//                        group.  A CTA takes (64x32 tile of start pixels, 8 velocity groups) work units from a global
+//                        counter; a group is <= 16 velocities adjacent in displacement space.  For each epoch the
+//                        tile (+) the group's displacement bounding box is staged by TMA (zero fill outside the
+//                        image = the off-chip rule) into a byte ring in shared memory, up to 16 regions ahead, and
+//                        every consumer thread gathers its 4 pixels x 16 velocities from it: 4 B per
+//                        trajectory-epoch evaluation, one conflict-free LDS.32 and one integer add.  full/empty
+//                        mbarriers per in-flight region; no CTA-wide barrier anywhere in the loop.  (pixel,
+//                        velocity) pairs whose bound reaches min_lh are appended to a global queue.
+//   exact_queue_kernel   the queued pairs get the same evaluation as the direct kernel (16-byte gathers from the
+//                        padded S4 canvas, register sorting network); results enter the per-pixel top-K through a
+//                        cascade of 64-bit atomicMax on (orderable L', ~vel_idx) keys.
+//   exact_overflow_kernel  (tile, group, warp) items that did not fit the queue, all pairs evaluated.
+// search_common.cu's finalize_kernel turns the keys into the four output arrays.
 #include <math.h>
 #include <stddef.h>
 #include <stdlib.h>
@@ -133,14 +135,27 @@ struct Queue {
 // a clamped term passes on its own.  Any floors > 0 and any unit > 0 give a CORRECT bound; these make it tight.
 constexpr int SC_BINS = 40, SC_SAMPLES = 16384;
 __global__ void __launch_bounds__(1024)
-bound_scale_kernel(const float2* __restrict__ psiphi, int T, size_t plane, float min_lh,
+bound_scale_kernel(const float2* __restrict__ psiphi, int T, int H, int W, float min_lh,
                                    const __grid_constant__ BoundParams BP, float* __restrict__ scale) {
     __shared__ float ssum[32];
     __shared__ int scnt[32];
     __shared__ int hist[SC_BINS + 1];
     __shared__ float s_mean;
     __shared__ float floors[KBMOD_MAX_T];
-    const size_t n_samp = plane < SC_SAMPLES ? plane : SC_SAMPLES, stride = plane / n_samp;
+    const size_t plane = (size_t)H * W;
+    const size_t n_samp = plane < SC_SAMPLES ? plane : SC_SAMPLES;
+    // the stride is made coprime with the row length, so that the samples spread over every column and row instead
+    // of landing in a handful of columns (a bad column or a masked disc would bias the floors)
+    size_t stride = plane / n_samp;
+    if (stride > 1) {
+        stride |= 1;
+        for (;;) {
+            size_t a = stride, b = (size_t)W;
+            while (b) { const size_t r = a % b; a = b; b = r; }
+            if (a == 1) break;
+            stride -= 2;
+        }
+    }
     for (int t = 0; t < T; ++t) {
         const float2* pl = psiphi + (size_t)t * plane;
         float sum = 0.0f;
@@ -249,11 +264,6 @@ __global__ void bound_plane_kernel(const float2* __restrict__ psiphi, unsigned i
     B[i] = o;
 }
 
-__device__ __forceinline__ unsigned int orderable(float f) {
-    const unsigned int u = __float_as_uint(f);
-    return (u & 0x80000000u) ? ~u : (u | 0x80000000u);
-}
-
 // insert into a descending list of K keys shared by all CTAs (empty = 0): each slot ends up
 // holding the maximum of everything that reached it, so the list is the top-K of all insertions.
 __device__ __forceinline__ void topk_insert(unsigned long long* keys, int K, unsigned long long key) {
@@ -283,8 +293,8 @@ __device__ __forceinline__ void tile_origin(int tile_lin, int tiles_x, int tiles
 // ---------------------------------------------------------------------------------------------
 // phase 1: bounds from shared-memory tiles; survivors -> queue
 __global__ void __launch_bounds__(PR_THREADS, 1)
-bound_phase_kernel(const __grid_constant__ TensorMaps maps, int T, int H, int W, int tile_begin, int tile_end,
-                   int g_begin, int g_end,
+bound_phase_kernel(const __grid_constant__ TensorMaps maps, int T, int row_begin, int row_end, int W, int tile_begin,
+                   int tile_end, int g_begin, int g_end,
                    const __grid_constant__ PrunedTables tb, const __grid_constant__ BoundParams BP, int min_obs,
                    const float* __restrict__ scale, const __grid_constant__ Queue Qu) {
     extern __shared__ __align__(1024) unsigned char smem[];
@@ -311,7 +321,8 @@ bound_phase_kernel(const __grid_constant__ TensorMaps maps, int T, int H, int W,
     }
     __syncthreads();
 
-    const int tiles_x = (W + PR_TW - 1) / PR_TW, tiles_y = (H + PR_TH - 1) / PR_TH;
+    // tiles cover the band of start rows [row_begin, row_end): tile row r starts at image row row_begin + r * PR_TH
+    const int tiles_x = (W + PR_TW - 1) / PR_TW, tiles_y = (row_end - row_begin + PR_TH - 1) / PR_TH;
     const int ng = tb.n_groups;
     // work units: (tile of the batch) x (PR_SUB consecutive groups of the chunk), tile-major
     const int n_sub = (g_end - g_begin + PR_SUB - 1) / PR_SUB;
@@ -338,6 +349,7 @@ bound_phase_kernel(const __grid_constant__ TensorMaps maps, int T, int H, int W,
             const int g_lo = g_begin + (int)(u % (unsigned int)n_sub) * PR_SUB, g_hi = min(g_end, g_lo + PR_SUB);
             int tile_x0, tile_y0, txi, tyi;
             tile_origin(tile_lin, tiles_x, tiles_y, tile_x0, tile_y0, txi, tyi);
+            tile_y0 += row_begin;
             // the ring chain of the tables restarts at offset 0 for every unit: drain first
             while (oldest < q) {
                 kb_mbar_wait(&empty[oldest & (PR_NB - 1)], (oldest / PR_NB) & 1);
@@ -447,6 +459,7 @@ bound_phase_kernel(const __grid_constant__ TensorMaps maps, int T, int H, int W,
         const int g_lo = g_begin + (int)(u % (unsigned int)n_sub) * PR_SUB, g_hi = min(g_end, g_lo + PR_SUB);
         int tile_x0, tile_y0, txi, tyi;
         tile_origin(tile_lin, tiles_x, tiles_y, tile_x0, tile_y0, txi, tyi);
+        tile_y0 += row_begin;
         const int px0 = tile_x0 + lane, py0 = tile_y0 + warp;  // this thread's pixels: (px0 + 32 h, py0 + 16 v)
 
         for (int g = g_lo; g < g_hi; ++g) {
@@ -556,7 +569,7 @@ bound_phase_kernel(const __grid_constant__ TensorMaps maps, int T, int H, int W,
             const float* thr = scale + SC_THR;
 #pragma unroll
             for (int h = 0; h < PR_PIX; ++h) {
-                const bool in_img = (px0 + 32 * (h & 1)) < W && (py0 + 16 * (h >> 1)) < H;
+                const bool in_img = (px0 + 32 * (h & 1)) < W && (py0 + 16 * (h >> 1)) < row_end;
                 m[h] = 0u;
 #pragma unroll
                 for (int j = 0; j < PR_G; ++j) {
@@ -612,40 +625,35 @@ bound_phase_kernel(const __grid_constant__ TensorMaps maps, int T, int H, int W,
 
 // ---------------------------------------------------------------------------------------------
 // phase 2: exact evaluation (steps 1-3 of kbmod_search) of one (pixel, velocity) pair + top-K insertion
+struct ExactArgs {
+    const float4* S4;
+    S4Geom G;
+    const int* off;      // [n_vel][kb_tp4(TP)]
+    int W, row_begin, row_end;
+    unsigned long long* keys;  // [row_end - row_begin][W][K]
+};
+
 template <int TP>
-__device__ __forceinline__ void eval_pair(const float2* __restrict__ psiphi, int H, int W,
-                                          const DispEntry* __restrict__ tab, const DevParams& P, int x0, int y0, int v,
-                                          float* scratch, int stride, unsigned long long* __restrict__ keys) {
-    const DispEntry* row = tab + (size_t)v * TP;
-    const int pixlin = y0 * W + x0;
-    float psi[TP], phi[TP];
-#pragma unroll
-    for (int t = 0; t < TP; ++t) {
-        const DispEntry d = row[t];
-        const int x = x0 + d.dx, y = y0 + d.dy;
-        float2 s = make_float2(0.0f, 0.0f);
-        if ((unsigned)x < (unsigned)W && (unsigned)y < (unsigned)H) s = __ldg(psiphi + (pixlin + d.off));
-        const bool ok = s.y > 0.0f;
-        psi[t] = ok ? s.x : 0.0f;
-        phi[t] = ok ? s.y : 0.0f;
-    }
-    float lh, flux;
-    unsigned long long kept;
-    const int nk = kb_score_lightcurve<TP>(psi, phi, P, scratch, stride, lh, flux, kept);
-    if (nk > 0 && lh >= P.min_lh) {
-        const unsigned long long key =
-            ((unsigned long long)orderable(lh) << 32) | (unsigned long long)(0xFFFFFFFFu - (unsigned)v);
-        topk_insert(keys + (size_t)pixlin * P.K, P.K, key);
+__device__ __forceinline__ void eval_pair(const ExactArgs& A, const DevParams& P, int x0, int y0, int v, float* scratch,
+                                          int stride) {
+    const unsigned int base = (unsigned int)(y0 + A.G.pyn) * (unsigned int)A.G.Wp + (unsigned int)(x0 + A.G.pxn);
+    float psi[TP], phi[TP], f[TP], sp, sf;
+    int n;
+    kb_gather_s4<TP>(A.S4, base, reinterpret_cast<const int4*>(A.off + (size_t)v * kb_tp4(TP)), psi, phi, f, n);
+    const int nk = kb_score_s4<TP>(psi, phi, f, n, P, scratch, stride, sp, sf);
+    if (nk > 0) {
+        const float lh = kb_lh_of(sp, sf);
+        if (lh >= P.min_lh) topk_insert(A.keys + ((size_t)(y0 - A.row_begin) * A.W + x0) * P.K, P.K, kb_topk_key(lh, v));
     }
 }
 
 constexpr int EX_THREADS = 256;
+constexpr int EX_CTAS_PER_SM = 4;
 
 template <int TP>
 __global__ void __launch_bounds__(EX_THREADS)
-exact_queue_kernel(const float2* __restrict__ psiphi, int H, int W, const DispEntry* __restrict__ tab,
-                   const __grid_constant__ DevParams P, const __grid_constant__ Queue Qu,
-                   unsigned long long* __restrict__ keys, unsigned long long* __restrict__ stats) {
+exact_queue_kernel(const __grid_constant__ ExactArgs A, const __grid_constant__ DevParams P,
+                   const __grid_constant__ Queue Qu, unsigned long long* __restrict__ stats) {
     extern __shared__ float scratch_all[];  // [TP][EX_THREADS]
     const unsigned long long cnt = *Qu.count;
     const unsigned long long n = cnt < Qu.cap ? cnt : Qu.cap;
@@ -664,8 +672,8 @@ exact_queue_kernel(const float2* __restrict__ psiphi, int H, int W, const DispEn
         const unsigned long long i_next = base + stride + (threadIdx.x & 31u);
         e_next = (i_next < n) ? __ldg(Qu.entries + i_next) : hole;
         if (e.y != 0xFFFFFFFFu) {
-            const int y0 = (int)(e.x / (unsigned)W), x0 = (int)(e.x - (unsigned)y0 * (unsigned)W);
-            eval_pair<TP>(psiphi, H, W, tab, P, x0, y0, (int)e.y, scratch_all + threadIdx.x, EX_THREADS, keys);
+            const int y0 = (int)(e.x / (unsigned)A.W), x0 = (int)(e.x - (unsigned)y0 * (unsigned)A.W);
+            eval_pair<TP>(A, P, x0, y0, (int)e.y, scratch_all + threadIdx.x, EX_THREADS);
             ++done;
         }
         __syncwarp();
@@ -678,15 +686,15 @@ exact_queue_kernel(const float2* __restrict__ psiphi, int H, int W, const DispEn
 // items that did not fit the queue: every pair of the (tile, group, warp) item is evaluated
 template <int TP>
 __global__ void __launch_bounds__(EX_THREADS)
-exact_overflow_kernel(const float2* __restrict__ psiphi, int H, int W, const DispEntry* __restrict__ tab,
-                      const __grid_constant__ DevParams P, const unsigned int* __restrict__ overflow, size_t n_words,
-                      const int32_t* __restrict__ gvel, int ng, unsigned long long* __restrict__ keys,
+exact_overflow_kernel(const __grid_constant__ ExactArgs A, const __grid_constant__ DevParams P,
+                      const unsigned int* __restrict__ overflow, size_t n_words, const int32_t* __restrict__ gvel, int ng,
                       unsigned long long* __restrict__ stats) {
     extern __shared__ float scratch_all[];
     const int lane = threadIdx.x & 31;
     const size_t warp_global = ((size_t)blockIdx.x * EX_THREADS + threadIdx.x) >> 5;
     const size_t n_warps = ((size_t)gridDim.x * EX_THREADS) >> 5;
-    const int tiles_x = (W + PR_TW - 1) / PR_TW, tiles_y = (H + PR_TH - 1) / PR_TH;
+    const int W = A.W;
+    const int tiles_x = (W + PR_TW - 1) / PR_TW, tiles_y = (A.row_end - A.row_begin + PR_TH - 1) / PR_TH;
     unsigned long long done = 0;
     for (size_t w = warp_global; w < n_words; w += n_warps) {
         unsigned int bits = __ldg(overflow + w);
@@ -700,11 +708,11 @@ exact_overflow_kernel(const float2* __restrict__ psiphi, int H, int W, const Dis
             int tile_x0, tile_y0;
             tile_origin(tile_lin, tiles_x, tiles_y, tile_x0, tile_y0);
             for (int h = 0; h < PR_PIX; ++h) {
-                const int x0 = tile_x0 + lane + 32 * (h & 1), y0 = tile_y0 + row + 16 * (h >> 1);
+                const int x0 = tile_x0 + lane + 32 * (h & 1), y0 = A.row_begin + tile_y0 + row + 16 * (h >> 1);
                 for (int j = 0; j < PR_G; ++j) {
                     const int v = __ldg(gvel + (size_t)g * PR_G + j);
-                    if (v >= 0 && x0 < W && y0 < H) {
-                        eval_pair<TP>(psiphi, H, W, tab, P, x0, y0, v, scratch_all + threadIdx.x, EX_THREADS, keys);
+                    if (v >= 0 && x0 < W && y0 < A.row_end) {
+                        eval_pair<TP>(A, P, x0, y0, v, scratch_all + threadIdx.x, EX_THREADS);
                         ++done;
                     }
                     __syncwarp();  // keep the warp converged (see exact_queue_kernel)
@@ -714,48 +722,6 @@ exact_overflow_kernel(const float2* __restrict__ psiphi, int H, int W, const Dis
     }
     for (int d = 16; d > 0; d >>= 1) done += __shfl_down_sync(0xFFFFFFFFu, done, d);
     if (lane == 0 && done) atomicAdd(stats, done);
-}
-
-// ---------------------------------------------------------------------------------------------
-// keys -> output arrays.  One thread per (pixel, slot); a filled slot is re-evaluated to get flux
-// and n_obs (the key carries L' and the velocity index only).
-constexpr int FIN_THREADS = 128;
-
-template <int TP>
-__global__ void __launch_bounds__(FIN_THREADS)
-finalize_kernel(const unsigned long long* __restrict__ keys, const float2* __restrict__ psiphi, int H, int W,
-                const DispEntry* __restrict__ tab, const __grid_constant__ DevParams P, float* __restrict__ out_lh,
-                float* __restrict__ out_flux, int32_t* __restrict__ out_vel, int32_t* __restrict__ out_nobs) {
-    extern __shared__ float scratch_all[];
-    const size_t i = (size_t)blockIdx.x * FIN_THREADS + threadIdx.x;
-    const size_t total = (size_t)H * W * P.K;
-    if (i >= total) return;
-    const unsigned long long key = keys[i];
-    float lh = -CUDART_INF_F, flux = 0.0f;
-    int vel = -1, nobs = 0;
-    if (key != 0ull) {
-        vel = (int)(0xFFFFFFFFu - (unsigned)(key & 0xFFFFFFFFull));
-        const int pixlin = (int)(i / P.K);
-        const int y0 = pixlin / W, x0 = pixlin - y0 * W;
-        const DispEntry* row = tab + (size_t)vel * TP;
-        float psi[TP], phi[TP];
-#pragma unroll
-        for (int t = 0; t < TP; ++t) {
-            const DispEntry d = row[t];
-            const int x = x0 + d.dx, y = y0 + d.dy;
-            float2 s = make_float2(0.0f, 0.0f);
-            if ((unsigned)x < (unsigned)W && (unsigned)y < (unsigned)H) s = __ldg(psiphi + (pixlin + d.off));
-            const bool ok = s.y > 0.0f;
-            psi[t] = ok ? s.x : 0.0f;
-            phi[t] = ok ? s.y : 0.0f;
-        }
-        unsigned long long kept;
-        nobs = kb_score_lightcurve<TP>(psi, phi, P, scratch_all + threadIdx.x, FIN_THREADS, lh, flux, kept);
-    }
-    out_lh[i] = lh;
-    out_flux[i] = flux;
-    out_vel[i] = vel;
-    out_nobs[i] = nobs;
 }
 
 }  // namespace
@@ -839,16 +805,6 @@ struct Planner {
     }
 };
 
-struct PlanCache {
-    bool valid = false;
-    int T = 0, H = 0, W = 0, n_vel = 0, ng = 0;
-    double staged = 0.0, evals = 0.0;
-    std::vector<int32_t> kdx, kdy, gvel;
-    std::vector<unsigned char> gtbl;
-    std::vector<unsigned long long> maskx, masky;
-    std::vector<uint32_t> gfoot;
-};
-
 int ring_bytes_for(int T) { return ((PR_SMEM_MAX - PR_SMEM_MISC - PR_NTBL * tbl_bytes(T)) / 1024) * 1024; }
 size_t max_groups(int n_vel) {
     const size_t full = ((size_t)n_vel + PR_G - 1) / PR_G;
@@ -863,26 +819,20 @@ size_t queue_cap(int n_vel) {
     const double want = 1100.0 * PR_TW * PR_TH * (double)n_vel / 32.0;
     return (size_t)std::min(268435456.0, std::max(1048576.0, want));
 }
-size_t n_tiles_of(int H, int W) { return (size_t)((W + PR_TW - 1) / PR_TW) * ((H + PR_TH - 1) / PR_TH); }
+size_t n_tiles_of(int n_rows, int W) { return (size_t)((W + PR_TW - 1) / PR_TW) * ((n_rows + PR_TH - 1) / PR_TH); }
 size_t al256(size_t x) { return (x + 255) & ~(size_t)255; }
 
-struct WsLayout {
-    size_t gvel, gtbl, maskx, masky, gfoot, B, keys, qentries, qcount, overflow, total, overflow_words;
+struct ScratchLayout {
+    size_t B, qentries, qcount, overflow, total, overflow_words;
 };
-WsLayout ws_layout(int T, int H, int W, int n_vel, int K) {
-    WsLayout L;
+ScratchLayout scratch_layout(int T, int H, int W, int n_rows, int n_vel) {
+    ScratchLayout L;
     const size_t ngm = max_groups(n_vel), Wp = ((size_t)W + 3) & ~(size_t)3;
     size_t o = 0;
-    L.gvel = o;     o += al256(ngm * PR_G * 4);
-    L.gtbl = o;     o += al256(ngm * tbl_bytes(T));
-    L.maskx = o;    o += al256(ngm * (size_t)((W + PR_TW - 1) / PR_TW) * 8);
-    L.masky = o;    o += al256(ngm * (size_t)((H + PR_TH - 1) / PR_TH) * 8);
-    L.gfoot = o;    o += al256(ngm * 4);
     L.B = o;        o += al256((size_t)T * H * Wp * 4);
-    L.keys = o;     o += al256((size_t)H * W * K * 8);
     L.qentries = o; o += al256(queue_cap(n_vel) * 8);
     L.qcount = o;   o += 256 + al256(SC_FLOATS * sizeof(float));  // queue counter, then the scale table
-    L.overflow_words = (n_tiles_of(H, W) * ngm * (PR_CONSUMERS / 32) + 31) / 32;
+    L.overflow_words = (n_tiles_of(n_rows, W) * ngm * (PR_CONSUMERS / 32) + 31) / 32;
     L.overflow = o; o += al256(L.overflow_words * 4);
     L.total = o;
     return L;
@@ -890,18 +840,140 @@ WsLayout ws_layout(int T, int H, int W, int n_vel, int K) {
 
 }  // namespace
 
-size_t kb_pruned_workspace_bytes(int T, int H, int W, int n_vel, int K) { return ws_layout(T, H, W, n_vel, K).total; }
+size_t kb_pruned_scratch_bytes(int T, int H, int W, int n_rows, int n_vel) {
+    return scratch_layout(T, H, W, n_rows, n_vel).total;
+}
 
-// m(n): a lower bound on the number of epochs the sigma-G filter keeps out of n valid ones, and the
-// thresholds of the bound test in fixed-point units
+// ---------------------------------------------------------------------------------------------
+// the host plan: velocity groups, staging geometry of every (group, epoch), ring chain, on-image masks
+int kb_pruned_plan_build(int T, int H, int W, int row_begin, int row_end, const int32_t* h_dx, const int32_t* h_dy,
+                         int n_vel, PrunedPlan* out) {
+    PrunedPlan& PC = *out;
+    PC = PrunedPlan();
+    const int TBL = tbl_bytes(T);
+    // displacements as the staging sees them: anything beyond every possible image size is off-image for all start
+    // pixels, wherever exactly it is; clamping keeps the geometry inside int32 / TMA coordinates
+    std::vector<int32_t> cdx((size_t)n_vel * T), cdy((size_t)n_vel * T);
+    for (size_t i = 0; i < cdx.size(); ++i) {
+        cdx[i] = std::max(-40000, std::min(40000, h_dx[i]));
+        cdy[i] = std::max(-40000, std::min(40000, h_dy[i]));
+    }
+    const int n_rows = row_end - row_begin;
+    const int tiles_x = (W + PR_TW - 1) / PR_TW, tiles_y = (n_rows + PR_TH - 1) / PR_TH;
+    Planner pl;
+    pl.T = T; pl.n_vel = n_vel; pl.ring_bytes = ring_bytes_for(T);
+    pl.max_region = (pl.ring_bytes / 2 / 1024) * 1024;
+    pl.dx = cdx.data(); pl.dy = cdy.data();
+    int t_far = 0;
+    {   // epoch with the largest displacement spread
+        long long best = -1;
+        for (int t = 0; t < T; ++t) {
+            long long s = 0;
+            for (int v = 0; v < n_vel; v += std::max(1, n_vel / 64)) s += llabs((long long)cdx[(size_t)v * T + t]) + llabs((long long)cdy[(size_t)v * T + t]);
+            if (s > best) { best = s; t_far = t; }
+        }
+    }
+    pl.idx.resize(n_vel); pl.px.resize(n_vel); pl.py.resize(n_vel);
+    for (int v = 0; v < n_vel; ++v) {
+        pl.idx[v] = v;
+        pl.px[v] = cdx[(size_t)v * T + t_far];
+        pl.py[v] = cdy[(size_t)v * T + t_far];
+    }
+    if (n_vel > 0) pl.split(0, n_vel);
+    const int ng = (int)pl.leaves.size();
+    // tables: gvel, per-group blocks {offs[T][G], ge[T]}, ring chain
+    std::vector<int32_t>& gvel = PC.gvel;
+    std::vector<unsigned char>& gtbl = PC.gtbl;
+    gvel.assign((size_t)ng * PR_G, -1);
+    gtbl.assign((size_t)ng * TBL, 0);
+    double staged = 0.0, evals = 0.0;
+    uint32_t ph = 0;
+    for (int g = 0; g < ng; ++g) {
+        if (g % PR_SUB == 0) ph = 0;  // every work unit starts its ring chain at offset 0
+        const int lo = pl.leaves[g].first, cnt = pl.leaves[g].second - pl.leaves[g].first;
+        for (int j = 0; j < cnt; ++j) gvel[(size_t)g * PR_G + j] = pl.idx[lo + j];
+        int32_t* offs = reinterpret_cast<int32_t*>(gtbl.data() + (size_t)g * TBL);
+        GroupEpoch* ge = reinterpret_cast<GroupEpoch*>(gtbl.data() + (size_t)g * TBL + (size_t)T * PR_G * 4);
+        for (int t = 0; t < T; ++t) {
+            GroupEpoch e;
+            memset(&e, 0, sizeof(e));
+            int x0, y0;
+            const long long bytes = pl.region(lo, lo + cnt, t, &e, &x0, &y0);
+            KB_REQUIRE(bytes > 0 && bytes <= pl.max_region, KBMOD_ERR_UNSUPPORTED, "planner: region of %lld bytes", bytes);
+            const int pitch = PR_TW + 16 * (int)(e.pitch_k & 0xFF);
+            for (int j = 0; j < cnt; ++j) {
+                const int v = pl.idx[lo + j];
+                offs[t * PR_G + j] = ((cdy[(size_t)v * T + t] - y0) * pitch + (cdx[(size_t)v * T + t] - x0)) * (int)sizeof(unsigned int);
+            }
+            uint32_t pad = 0;
+            if (ph + (uint32_t)bytes > (uint32_t)pl.ring_bytes) { pad = (uint32_t)pl.ring_bytes - ph; ph = 0; }
+            e.smem_off = ph;
+            e.footprint = (uint32_t)bytes + pad;
+            e.vmask = cnt >= 32 ? 0xFFFFFFFFu : ((1u << cnt) - 1u);
+            bool same = true;
+            for (int j = 1; j < cnt; ++j) same = same && offs[t * PR_G + j] == offs[t * PR_G];
+            if (same) e.pitch_k |= 0x100;
+            ph += (uint32_t)bytes;
+            ge[t] = e;
+            staged += (double)bytes;
+        }
+        evals += (double)PR_TW * PR_TH * cnt * T;
+    }
+    // on-image masks: region t of group g touches the image iff the tile column AND the tile row allow it
+    // (tile row r of the band starts at image row row_begin + r * PR_TH)
+    std::vector<unsigned long long>&maskx = PC.maskx, &masky = PC.masky;
+    std::vector<uint32_t>& gfoot = PC.gfoot;
+    maskx.assign((size_t)ng * tiles_x, 0ull);
+    masky.assign((size_t)ng * tiles_y, 0ull);
+    gfoot.assign((size_t)ng, 0u);
+    double on = 0.0, all = 0.0;
+    for (int g = 0; g < ng; ++g) {
+        const GroupEpoch* ge = reinterpret_cast<const GroupEpoch*>(gtbl.data() + (size_t)g * TBL + (size_t)T * PR_G * 4);
+        unsigned long long foot = 0;
+        for (int t = 0; t < T; ++t) {
+            const long long pitch = PR_TW + 16 * (long long)(ge[t].pitch_k & 0xFF), rows = (long long)ge[t].n_box * PR_RB;
+            for (int c = 0; c < tiles_x; ++c) {
+                const long long x0 = (long long)c * PR_TW + ge[t].ox;
+                if (x0 < W && x0 + pitch > 0) maskx[(size_t)g * tiles_x + c] |= 1ull << t;
+            }
+            for (int r = 0; r < tiles_y; ++r) {
+                const long long y0 = (long long)row_begin + (long long)r * PR_TH + ge[t].oy;
+                if (y0 < H && y0 + rows > 0) masky[(size_t)g * tiles_y + r] |= 1ull << t;
+            }
+            foot += ge[t].footprint;
+        }
+        gfoot[g] = (uint32_t)std::min<unsigned long long>(foot, 0xFFFFFFFFull);  // > ring / 2 is all that matters
+        for (int c = 0; c < tiles_x; ++c)
+            for (int r = 0; r < tiles_y; ++r) {
+                on += (double)__builtin_popcountll(maskx[(size_t)g * tiles_x + c] & masky[(size_t)g * tiles_y + r]);
+                all += (double)T;
+            }
+    }
+    PC.T = T; PC.H = H; PC.W = W; PC.row_begin = row_begin; PC.row_end = row_end; PC.n_vel = n_vel;
+    PC.ng = ng; PC.staged = staged; PC.evals = evals;
+    PC.off_image = all > 0 ? 1.0 - on / all : 0.0;
+    PC.ring_bytes = ring_bytes_for(T);
+    PC.tiles_x = tiles_x; PC.tiles_y = tiles_y;
+    PC.too_scattered = (size_t)ng > max_groups(n_vel) ? 1 : 0;
+    return KBMOD_OK;
+}
+
+// m(n): a lower bound on the number of epochs the sigma-G filter keeps out of n valid ones.  The clip window is
+// [P50 - w, P50 + w], w = n_sigma C (P_hi - P_lo); with n_sigma C >= 1 (1e-3 of margin absorbs the float32
+// roundings) and P_lo <= P50 <= P_hi it contains [P_lo, P_hi], hence every sample whose sorted index lies in
+// [k_lo (+1 if P_lo is interpolated above s[k_lo]), k_hi].  Nearest rank: k = the rank itself, no interpolation.
 static bool bound_min_kept(const kbmod_search_params* p, const DevParams& P, int T, BoundParams* bp) {
     const float prod = p->n_sigma * p->sigmag_coeff;
     for (int n = 0; n <= KBMOD_MAX_T; ++n) {
         int m = 1;
         if (n >= 1 && n <= T) {
             if (!P.sigmag_enable) m = n;
-            else if (prod >= 1.001f && p->pct_lo <= 50.0f && p->pct_hi >= 50.0f) m = P.rk_hi[n] - P.rk_lo[n] + 1;
-            else if (prod >= 0.0f && p->n_sigma >= 0.0f) m = 1;
+            else if (prod >= 1.001f && p->pct_lo <= 50.0f && p->pct_hi >= 50.0f) {
+                // an interpolation weight within 1e-6 of 1 could round the interpolant onto (or past) s[k+1]: no claim
+                const bool g_ok = P.fr_lo[n] < 1.0f - 1e-6f && P.fr_hi[n] < 1.0f - 1e-6f && P.fr_md[n] < 1.0f - 1e-6f;
+                const int first = P.rk_lo[n] + (P.fr_lo[n] > 0.0f ? 1 : 0);
+                m = g_ok ? std::max(1, (int)P.rk_hi[n] - first + 1) : 1;
+            } else if (prod >= 0.0f && p->n_sigma >= 0.0f) m = 1;
             else return false;
         }
         bp->mkept[n] = (unsigned char)(n == 0 ? 0 : m);
@@ -912,172 +984,41 @@ static bool bound_min_kept(const kbmod_search_params* p, const DevParams& P, int
     return true;
 }
 
-int kb_launch_search_pruned(const float* d_psiphi, int T, int TPv, int H, int W, const DispEntry* d_tab,
-                            const int32_t* h_dx, const int32_t* h_dy, int n_vel, const kbmod_search_params* p,
-                            const DevParams& P, float* d_lh, float* d_flux, int32_t* d_vel, int32_t* d_nobs,
-                            void* d_ws, size_t ws_bytes, unsigned long long* d_stats, cudaStream_t st, int plan_only,
-                            double* plan_stats, int* n_launches) {
+int kb_launch_search_pruned(const float* d_psiphi, const PrunedPlan& plan, const PrunedTablesDev& tbd, int TPv,
+                            const void* d_S4, const S4Geom& G, const int* d_off, const kbmod_search_params* p,
+                            const DevParams& P, unsigned long long* d_keys, void* d_scratch, size_t scratch_bytes,
+                            unsigned long long* d_stats, cudaStream_t st, int* n_launches) {
     BoundParams bp;
-    if (!bound_min_kept(p, P, T, &bp)) {
+    if (!bound_min_kept(p, P, plan.T, &bp)) {
         kb_set_error("pruned search needs n_sigma >= 0 and n_sigma*coeff >= 0");
         return KBMOD_ERR_UNSUPPORTED;
     }
+    const int T = plan.T, H = plan.H, W = plan.W, n_vel = plan.n_vel, ng = plan.ng;
+    const int row_begin = plan.row_begin, row_end = plan.row_end, n_rows = row_end - row_begin;
     const int TBL = tbl_bytes(T);
-    // ---- displacements as the staging sees them: anything beyond every possible image size is off-image
-    // for all start pixels, wherever exactly it is; clamping keeps the geometry inside int32 / TMA coordinates
-    std::vector<int32_t> cdx((size_t)n_vel * T), cdy((size_t)n_vel * T);
-    for (size_t i = 0; i < cdx.size(); ++i) {
-        cdx[i] = std::max(-40000, std::min(40000, h_dx[i]));
-        cdy[i] = std::max(-40000, std::min(40000, h_dy[i]));
-    }
-    // ---- the plan depends only on the geometry (T, H, W and the displacement table): searching the CCDs of one
-    // pointing group, or the AUTO decision followed by the search itself, reuses it (one entry per host thread)
-    static thread_local PlanCache PC;
-    const bool plan_hit = PC.valid && PC.T == T && PC.H == H && PC.W == W && PC.n_vel == n_vel &&
-                          PC.kdx.size() == cdx.size() && (cdx.empty() || (memcmp(PC.kdx.data(), cdx.data(), cdx.size() * 4) == 0 &&
-                                                                        memcmp(PC.kdy.data(), cdy.data(), cdy.size() * 4) == 0));
-    const int tiles_x = (W + PR_TW - 1) / PR_TW, tiles_y = (H + PR_TH - 1) / PR_TH;
-    const int ring_bytes = ring_bytes_for(T);
-    if (!plan_hit) {
-        PC.valid = false;
-        Planner pl;
-        pl.T = T; pl.n_vel = n_vel; pl.ring_bytes = ring_bytes_for(T);
-        pl.max_region = (pl.ring_bytes / 2 / 1024) * 1024;
-        pl.dx = cdx.data(); pl.dy = cdy.data();
-        int t_far = 0;
-        {   // epoch with the largest displacement spread
-            long long best = -1;
-            for (int t = 0; t < T; ++t) {
-                long long s = 0;
-                for (int v = 0; v < n_vel; v += std::max(1, n_vel / 64)) s += llabs((long long)cdx[(size_t)v * T + t]) + llabs((long long)cdy[(size_t)v * T + t]);
-                if (s > best) { best = s; t_far = t; }
-            }
-        }
-        pl.idx.resize(n_vel); pl.px.resize(n_vel); pl.py.resize(n_vel);
-        for (int v = 0; v < n_vel; ++v) {
-            pl.idx[v] = v;
-            pl.px[v] = cdx[(size_t)v * T + t_far];
-            pl.py[v] = cdy[(size_t)v * T + t_far];
-        }
-        if (n_vel > 0) pl.split(0, n_vel);
-        const int ng = (int)pl.leaves.size();
-        // ---- tables: gvel, per-group blocks {offs[T][G], ge[T]}, ring chain
-        std::vector<int32_t>& gvel = PC.gvel;
-        std::vector<unsigned char>& gtbl = PC.gtbl;
-        gvel.assign((size_t)ng * PR_G, -1);
-        gtbl.assign((size_t)ng * TBL, 0);
-        double staged = 0.0, evals = 0.0;
-        uint32_t ph = 0;
-        for (int g = 0; g < ng; ++g) {
-            if (g % PR_SUB == 0) ph = 0;  // every work unit starts its ring chain at offset 0
-            const int lo = pl.leaves[g].first, cnt = pl.leaves[g].second - pl.leaves[g].first;
-            for (int j = 0; j < cnt; ++j) gvel[(size_t)g * PR_G + j] = pl.idx[lo + j];
-            int32_t* offs = reinterpret_cast<int32_t*>(gtbl.data() + (size_t)g * TBL);
-            GroupEpoch* ge = reinterpret_cast<GroupEpoch*>(gtbl.data() + (size_t)g * TBL + (size_t)T * PR_G * 4);
-            for (int t = 0; t < T; ++t) {
-                GroupEpoch e;
-                memset(&e, 0, sizeof(e));
-                int x0, y0;
-                const long long bytes = pl.region(lo, lo + cnt, t, &e, &x0, &y0);
-                KB_REQUIRE(bytes > 0 && bytes <= pl.max_region, KBMOD_ERR_UNSUPPORTED, "planner: region of %lld bytes", bytes);
-                const int pitch = PR_TW + 16 * (int)(e.pitch_k & 0xFF);
-                for (int j = 0; j < cnt; ++j) {
-                    const int v = pl.idx[lo + j];
-                    offs[t * PR_G + j] = ((cdy[(size_t)v * T + t] - y0) * pitch + (cdx[(size_t)v * T + t] - x0)) * (int)sizeof(unsigned int);
-                }
-                uint32_t pad = 0;
-                if (ph + (uint32_t)bytes > (uint32_t)pl.ring_bytes) { pad = (uint32_t)pl.ring_bytes - ph; ph = 0; }
-                e.smem_off = ph;
-                e.footprint = (uint32_t)bytes + pad;
-                e.vmask = cnt >= 32 ? 0xFFFFFFFFu : ((1u << cnt) - 1u);
-                bool same = true;
-                for (int j = 1; j < cnt; ++j) same = same && offs[t * PR_G + j] == offs[t * PR_G];
-                if (same) e.pitch_k |= 0x100;
-                ph += (uint32_t)bytes;
-                ge[t] = e;
-                staged += (double)bytes;
-            }
-            evals += (double)PR_TW * PR_TH * cnt * T;
-        }
-        // on-image masks: region t of group g touches the image iff the tile column AND the tile row allow it
-        std::vector<unsigned long long>&maskx = PC.maskx, &masky = PC.masky;
-        std::vector<uint32_t>& gfoot = PC.gfoot;
-        maskx.assign((size_t)ng * tiles_x, 0ull);
-        masky.assign((size_t)ng * tiles_y, 0ull);
-        gfoot.assign((size_t)ng, 0u);
-        for (int g = 0; g < ng; ++g) {
-            const GroupEpoch* ge = reinterpret_cast<const GroupEpoch*>(gtbl.data() + (size_t)g * TBL + (size_t)T * PR_G * 4);
-            unsigned long long foot = 0;
-            for (int t = 0; t < T; ++t) {
-                const long long pitch = PR_TW + 16 * (long long)(ge[t].pitch_k & 0xFF), rows = (long long)ge[t].n_box * PR_RB;
-                for (int c = 0; c < tiles_x; ++c) {
-                    const long long x0 = (long long)c * PR_TW + ge[t].ox;
-                    if (x0 < W && x0 + pitch > 0) maskx[(size_t)g * tiles_x + c] |= 1ull << t;
-                }
-                for (int r = 0; r < tiles_y; ++r) {
-                    const long long y0 = (long long)r * PR_TH + ge[t].oy;
-                    if (y0 < H && y0 + rows > 0) masky[(size_t)g * tiles_y + r] |= 1ull << t;
-                }
-                foot += ge[t].footprint;
-            }
-            gfoot[g] = (uint32_t)std::min<unsigned long long>(foot, 0xFFFFFFFFull);  // > ring / 2 is all that matters
-        }
-        PC.T = T; PC.H = H; PC.W = W; PC.n_vel = n_vel;
-        PC.kdx = cdx; PC.kdy = cdy;
-        PC.ng = ng; PC.staged = staged; PC.evals = evals;
-        PC.valid = true;
-    }
-    const int ng = PC.ng;
-    const double staged = PC.staged, evals = PC.evals;
-    const std::vector<int32_t>& gvel = PC.gvel;
-    const std::vector<unsigned char>& gtbl = PC.gtbl;
-    const std::vector<unsigned long long>&maskx = PC.maskx, &masky = PC.masky;
-    const std::vector<uint32_t>& gfoot = PC.gfoot;
     const size_t ngm = max_groups(n_vel);
+    KB_REQUIRE(!plan.too_scattered && (size_t)ng <= ngm, KBMOD_ERR_UNSUPPORTED,
+               "pruned search: %d velocity groups needed, workspace holds %zu (velocities too scattered; use the direct kernel)",
+               ng, ngm);
     // launches cover (a batch of whole waves of tiles) x (a chunk of the groups), sized so that 1/4 of the launch's
     // trajectories fit the survivor queue (what does not fit is evaluated wholesale by the overflow kernel)
-    int n_sm = 148;
-    if (!plan_only) {
-        int dev = 0;
-        KB_CUDA(cudaGetDevice(&dev));
-        KB_CUDA(cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev));
-    }
-    const int n_tiles = (int)n_tiles_of(H, W);
+    int n_sm = 148, dev = 0;
+    KB_CUDA(cudaGetDevice(&dev));
+    KB_CUDA(cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev));
+    const int n_tiles = (int)n_tiles_of(n_rows, W);
     const int grid = std::max(1, std::min(n_sm, n_tiles));
     const double budget = 4.0 * (double)queue_cap(n_vel);
     const double wave_nominal = (double)grid * PR_TW * PR_TH * (double)ng * PR_G;  // one wave, all groups
     const int n_chunks = std::max(1, std::min(std::max(ng, 1), (int)ceil(wave_nominal / budget)));
     const int groups_per_chunk = ((std::max(1, (ng + n_chunks - 1) / n_chunks) + PR_SUB - 1) / PR_SUB) * PR_SUB;
 
-    if (plan_stats) {
-        plan_stats[0] = (size_t)ng > ngm ? 1.0 : 0.0;       // the velocity list is too scattered to group
-        plan_stats[1] = evals > 0 ? staged / evals : 0.0;   // staged bytes per evaluation (before off-image skipping)
-        plan_stats[2] = (double)ng;                         // velocity groups
-        // share of the (tile, group, epoch) region loads that lie off the image and are skipped
-        double on = 0.0, all = 0.0;
-        for (int g = 0; g < ng; ++g)
-            for (int c = 0; c < tiles_x; ++c)
-                for (int r = 0; r < tiles_y; ++r) {
-                    on += (double)__builtin_popcountll(maskx[(size_t)g * tiles_x + c] & masky[(size_t)g * tiles_y + r]);
-                    all += (double)T;
-                }
-        plan_stats[3] = all > 0 ? 1.0 - on / all : 0.0;
-    }
-    if (plan_only) return KBMOD_OK;
-    KB_REQUIRE((size_t)ng <= ngm, KBMOD_ERR_UNSUPPORTED,
-               "pruned search: %d velocity groups needed, workspace holds %zu (velocities too scattered; use the direct kernel)",
-               ng, ngm);
-
-    // ---- workspace carve-up
-    const WsLayout L = ws_layout(T, H, W, n_vel, P.K);
-    KB_REQUIRE(L.total <= ws_bytes, KBMOD_ERR_WORKSPACE, "pruned search workspace: need %zu, have %zu", L.total, ws_bytes);
+    // ---- scratch carve-up
+    const ScratchLayout L = scratch_layout(T, H, W, n_rows, n_vel);
+    KB_REQUIRE(L.total <= scratch_bytes, KBMOD_ERR_WORKSPACE, "pruned search scratch: need %zu, have %zu", L.total, scratch_bytes);
     const size_t Wp = ((size_t)W + 3) & ~(size_t)3;
     KB_REQUIRE((double)T * H * Wp < 2147483648.0, KBMOD_ERR_UNSUPPORTED, "T*H*Wp exceeds 2^31");
-    char* w = (char*)d_ws;
-    int32_t* d_gvel = (int32_t*)(w + L.gvel);
-    unsigned char* d_gtbl = (unsigned char*)(w + L.gtbl);
+    char* w = (char*)d_scratch;
     unsigned int* d_B = (unsigned int*)(w + L.B);
-    unsigned long long* d_keys = (unsigned long long*)(w + L.keys);
     Queue Qu;
     Qu.entries = (uint2*)(w + L.qentries);
     Qu.count = (unsigned long long*)(w + L.qcount);
@@ -1086,14 +1027,7 @@ int kb_launch_search_pruned(const float* d_psiphi, int T, int TPv, int H, int W,
     Qu.cap = queue_cap(n_vel);
     Qu.overflow = (unsigned int*)(w + L.overflow);
 
-    if (ng > 0) {
-        KB_CUDA(cudaMemcpyAsync(d_gvel, gvel.data(), gvel.size() * 4, cudaMemcpyHostToDevice, st));
-        KB_CUDA(cudaMemcpyAsync(d_gtbl, gtbl.data(), gtbl.size(), cudaMemcpyHostToDevice, st));
-        KB_CUDA(cudaMemcpyAsync(w + L.maskx, maskx.data(), maskx.size() * 8, cudaMemcpyHostToDevice, st));
-        KB_CUDA(cudaMemcpyAsync(w + L.masky, masky.data(), masky.size() * 8, cudaMemcpyHostToDevice, st));
-        KB_CUDA(cudaMemcpyAsync(w + L.gfoot, gfoot.data(), gfoot.size() * 4, cudaMemcpyHostToDevice, st));
-    }
-    KB_CUDA(cudaMemsetAsync(d_keys, 0, (size_t)H * W * P.K * 8, st));
+    KB_CUDA(cudaMemsetAsync(d_keys, 0, (size_t)n_rows * W * P.K * 8, st));
     KB_CUDA(cudaMemsetAsync(Qu.overflow, 0, L.overflow_words * 4, st));
 
     // ---- tensor maps over the bound planes: uint32 elements, dims {Wp, H, T}
@@ -1117,7 +1051,7 @@ int kb_launch_search_pruned(const float* d_psiphi, int T, int TPv, int H, int W,
     int launches = 0;
     {
         const size_t n = (size_t)T * H * Wp;
-        bound_scale_kernel<<<1, 1024, 0, st>>>(reinterpret_cast<const float2*>(d_psiphi), T, (size_t)H * W, P.min_lh, bp, d_scale);
+        bound_scale_kernel<<<1, 1024, 0, st>>>(reinterpret_cast<const float2*>(d_psiphi), T, H, W, P.min_lh, bp, d_scale);
         bound_plane_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(reinterpret_cast<const float2*>(d_psiphi), d_B, H, W,
                                                                         (int)Wp, (size_t)T * H, bp.cbits, d_scale);
         KB_CUDA(cudaGetLastError());
@@ -1127,11 +1061,10 @@ int kb_launch_search_pruned(const float* d_psiphi, int T, int TPv, int H, int W,
     long long waves = (long long)(budget / std::max(1.0, wave_nominal / n_chunks));
     waves = std::max<long long>(1, std::min<long long>(PR_WAVES_PER_BATCH, waves));
     const int batch = (int)std::min<long long>((long long)n_tiles, waves * grid);
-    const size_t smem1 = (size_t)ring_bytes + (size_t)PR_NTBL * TBL + PR_SMEM_MISC;
+    const size_t smem1 = (size_t)plan.ring_bytes + (size_t)PR_NTBL * TBL + PR_SMEM_MISC;
     KB_CUDA(cudaFuncSetAttribute(bound_phase_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem1));
-    PrunedTables tb{d_gvel, d_gtbl, (const unsigned long long*)(w + L.maskx), (const unsigned long long*)(w + L.masky),
-                    (const uint32_t*)(w + L.gfoot), ng, ring_bytes};
-    const float2* psiphi2 = reinterpret_cast<const float2*>(d_psiphi);
+    PrunedTables tb{tbd.gvel, tbd.gtbl, tbd.maskx, tbd.masky, tbd.gfoot, ng, plan.ring_bytes};
+    ExactArgs EA{reinterpret_cast<const float4*>(d_S4), G, d_off, W, row_begin, row_end, d_keys};
     KB_DISPATCH_TP(TPv, {
         const size_t smem2 = (size_t)TP * EX_THREADS * sizeof(float);
         KB_CUDA(cudaFuncSetAttribute(exact_queue_kernel<TP>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem2));
@@ -1142,25 +1075,19 @@ int kb_launch_search_pruned(const float* d_psiphi, int T, int TPv, int H, int W,
                 for (int g0 = 0; g0 < ng; g0 += groups_per_chunk) {
                     const int g1 = std::min(ng, g0 + groups_per_chunk);
                     KB_CUDA(cudaMemsetAsync(Qu.count, 0, 2 * sizeof(unsigned long long), st));  // queue and unit counters
-                    bound_phase_kernel<<<std::min(grid, b1 - b0), PR_THREADS, smem1, st>>>(maps, T, H, W, b0, b1, g0, g1, tb, bp,
-                                                                                          P.min_obs, d_scale, Qu);
+                    bound_phase_kernel<<<std::min(grid, b1 - b0), PR_THREADS, smem1, st>>>(maps, T, row_begin, row_end, W, b0, b1,
+                                                                                          g0, g1, tb, bp, P.min_obs, d_scale, Qu);
                     kb_phase_mark(KB_PHASE_BOUND, st);
-                    exact_queue_kernel<TP><<<n_sm * 4, EX_THREADS, smem2, st>>>(psiphi2, H, W, d_tab, P, Qu, d_keys, d_stats);
+                    exact_queue_kernel<TP><<<n_sm * EX_CTAS_PER_SM, EX_THREADS, smem2, st>>>(EA, P, Qu, d_stats);
                     kb_phase_mark(KB_PHASE_EXACT, st);
                     launches += 2;
                 }
             }
-            exact_overflow_kernel<TP><<<n_sm * 4, EX_THREADS, smem2, st>>>(psiphi2, H, W, d_tab, P, Qu.overflow,
-                                                                           L.overflow_words, d_gvel, ng, d_keys, d_stats);
+            exact_overflow_kernel<TP><<<n_sm * EX_CTAS_PER_SM, EX_THREADS, smem2, st>>>(EA, P, Qu.overflow, L.overflow_words,
+                                                                                       tbd.gvel, ng, d_stats);
             kb_phase_mark(KB_PHASE_EXACT, st);
             ++launches;
         }
-        const size_t total = (size_t)H * W * P.K;
-        finalize_kernel<TP><<<(unsigned)((total + FIN_THREADS - 1) / FIN_THREADS), FIN_THREADS,
-                              (size_t)TP * FIN_THREADS * sizeof(float), st>>>(d_keys, psiphi2, H, W, d_tab, P, d_lh, d_flux,
-                                                                             d_vel, d_nobs);
-        kb_phase_mark(KB_PHASE_FINALIZE, st);
-        ++launches;
     });
     KB_CUDA(cudaGetLastError());
     if (n_launches) *n_launches = launches;

@@ -41,16 +41,15 @@ int run_peak(int iters, int grid, unsigned int* sink, cudaStream_t st) {
 
 }  // namespace
 
-extern "C" int kbmod_measure_smem_gbs(int bytes_per_lane, double* h_gbs, void* stream) {
-    KB_REQUIRE(h_gbs, KBMOD_ERR_INVALID_ARG, "NULL argument");
+extern "C" int kbmod_measure_smem_gbs(int bytes_per_lane, void* d_scratch4, double* h_gbs, void* stream) {
+    KB_REQUIRE(h_gbs && d_scratch4, KBMOD_ERR_INVALID_ARG, "NULL argument");
     KB_REQUIRE(bytes_per_lane == 4 || bytes_per_lane == 8 || bytes_per_lane == 16, KBMOD_ERR_INVALID_ARG,
                "bytes_per_lane = %d must be 4, 8 or 16", bytes_per_lane);
     cudaStream_t st = (cudaStream_t)stream;
     int dev = 0, n_sm = 0;
     KB_CUDA(cudaGetDevice(&dev));
     KB_CUDA(cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev));
-    unsigned int* sink = nullptr;
-    KB_CUDA(cudaMalloc(&sink, 4));  // measurement helper only: the search path never allocates
+    unsigned int* sink = (unsigned int*)d_scratch4;  // caller-owned: the library never allocates device memory
     cudaEvent_t e0, e1;
     KB_CUDA(cudaEventCreate(&e0));
     KB_CUDA(cudaEventCreate(&e1));
@@ -70,7 +69,6 @@ extern "C" int kbmod_measure_smem_gbs(int bytes_per_lane, double* h_gbs, void* s
     }
     cudaEventDestroy(e0);
     cudaEventDestroy(e1);
-    cudaFree(sink);
     KB_CUDA(cudaGetLastError());
     *h_gbs = best;
     return KBMOD_OK;

@@ -101,7 +101,8 @@ def compare_topk(O, psiphi, times, vx, vy, p, px, py, gpu, ora):
 def oracle_params(O, sp):
     """SearchParams (binding) -> oracle.Params, field by field."""
     return O.Params(sigmag_enable=sp.sigmag_enable, pct_lo=sp.pct_lo, pct_hi=sp.pct_hi, coeff=sp.sigmag_coeff,
-                    n_sigma=sp.n_sigma, filter_on=sp.filter_on, min_lh=sp.min_lh, min_obs=sp.min_obs, K=sp.K)
+                    n_sigma=sp.n_sigma, filter_on=sp.filter_on, min_lh=sp.min_lh, min_obs=sp.min_obs, K=sp.K,
+                    pct_interp=getattr(sp, "pct_interp", 0))
 
 
 def check_prep(O, stack, g_psiphi, psf=None):

@@ -23,7 +23,9 @@ local_ms = 10.0 + 5.0 * rank                      # rank 1 is the slow one
 ms = bench.max_over_ranks(local_ms, dist, torch.device("cpu"), world)
 T, H, W = st.img.shape
 value = bench.whole_job_value(float(H) * W * len(vx) * T, world, ms)
-print(json.dumps(dict(rank=rank, ms=ms, value=value, checksum=float(np.abs(st.img).sum()))), flush=True)
+# one file per rank: two processes writing to one pipe can interleave their lines
+open(os.path.join({out!r}, "rank%d.json" % rank), "w").write(
+    json.dumps(dict(rank=rank, ms=ms, value=value, checksum=float(np.abs(st.img).sum()))))
 dist.barrier()
 dist.destroy_process_group()
 """
@@ -32,13 +34,13 @@ dist.destroy_process_group()
 def test_two_rank_gloo_replicas(tmp_path):
     s = socket.socket(); s.bind(("127.0.0.1", 0)); port = s.getsockname()[1]; s.close()
     script = tmp_path / "worker.py"
-    script.write_text(WORKER.format(root=ROOT))
+    script.write_text(WORKER.format(root=ROOT, out=str(tmp_path)))
     cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node=2", "--master-addr", "127.0.0.1",
            "--master-port", str(port), str(script)]
     out = subprocess.run(cmd, capture_output=True, text=True, timeout=300, cwd=ROOT)
     assert out.returncode == 0, out.stderr[-2000:]
     import json
-    recs = sorted((json.loads(l) for l in out.stdout.splitlines() if l.startswith("{")), key=lambda r: r["rank"])
+    recs = [json.loads((tmp_path / f"rank{r}.json").read_text()) for r in (0, 1)]
     assert [r["rank"] for r in recs] == [0, 1]
     assert recs[0]["ms"] == recs[1]["ms"] == 15.0                       # max over ranks, on every rank
     evals = 64 * 64 * 256 * 5
