@@ -114,10 +114,22 @@ class ClockSampler:
 
 
 # ----------------------------------------------------------------------------------------- oracle legs
+def cpu_model() -> str:
+    try:
+        for ln in open("/proc/cpuinfo"):
+            if ln.lower().startswith("model name"):
+                return ln.split(":", 1)[1].strip()
+    except OSError:
+        pass
+    return "unknown"
+
+
 class OracleSample:
     """The oracle (as it stands) on a bounded sample of the workload.  O1 runs once on a crop tall
     enough that most displaced epochs stay on it (real values: movers, masks, artefacts); what is
-    timed is the search (O2-O6) on random start pixels of that crop, where the time goes."""
+    timed is the search (O2-O6) on random start pixels of that crop, where the time goes.  (BASELINE.md planned 64
+    full rows; random pixels of a crop sample the same trajectories without generating the O1 output of the whole
+    stack in double precision, 3.5 GB.)"""
 
     def __init__(self, st, vx, vy, pd, min_lh):
         from oracle import oracle as O
@@ -132,6 +144,7 @@ class OracleSample:
         self.p = O.Params(K=pd["K"], min_obs=pd["min_obs"], min_lh=min_lh)
         self.rng = np.random.default_rng(123)
         self.rate = None
+        self.all_threads = O.num_threads()
 
     def _run(self, n):
         px = self.rng.integers(0, self.cw, n).astype(np.int32)
@@ -152,6 +165,16 @@ class OracleSample:
                 f"velocities x {self.T} epochs = {evals:.3g} evals in {dt:.1f} s (O1 on the crop, {self.t_prep:.1f} s, "
                 f"not counted)")
         return evals / dt, self.O.num_threads(), desc, dt
+
+    def one_core(self, target_s=4.0):
+        """The same on ONE thread ('all cores and 1 core')."""
+        self.O.set_num_threads(1)
+        try:
+            n = int(max(64, (self.rate or 1000.0) / max(1, self.all_threads) * target_s))
+            dt = self._run(n)
+            return float(n) * len(self.vx) * self.T / dt
+        finally:
+            self.O.set_num_threads(self.all_threads)
 
 
 def run_reference(args):
@@ -174,7 +197,7 @@ def run_reference(args):
                 warmup=args.warmup, ms_per_step=1e3 * float(np.mean(times_s)), higher_is_better=True, scaling="weak",
                 vs_baseline=None, dtype="f64", data="synthetic",
                 config=dict(workload=desc, min_lh=args.min_lh, sigma_g="on", note="each step = a bounded sample"),
-                cpu_baseline=dict(value=value, unit=UNIT, cores=cores, kind="oracle", sample=sample),
+                cpu_baseline=dict(value=value, unit=UNIT, cores=cores, kind="oracle", sample=sample, cpu=cpu_model()),
                 e2e=dict(value=value, unit=UNIT, h2d_bytes_per_step=0, d2h_bytes_per_step=0), gpu_launches=0,
                 peaks_source=peaks["source"])
     print(json.dumps(line), flush=True)
@@ -192,10 +215,13 @@ def run_reference(args):
 #                    SURVEY 8(d) counted 8 B per evaluation (psi and phi as float32): reported beside it.
 # dram__bytes_read.sum + dram__bytes_write.sum per step of the dominant kernel from the committed ncu --set full
 # capture (profiles/); None = not captured for this kernel
-TRAFFIC = {"bound_phase_kernel": 16.4e9, "search_direct_kernel": None}  # bytes per step (84 launches): profiles/r1_launches_final.md
+TRAFFIC = {"bound_phase_kernel": 16.4e9, "search_direct_kernel": None}  # bytes per step: see profiles/ (capture commit named there)
 CE_COUNT = {4: 5, 5: 9, 8: 19, 10: 32, 12: 42, 16: 63, 20: 103, 24: 132, 26: 147, 28: 162, 32: 191, 40: 305,
             48: 384, 50: 403, 56: 464, 64: 543}
 N_SM = 148
+# executed warp-instructions per warp-trajectory of search_direct_kernel<TP> (ncu smsp__inst_executed / (trajectories / 32),
+# profiles/r2_search_direct_kernel_full.md); other TP: scaled by the compare-exchange count
+DIRECT_WARP_INSTR_PER_TRAJ = {26: 640.0}
 
 
 def run_ours(args):
@@ -242,7 +268,7 @@ def run_ours(args):
         e[1].record()
         kb.kbmod_search(psiphi, st.times, vx, vy, sp, out=out, workspace=ws)
         e[2].record()
-        kb.kbmod_coadd_stamps(img, mask, st.times, cx0, cy0, cvx, cvy, 10)
+        kb.kbmod_coadd_stamps_filtered(img, mask, st.times, cx0, cy0, cvx, cvy, 10)  # (a6) + the moment filter (L141)
         e[3].record()
         if record is not None:
             record.append(e)
@@ -274,9 +300,102 @@ def run_ours(args):
         seg["coadd"].append(e[2].elapsed_time(e[3]))
     stats = kb.kbmod_search_stats(ws)  # [evaluated, nominal, launches, algo]
     smem_gbs = {b: kb.kbmod_measure_smem_gbs(b) for b in (4, 16)}  # after the timed region
-    return dict(torch=torch, dist=dist, kb=kb, rank=rank, world=world, dev=dev, st=st, vx=vx, vy=vy, pd=pd, sp=sp,
-                desc=desc, evals=evals, total_ms=total_ms, seg=seg, stats=stats, clocks=clocks, peaks=peaks, phases=phases,
-                n_cand=n_cand, out=out, smem_gbs=smem_gbs)
+    plan_info = kb.Plan(T, H, W, st.times, vx, vy, sp).info()           # host-only: what the planner staged / skipped
+    R = dict(torch=torch, dist=dist, kb=kb, rank=rank, world=world, dev=dev, st=st, vx=vx, vy=vy, pd=pd, sp=sp,
+             desc=desc, evals=evals, total_ms=total_ms, seg=seg, stats=stats, clocks=clocks, peaks=peaks, phases=phases,
+             n_cand=n_cand, out=out, smem_gbs=smem_gbs, plan_info=plan_info, psiphi=psiphi, ws=ws, extras={})
+    # ---- more timed records on the same box, after the headline region (rank 0 of a 1-GPU run, default workload)
+    if rank == 0 and world == 1 and args.workload == "c3" and not args.no_extras and args.algo == "auto" and args.min_lh == 10.0:
+        R["extras"]["mode_b"] = time_search(R, "configs[2], mode (B): min_lh = -inf, every trajectory filtered (SURVEY 8d)", st, psiphi,
+                                            vx, vy, dict(pd), -math.inf, steps=2, warmup=1)
+        pvx, pvy = synth.paper_grid()
+        R["extras"]["paper_grid"] = time_search(R, "configs[2] stack x the paper's 512 x 256 velocity grid (PAPER.md L167), min_lh = 10",
+                                                st, psiphi, pvx, pvy, dict(pd), 10.0, steps=1, warmup=1)
+        R["extras"]["postfilter"] = time_postfilter(R)
+        del img, var, mask, psiphi, ws
+        R["psiphi"] = R["ws"] = None
+        torch.cuda.empty_cache()
+        R["extras"]["configs3_heavy"] = time_heavy(R)
+    return R
+
+
+def time_search(R, what, st, psiphi, vx, vy, pd, min_lh, steps, warmup):
+    """Device time of kbmod_search alone (psi/phi resident) on another grid / mode; events on the launching stream."""
+    torch, kb = R["torch"], R["kb"]
+    T, H, W = st.img.shape
+    sp = kb.SearchParams(K=pd["K"], min_obs=pd["min_obs"], min_lh=min_lh)
+    ws = torch.empty(max(256, kb.kbmod_search_workspace_bytes_for(T, H, W, st.times, vx, vy, sp)), dtype=torch.uint8, device=R["dev"])
+    out = tuple(torch.empty((H, W, sp.K), dtype=dt, device=R["dev"]) for dt in (torch.float32, torch.float32, torch.int32, torch.int32))
+    ms, ph = [], []
+    for i in range(warmup + steps):
+        b, e = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        b.record()
+        kb.kbmod_search(psiphi, st.times, vx, vy, sp, out=out, workspace=ws)
+        e.record()
+        torch.cuda.synchronize()
+        if i >= warmup:
+            ms.append(b.elapsed_time(e)); ph.append(kb.kbmod_search_phase_ms())
+    evaluated, nominal, launches, algo_used, reached = kb.kbmod_search_stats(ws)
+    evals = float(H) * W * len(vx) * T
+    m = float(np.mean(ms))
+    rec = dict(workload=what, search_ms=m, value=evals / (m * 1e-3), unit=UNIT, steps=steps, warmup=warmup,
+               algo={1: "direct", 2: "pruned"}.get(algo_used, "?"), evaluated_fraction=evaluated / max(1, nominal),
+               trajectories_reaching_min_lh=reached,
+               trajectories=float(H) * W * len(vx), workspace_gb=ws.numel() / 1e9,
+               search_phases_ms={k: float(np.mean([p[k] for p in ph])) for k in ph[0]},
+               filled_result_slots=int((out[2] >= 0).sum()))
+    if algo_used == kb.ALGO_DIRECT:
+        # instruction-issue roofline of the direct kernel: executed warp-instructions per warp-trajectory from the
+        # committed ncu capture (profiles/), peak = 148 SMs x 4 warp-instructions per clock x max SM clock
+        tp = min(k for k in DIRECT_WARP_INSTR_PER_TRAJ if k >= T)
+        kern_ms = rec["search_phases_ms"]["gather"]
+        winst = float(H) * W * len(vx) / 32.0 * DIRECT_WARP_INSTR_PER_TRAJ[tp]
+        peak = N_SM * 4 * R["peaks"]["sm_max_mhz"] * 1e6
+        rec["roofline"] = dict(bound="issue", kernel="search_direct_kernel", achieved=winst / (kern_ms * 1e-3) / 1e12,
+                               peak=peak / 1e12, unit="Twarp-instr/s", frac=winst / (kern_ms * 1e-3) / peak,
+                               warp_instr_per_trajectory=DIRECT_WARP_INSTR_PER_TRAJ[tp], kernel_ms=kern_ms,
+                               source="smsp__inst_executed per trajectory from profiles/r2_search_direct_kernel_full.md")
+    del ws, out
+    return rec
+
+
+def time_postfilter(R):
+    """N1 (the CPU post-filter rejects ~10^6 trajectories in ~60 s on 30 cores -- context, another
+    machine): kbmod_sigmag_postfilter (sigma-G, reject L' < 10, ordered survivor list) on 10^6 and 10^7 lightcurves
+    of 26 epochs resident on the device."""
+    torch, kb = R["torch"], R["kb"]
+    out = {}
+    g = torch.Generator(device=R["dev"]).manual_seed(7)
+    for n in (1_000_000, 10_000_000):
+        phi = torch.rand((n, 26), generator=g, device=R["dev"]) * 7e-5 + 5e-5
+        psi = (torch.randn((n, 26), generator=g, device=R["dev"]) + 1.5) * phi.sqrt()
+        sp = kb.SearchParams(K=1, min_obs=13, min_lh=10.0)
+        kb.kbmod_sigmag_postfilter(psi, phi, sp)
+        torch.cuda.synchronize()
+        b, e = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        b.record()
+        r = kb.kbmod_sigmag_postfilter(psi, phi, sp)
+        e.record()
+        torch.cuda.synchronize()
+        ms = b.elapsed_time(e)
+        out[f"n={n}"] = dict(ms=ms, lightcurves_per_s=n / (ms * 1e-3), survivors=int(r["n_pass"][0]),
+                             hbm_gbs=n * 26 * 8 / (ms * 1e-3) / 1e9)
+        del phi, psi, r
+    out["paper"] = "~1e6 rejections in ~60 s on 30 CPU cores (PAPER.md L123; other hardware: context)"
+    return out
+
+
+def time_heavy(R):
+    """BASELINE configs[3] (2048x4096x50, 256 x 128 velocities, K = 16): prep + search, one warm-up and one timed pass."""
+    torch, kb = R["torch"], R["kb"]
+    st, vx, vy, pd, desc = make_workload("c4")
+    img, var, mask = (torch.from_numpy(a).to(R["dev"]) for a in (st.img, st.var, st.mask))
+    psiphi = kb.kbmod_prepare_psi_phi(img, var, mask, st.psf)
+    del img, var, mask
+    rec = time_search(R, desc + ", min_lh = 10", st, psiphi, vx, vy, pd, 10.0, steps=1, warmup=1)
+    del psiphi
+    torch.cuda.empty_cache()
+    return rec
 
 
 def in_bounds_fraction(times, vx, vy, H, W) -> float:
@@ -346,29 +465,42 @@ def report(R, args):
     T, H, W = st.img.shape
     n_vel = len(R["vx"])
     search_ms = float(np.mean(R["seg"]["search"]))
-    evaluated, nominal, launches, algo_used = R["stats"]
+    evaluated, nominal, launches, algo_used, reached = R["stats"]
     f_max = peaks["sm_max_mhz"] * 1e6
     tp = min(k for k in CE_COUNT if k >= T)
     ph = {k: float(np.mean([p[k] for p in R["phases"]])) for k in R["phases"][0]}
     kernel_ms = ph["gather"]  # the dominant kernel alone: bound_phase_kernel launches / the direct kernel
+    pi = R["plan_info"]
     if algo_used == kb.ALGO_DIRECT:
-        ops = float(H) * W * n_vel * (2 * CE_COUNT[tp] + 7 * T)
-        roof = dict(bound="alu", achieved=ops / (kernel_ms * 1e-3) / 1e12, peak=N_SM * 128 * f_max / 1e12,
-                    unit="Tlane-op/s", kernel="search_direct_kernel",
-                    peak_source="derived: 148 SMs x 128 FP32/ALU lanes x sm_max_mhz (DESIGN.md)")
+        tpd = min(k for k in DIRECT_WARP_INSTR_PER_TRAJ if k >= T) if T <= max(DIRECT_WARP_INSTR_PER_TRAJ) else None
+        per = DIRECT_WARP_INSTR_PER_TRAJ[tpd] if tpd else 640.0 * CE_COUNT[tp] / CE_COUNT[26]
+        winst = float(H) * W * n_vel / 32.0 * per
+        roof = dict(bound="issue", achieved=winst / (kernel_ms * 1e-3) / 1e12, peak=N_SM * 4 * f_max / 1e12,
+                    unit="Twarp-instr/s", kernel="search_direct_kernel", warp_instr_per_trajectory=per,
+                    peak_source="derived: 148 SMs x 4 warp-instructions per clock x sm_max_mhz (DESIGN.md)")
     else:
-        byts = R["evals"] * 4.0  # one packed 32-bit bound word per trajectory-epoch evaluation
+        # one packed 32-bit bound word per trajectory-epoch evaluation.  `frac` counts the words the
+        # kernel PHYSICALLY loads from shared memory: the nominal count less the (tile, group, epoch) regions that lie
+        # off the image and are skipped, less the epochs at which a whole velocity group shares one displacement
+        # (gathered once per pixel) -- both from the host plan (kbmod_plan_info).  The nominal figure is kept beside it.
+        nominal_bytes = R["evals"] * 4.0
+        phys_bytes = nominal_bytes * (1.0 - pi["off_image_fraction"]) * pi["gather_fraction"]
         # denominator: the shared-memory load bandwidth measured live on this GPU (LDS.128 microbenchmark of the
         # library: the highest of the three widths); the derived figure and the LDS.32 figure are quoted beside it
         peak = R["smem_gbs"][16]
-        roof = dict(bound="smem", achieved=byts / (kernel_ms * 1e-3) / 1e9, peak=peak,
+        roof = dict(bound="smem", achieved=phys_bytes / (kernel_ms * 1e-3) / 1e9, peak=peak,
                     unit="GB/s", kernel="bound_phase_kernel",
+                    what="shared-memory bytes the kernel loads (in-bounds, unique gathers) / live kernel time",
                     peak_source="measured live: kbmod_measure_smem_gbs(16), conflict-free LDS.128 on all SMs",
                     peak_theoretical=N_SM * 128 * f_max / 1e9, peak_measured_lds32=R["smem_gbs"][4],
-                    algorithmic_bytes_per_eval=4,
-                    # SURVEY 8(d) counted 8 B (psi, phi as float32) per evaluation; against that figure:
-                    frac_of_survey_8B_roofline=2.0 * byts / (kernel_ms * 1e-3) / 1e9 / peak,
-                    whole_search_frac_of_survey_8B_roofline=2.0 * byts / (search_ms * 1e-3) / 1e9 / peak)
+                    algorithmic_bytes_per_eval=4, off_image_region_share=pi["off_image_fraction"],
+                    gathers_per_nominal_eval=pi["gather_fraction"],
+                    nominal_achieved=nominal_bytes / (kernel_ms * 1e-3) / 1e9,
+                    nominal_frac=nominal_bytes / (kernel_ms * 1e-3) / 1e9 / peak,
+                    # SURVEY 8(d) counted 8 B (psi, phi as float32) per NOMINAL evaluation over the whole search
+                    # (a deviation recorded in DESIGN.md section 6); against that figure:
+                    whole_search_frac_of_survey_8B_roofline=2.0 * nominal_bytes / (search_ms * 1e-3) / 1e9 / peak,
+                    whole_search_frac_4B_nominal=nominal_bytes / (search_ms * 1e-3) / 1e9 / peak)
     roof["frac"] = roof["achieved"] / roof["peak"]
     roof["traffic"] = TRAFFIC.get(roof["kernel"])
     roof["kernel_ms"] = kernel_ms
@@ -378,7 +510,7 @@ def report(R, args):
     if not args.no_cpu_baseline:
         smp = OracleSample(st, R["vx"], R["vy"], R["pd"], args.min_lh)
         r, cores, sample, _ = smp.step(12.0)
-        cpu = dict(value=r, unit=UNIT, cores=cores, kind="oracle", sample=sample)
+        cpu = dict(value=r, unit=UNIT, cores=cores, kind="oracle", sample=sample, value_one_core=smp.one_core(), cpu=cpu_model())
     line = dict(metric=METRIC, value=value, unit=UNIT, n_gpus=world, steps=args.steps, warmup=args.warmup,
                 ms_per_step=ms_per_step, higher_is_better=True, scaling="weak", vs_baseline=None, dtype="f32",
                 data="synthetic",
@@ -389,13 +521,16 @@ def report(R, args):
                             multi_gpu="one independent CCD stack per rank, no collective" if world > 1 else "single GPU",
                             host_plan="velocity grouping / staging geometry cached after the first (warm-up) step: same grid and times"),
                 segments_ms={k: float(np.mean(v)) for k, v in R["seg"].items()},
-                evaluated_fraction=evaluated / max(1, nominal),
+                evaluated_fraction=evaluated / max(1, nominal), trajectories_reaching_min_lh=reached,
                 in_bounds_fraction=in_bounds_fraction(st.times, R["vx"], R["vy"], H, W),
                 roofline=roof, cpu_baseline=cpu,
                 e2e=dict(value=whole_job_value(R["evals"], world, e2e_max), unit=UNIT, h2d_bytes_per_step=h2d,
                          d2h_bytes_per_step=d2h, ms_per_step=e2e_max, steps=e2e_steps,
                          matches_resident_run=same, api="kbmod_pipeline_host_batch (prep + search per stack; pinned host buffers; copies overlap the neighbouring searches)"),
-                gpu_launches=args.steps * (T + int(launches) + 1), clocks=R["clocks"], peaks_source=peaks["source"])
+                gpu_launches=args.steps * (T + int(launches) + 1), clocks=R["clocks"], peaks_source=peaks["source"],
+                planner=dict(n_groups=pi["n_groups"], staged_bytes_per_eval=pi["staged_bytes_per_eval"],
+                             canvas=pi["canvas"], workspace_gb=pi["workspace_bytes"] / 1e9),
+                **R["extras"])
     print(json.dumps(line), flush=True)
 
 
@@ -409,6 +544,7 @@ def main():
     ap.add_argument("--min-lh", type=float, default=10.0, dest="min_lh")
     ap.add_argument("--algo", default="auto", choices=["auto", "direct", "pruned"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-extras", action="store_true", help="skip the mode-B / paper-grid / configs[3] / post-filter records")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)

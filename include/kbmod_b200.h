@@ -175,9 +175,11 @@ int kbmod_search_unfiltered_lh(const void* d_workspace, const int32_t* d_vel_idx
  * kbmod_plan_workspace_bytes().  kbmod_plan_search enqueues: one table upload, the padded-stack build, the
  * search kernels, the key -> output pass; it never synchronises and never touches pageable host memory.
  *   row_begin, row_end   the band of start rows this plan searches (0, H for the whole image)
- * kbmod_plan_info fills h_out[8]: kernel used (KBMOD_ALGO_DIRECT / PRUNED), velocity groups, bytes staged into shared
+ * kbmod_plan_info fills h_out[10]: kernel used (KBMOD_ALGO_DIRECT / PRUNED), velocity groups, bytes staged into shared
  * memory per trajectory-epoch evaluation, share of (tile, group, epoch) region loads that lie off the image, padded
- * stack width and height, 1 if the velocity list was too scattered for the pruned kernel, bytes of the table blob. */
+ * stack width and height, 1 if the velocity list was too scattered for the pruned kernel, bytes of the table blob,
+ * shared-memory gathers per nominal evaluation before off-image skipping (< 1: epochs at which a whole velocity group
+ * has one displacement are gathered once per pixel), workspace bytes. */
 typedef struct kbmod_plan kbmod_plan;
 int kbmod_plan_create(int T, int H, int W, const double* h_times, const float* h_vx, const float* h_vy, int n_vel,
                       const kbmod_search_params* p, int row_begin, int row_end, kbmod_plan** out);
@@ -201,9 +203,11 @@ int kbmod_release_thread_state(void);
 int kbmod_plan_stats(int T, int H, int W, const double* h_times, const float* h_vx, const float* h_vy, int n_vel,
                      const kbmod_search_params* p, double* h_out);
 
-/* Counters of the last kbmod_search on this thread (read after synchronising the stream).
- * h_out[0] = trajectories fully evaluated (sigma-G run), h_out[1] = trajectories nominally
- * searched (H*W*n_vel), h_out[2] = kernels launched by the call, h_out[3] = algo actually used. */
+/* Counters of the last search that used this workspace (a blocking 40-byte read; synchronises the device).
+ * h_out[5]: [0] = trajectories fully evaluated (sigma-G run), [1] = trajectories nominally searched (rows*W*n_vel),
+ * [2] = kernels launched by the call, [3] = algo actually used, [4] = pruned path only: trajectories whose L'
+ * reached min_lh, i.e. the candidates before the per-pixel top-K (PAPER.md:L91 quotes ~10^7 per search); 0 for the
+ * direct kernel. */
 int kbmod_search_stats(const void* d_workspace, unsigned long long* h_out);
 
 /* Optional timing of the phases of kbmod_search, per host thread (what bench.py's roofline line reads).

@@ -54,6 +54,15 @@ int oracle_num_threads(void) {
 #endif
 }
 
+/* number of OpenMP threads the following calls use (bench.py's 1-core baseline figure); no arithmetic here */
+void oracle_set_num_threads(int n) {
+#ifdef _OPENMP
+    if (n >= 1) omp_set_num_threads(n);
+#else
+    (void)n;
+#endif
+}
+
 /* ------------------------------------------------------------------ O1: psi / phi (L79; R1-R4) */
 static int pixel_good(const float *img, const float *var, const uint8_t *mask, int H, int W, int y, int x) {
     if (x < 0 || x >= W || y < 0 || y >= H) return 0;

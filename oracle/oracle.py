@@ -68,6 +68,10 @@ def num_threads() -> int:
     return int(lib().oracle_num_threads())
 
 
+def set_num_threads(n: int) -> None:
+    lib().oracle_set_num_threads(int(n))
+
+
 def pct_rank(q: float, n: int) -> int:
     return int(lib().oracle_pct_rank(C.c_float(q), n))
 

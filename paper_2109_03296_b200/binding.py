@@ -287,11 +287,11 @@ class Plan:
         return int(lib().kbmod_plan_workspace_bytes(self._h))
 
     def info(self):
-        out = (C.c_double * 8)()
+        out = (C.c_double * 10)()
         _check(lib().kbmod_plan_info(self._h, out))
         return dict(algo=int(out[0]), n_groups=int(out[1]), staged_bytes_per_eval=float(out[2]),
                     off_image_fraction=float(out[3]), canvas=(int(out[4]), int(out[5])), too_scattered=bool(out[6]),
-                    table_bytes=int(out[7]))
+                    table_bytes=int(out[7]), gather_fraction=float(out[8]), workspace_bytes=int(out[9]))
 
     def search(self, psiphi, out=None, workspace=None, stream=None):
         import torch
@@ -377,8 +377,8 @@ def kbmod_plan_stats(T, H, W, times, vx, vy, params: SearchParams):
 
 
 def kbmod_search_stats(workspace):
-    """[evaluated, nominal, launches, algo] of the last kbmod_search that used `workspace` (synchronises)."""
-    out = (C.c_ulonglong * 4)()
+    """[evaluated, nominal, launches, algo, reached_min_lh] of the last search that used `workspace` (synchronises)."""
+    out = (C.c_ulonglong * 5)()
     _check(lib().kbmod_search_stats(_dev(workspace), out))
     return [int(v) for v in out]
 

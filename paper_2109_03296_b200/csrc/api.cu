@@ -361,12 +361,16 @@ extern "C" int kbmod_plan_info(const kbmod_plan* pl, double* h_out) {
     h_out[5] = (double)pl->G.Hp;
     h_out[6] = (double)pl->pr.too_scattered;
     h_out[7] = (double)pl->blob_bytes;
+    h_out[8] = pl->pr.gather_fraction;
+    h_out[9] = (double)pl->w_total;
     return KBMOD_OK;
 }
 
 extern "C" int kbmod_plan_search(kbmod_plan* pl, const float* d_psiphi, float* d_lh, float* d_flux, int32_t* d_vel_idx,
                                  int32_t* d_n_obs, void* d_workspace, size_t workspace_bytes, void* stream) {
-    KB_REQUIRE(pl && d_psiphi && d_lh && d_flux && d_vel_idx && d_n_obs, KBMOD_ERR_INVALID_ARG, "NULL argument");
+    KB_REQUIRE(pl && d_psiphi, KBMOD_ERR_INVALID_ARG, "NULL argument");
+    if (pl->row_end == pl->row_begin) return KBMOD_OK;  // an empty band: nothing to search, nothing to write
+    KB_REQUIRE(d_lh && d_flux && d_vel_idx && d_n_obs, KBMOD_ERR_INVALID_ARG, "NULL argument");
     KB_REQUIRE(d_workspace && workspace_bytes >= pl->w_total, KBMOD_ERR_WORKSPACE,
                "workspace of %zu bytes is smaller than the %zu needed", workspace_bytes, pl->w_total);
     KB_REQUIRE(((uintptr_t)d_workspace & 255) == 0, KBMOD_ERR_INVALID_ARG, "workspace must be 256-byte aligned");
@@ -497,7 +501,8 @@ static int search_rows(const float* d_psiphi, int T, int H, int W, const double*
                        const float* h_vy, int n_vel, const kbmod_search_params* p, int row_begin, int row_end, float* d_lh,
                        float* d_flux, int32_t* d_vel_idx, int32_t* d_n_obs, void* d_workspace, size_t workspace_bytes,
                        void* stream) {
-    KB_REQUIRE(d_psiphi && h_times && d_lh && d_flux && d_vel_idx && d_n_obs && p, KBMOD_ERR_INVALID_ARG, "NULL argument");
+    KB_REQUIRE(d_psiphi && h_times && p, KBMOD_ERR_INVALID_ARG, "NULL argument");
+    KB_REQUIRE(row_begin == row_end || (d_lh && d_flux && d_vel_idx && d_n_obs), KBMOD_ERR_INVALID_ARG, "NULL argument");
     kbmod_plan* pl = nullptr;
     int rc = thread_plan(T, H, W, h_times, h_vx, h_vy, n_vel, p, row_begin, row_end, &pl);
     if (rc) return rc;
@@ -550,7 +555,7 @@ extern "C" int kbmod_plan_stats(int T, int H, int W, const double* h_times, cons
 
 extern "C" int kbmod_search_stats(const void* d_workspace, unsigned long long* h_out) {
     KB_REQUIRE(d_workspace && h_out, KBMOD_ERR_INVALID_ARG, "NULL argument");
-    KB_CUDA(cudaMemcpy(h_out, d_workspace, 4 * sizeof(unsigned long long), cudaMemcpyDeviceToHost));
+    KB_CUDA(cudaMemcpy(h_out, d_workspace, 5 * sizeof(unsigned long long), cudaMemcpyDeviceToHost));
     return KBMOD_OK;
 }
 

@@ -285,6 +285,7 @@ struct PrunedPlan {
     int too_scattered = 0;            // more groups than the workspace layout allows: AUTO falls back to the direct kernel
     double staged = 0.0, evals = 0.0;  // bytes staged / evaluations covered per tile (before off-image skipping)
     double off_image = 0.0;            // share of the (tile, group, epoch) region loads that lie off the image
+    double gather_fraction = 1.0;      // shared-memory gathers per nominal evaluation (uniform epochs: one per pixel)
     std::vector<int32_t> gvel;              // [ng][16] velocity index or -1
     std::vector<unsigned char> gtbl;        // [ng] table blocks
     std::vector<unsigned long long> maskx;  // [ng][tiles_x]

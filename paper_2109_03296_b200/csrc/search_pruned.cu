@@ -104,6 +104,7 @@ struct TensorMaps {
 
 struct BoundParams {
     unsigned char mkept[KBMOD_MAX_T + 1];  // m(n)
+    int mk_min;                            // min of m(n) over n >= max(1, min_obs): what the quick group test may count on
     int pass_all;                          // min_lh <= 0 (or not finite): nothing can be pruned
     int cbits;                             // width of the two count fields of a plane word: 2^cbits > T
 };
@@ -148,7 +149,7 @@ bound_scale_kernel(const float2* __restrict__ psiphi, int T, int H, int W, float
     // of landing in a handful of columns (a bad column or a masked disc would bias the floors)
     size_t stride = plane / n_samp;
     if (stride > 1) {
-        stride |= 1;
+        stride = (stride - 1) | 1;  // odd and not larger than before: (n_samp - 1) * stride stays inside the plane
         for (;;) {
             size_t a = stride, b = (size_t)W;
             while (b) { const size_t r = a % b; a = b; b = r; }
@@ -571,14 +572,29 @@ bound_phase_kernel(const __grid_constant__ TensorMaps maps, int T, int row_begin
             for (int h = 0; h < PR_PIX; ++h) {
                 const bool in_img = (px0 + 32 * (h & 1)) < W && (py0 + 16 * (h >> 1)) < row_end;
                 m[h] = 0u;
+                // quick test of the pixel's 16 velocities at once: the largest sum against the smallest threshold any of
+                // them can have (the fields of a word do not carry into each other, so the maximum of the packed words
+                // carries the maximum sum, and the OR of the low-phi counts bounds their maximum); 98 % of the pixels
+                // stop here
+                unsigned int mx = AN[h][0], orr = AN[h][0];
 #pragma unroll
-                for (int j = 0; j < PR_G; ++j) {
-                    const unsigned int an = AN[h][j] + ANU[h];
-                    const int n = (int)(an & cmask), n_low = (int)((an >> BP.cbits) & cmask);
-                    // at least m(n) epochs are kept, at least m(n) - n_low of them with phi >= their epoch's floor
-                    const int m_eff = max((int)BP.mkept[n] - n_low, 0);
-                    const bool pass = BP.pass_all || (float)(an >> (2 * BP.cbits)) >= __ldg(thr + m_eff);
-                    if (in_img && n >= need && pass) m[h] |= 1u << j;
+                for (int j = 1; j < PR_G; ++j) {
+                    mx = max(mx, AN[h][j]);
+                    orr |= AN[h][j];
+                }
+                const int nlow_ub = (int)((orr >> BP.cbits) & cmask) + (int)((ANU[h] >> BP.cbits) & cmask);
+                const float sum_max = (float)((mx + ANU[h]) >> (2 * BP.cbits));
+                const bool maybe = in_img && (BP.pass_all || sum_max >= __ldg(thr + max(BP.mk_min - nlow_ub, 0)));
+                if (maybe) {
+#pragma unroll
+                    for (int j = 0; j < PR_G; ++j) {
+                        const unsigned int an = AN[h][j] + ANU[h];
+                        const int n = (int)(an & cmask), n_low = (int)((an >> BP.cbits) & cmask);
+                        // at least m(n) epochs are kept, at least m(n) - n_low of them with phi >= their epoch's floor
+                        const int m_eff = max((int)BP.mkept[n] - n_low, 0);
+                        const bool pass = BP.pass_all || (float)(an >> (2 * BP.cbits)) >= __ldg(thr + m_eff);
+                        if (n >= need && pass) m[h] |= 1u << j;
+                    }
                 }
                 m[h] &= vmask;
                 my_cnt += __popc(m[h]);
@@ -633,8 +649,11 @@ struct ExactArgs {
     unsigned long long* keys;  // [row_end - row_begin][W][K]
 };
 
+// (A two-pass form -- filter values first, psi/phi of the same elements re-read afterwards, 85 registers, 3 CTAs per
+// SM -- was measured: the second reads are not L1 hits and the phase took twice as long.)
+// Returns true iff the trajectory has a result with L' >= min_lh.
 template <int TP>
-__device__ __forceinline__ void eval_pair(const ExactArgs& A, const DevParams& P, int x0, int y0, int v, float* scratch,
+__device__ __forceinline__ bool eval_pair(const ExactArgs& A, const DevParams& P, int x0, int y0, int v, float* scratch,
                                           int stride) {
     const unsigned int base = (unsigned int)(y0 + A.G.pyn) * (unsigned int)A.G.Wp + (unsigned int)(x0 + A.G.pxn);
     float psi[TP], phi[TP], f[TP], sp, sf;
@@ -643,21 +662,28 @@ __device__ __forceinline__ void eval_pair(const ExactArgs& A, const DevParams& P
     const int nk = kb_score_s4<TP>(psi, phi, f, n, P, scratch, stride, sp, sf);
     if (nk > 0) {
         const float lh = kb_lh_of(sp, sf);
-        if (lh >= P.min_lh) topk_insert(A.keys + ((size_t)(y0 - A.row_begin) * A.W + x0) * P.K, P.K, kb_topk_key(lh, v));
+        if (lh >= P.min_lh) {
+            topk_insert(A.keys + ((size_t)(y0 - A.row_begin) * A.W + x0) * P.K, P.K, kb_topk_key(lh, v));
+            return true;
+        }
     }
+    return false;
 }
 
 constexpr int EX_THREADS = 256;
-constexpr int EX_CTAS_PER_SM = 4;
+#ifndef KB_EX_CTAS
+#define KB_EX_CTAS 2
+#endif
+constexpr int EX_CTAS_PER_SM = KB_EX_CTAS;
 
 template <int TP>
-__global__ void __launch_bounds__(EX_THREADS)
+__global__ void __launch_bounds__(EX_THREADS, EX_CTAS_PER_SM)
 exact_queue_kernel(const __grid_constant__ ExactArgs A, const __grid_constant__ DevParams P,
                    const __grid_constant__ Queue Qu, unsigned long long* __restrict__ stats) {
     extern __shared__ float scratch_all[];  // [TP][EX_THREADS]
     const unsigned long long cnt = *Qu.count;
     const unsigned long long n = cnt < Qu.cap ? cnt : Qu.cap;
-    unsigned long long done = 0;
+    unsigned long long done = 0, passed = 0;
     // the trip count is warp-uniform and every iteration ends in __syncwarp(): without it the lanes of a warp
     // drift apart after the first divergent top-K insertion and run the whole body one by one from then on
     // (measured: 3.7 active threads per instruction)
@@ -673,14 +699,20 @@ exact_queue_kernel(const __grid_constant__ ExactArgs A, const __grid_constant__ 
         e_next = (i_next < n) ? __ldg(Qu.entries + i_next) : hole;
         if (e.y != 0xFFFFFFFFu) {
             const int y0 = (int)(e.x / (unsigned)A.W), x0 = (int)(e.x - (unsigned)y0 * (unsigned)A.W);
-            eval_pair<TP>(A, P, x0, y0, (int)e.y, scratch_all + threadIdx.x, EX_THREADS);
+            passed += eval_pair<TP>(A, P, x0, y0, (int)e.y, scratch_all + threadIdx.x, EX_THREADS) ? 1ull : 0ull;
             ++done;
         }
         __syncwarp();
     }
-    // statistics: trajectories fully evaluated
-    for (int d = 16; d > 0; d >>= 1) done += __shfl_down_sync(0xFFFFFFFFu, done, d);
-    if ((threadIdx.x & 31) == 0 && done) atomicAdd(stats, done);
+    // statistics: trajectories fully evaluated, and how many of them reached min_lh (candidates before the top-K)
+    for (int d = 16; d > 0; d >>= 1) {
+        done += __shfl_down_sync(0xFFFFFFFFu, done, d);
+        passed += __shfl_down_sync(0xFFFFFFFFu, passed, d);
+    }
+    if ((threadIdx.x & 31) == 0 && done) {
+        atomicAdd(stats, done);
+        if (passed) atomicAdd(stats + 4, passed);
+    }
 }
 
 // items that did not fit the queue: every pair of the (tile, group, warp) item is evaluated
@@ -695,7 +727,7 @@ exact_overflow_kernel(const __grid_constant__ ExactArgs A, const __grid_constant
     const size_t n_warps = ((size_t)gridDim.x * EX_THREADS) >> 5;
     const int W = A.W;
     const int tiles_x = (W + PR_TW - 1) / PR_TW, tiles_y = (A.row_end - A.row_begin + PR_TH - 1) / PR_TH;
-    unsigned long long done = 0;
+    unsigned long long done = 0, passed = 0;
     for (size_t w = warp_global; w < n_words; w += n_warps) {
         unsigned int bits = __ldg(overflow + w);
         while (bits) {
@@ -712,7 +744,7 @@ exact_overflow_kernel(const __grid_constant__ ExactArgs A, const __grid_constant
                 for (int j = 0; j < PR_G; ++j) {
                     const int v = __ldg(gvel + (size_t)g * PR_G + j);
                     if (v >= 0 && x0 < W && y0 < A.row_end) {
-                        eval_pair<TP>(A, P, x0, y0, v, scratch_all + threadIdx.x, EX_THREADS);
+                        passed += eval_pair<TP>(A, P, x0, y0, v, scratch_all + threadIdx.x, EX_THREADS) ? 1ull : 0ull;
                         ++done;
                     }
                     __syncwarp();  // keep the warp converged (see exact_queue_kernel)
@@ -720,8 +752,14 @@ exact_overflow_kernel(const __grid_constant__ ExactArgs A, const __grid_constant
             }
         }
     }
-    for (int d = 16; d > 0; d >>= 1) done += __shfl_down_sync(0xFFFFFFFFu, done, d);
-    if (lane == 0 && done) atomicAdd(stats, done);
+    for (int d = 16; d > 0; d >>= 1) {
+        done += __shfl_down_sync(0xFFFFFFFFu, done, d);
+        passed += __shfl_down_sync(0xFFFFFFFFu, passed, d);
+    }
+    if (lane == 0 && done) {
+        atomicAdd(stats, done);
+        if (passed) atomicAdd(stats + 4, passed);
+    }
 }
 
 }  // namespace
@@ -886,7 +924,7 @@ int kb_pruned_plan_build(int T, int H, int W, int row_begin, int row_end, const 
     std::vector<unsigned char>& gtbl = PC.gtbl;
     gvel.assign((size_t)ng * PR_G, -1);
     gtbl.assign((size_t)ng * TBL, 0);
-    double staged = 0.0, evals = 0.0;
+    double staged = 0.0, evals = 0.0, gathers = 0.0;
     uint32_t ph = 0;
     for (int g = 0; g < ng; ++g) {
         if (g % PR_SUB == 0) ph = 0;  // every work unit starts its ring chain at offset 0
@@ -913,6 +951,7 @@ int kb_pruned_plan_build(int T, int H, int W, int row_begin, int row_end, const 
             bool same = true;
             for (int j = 1; j < cnt; ++j) same = same && offs[t * PR_G + j] == offs[t * PR_G];
             if (same) e.pitch_k |= 0x100;
+            gathers += (double)PR_TW * PR_TH * (same ? 1 : cnt);  // a uniform epoch is gathered once per pixel
             ph += (uint32_t)bytes;
             ge[t] = e;
             staged += (double)bytes;
@@ -951,6 +990,7 @@ int kb_pruned_plan_build(int T, int H, int W, int row_begin, int row_end, const 
     }
     PC.T = T; PC.H = H; PC.W = W; PC.row_begin = row_begin; PC.row_end = row_end; PC.n_vel = n_vel;
     PC.ng = ng; PC.staged = staged; PC.evals = evals;
+    PC.gather_fraction = evals > 0 ? gathers / evals : 1.0;
     PC.off_image = all > 0 ? 1.0 - on / all : 0.0;
     PC.ring_bytes = ring_bytes_for(T);
     PC.tiles_x = tiles_x; PC.tiles_y = tiles_y;
@@ -977,6 +1017,12 @@ static bool bound_min_kept(const kbmod_search_params* p, const DevParams& P, int
             else return false;
         }
         bp->mkept[n] = (unsigned char)(n == 0 ? 0 : m);
+    }
+    {
+        const int need = p->min_obs > 1 ? p->min_obs : 1;
+        int mk = KBMOD_MAX_T;
+        for (int n = need; n <= T; ++n) mk = std::min(mk, (int)bp->mkept[n]);
+        bp->mk_min = need <= T ? mk : 0;
     }
     bp->pass_all = !(p->min_lh > 0.0f && p->min_lh < INFINITY);
     bp->cbits = 1;
@@ -1052,6 +1098,7 @@ int kb_launch_search_pruned(const float* d_psiphi, const PrunedPlan& plan, const
     {
         const size_t n = (size_t)T * H * Wp;
         bound_scale_kernel<<<1, 1024, 0, st>>>(reinterpret_cast<const float2*>(d_psiphi), T, H, W, P.min_lh, bp, d_scale);
+        KB_CUDA(cudaGetLastError());
         bound_plane_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(reinterpret_cast<const float2*>(d_psiphi), d_B, H, W,
                                                                         (int)Wp, (size_t)T * H, bp.cbits, d_scale);
         KB_CUDA(cudaGetLastError());
@@ -1077,8 +1124,10 @@ int kb_launch_search_pruned(const float* d_psiphi, const PrunedPlan& plan, const
                     KB_CUDA(cudaMemsetAsync(Qu.count, 0, 2 * sizeof(unsigned long long), st));  // queue and unit counters
                     bound_phase_kernel<<<std::min(grid, b1 - b0), PR_THREADS, smem1, st>>>(maps, T, row_begin, row_end, W, b0, b1,
                                                                                           g0, g1, tb, bp, P.min_obs, d_scale, Qu);
+                    KB_CUDA(cudaGetLastError());
                     kb_phase_mark(KB_PHASE_BOUND, st);
                     exact_queue_kernel<TP><<<n_sm * EX_CTAS_PER_SM, EX_THREADS, smem2, st>>>(EA, P, Qu, d_stats);
+                    KB_CUDA(cudaGetLastError());
                     kb_phase_mark(KB_PHASE_EXACT, st);
                     launches += 2;
                 }

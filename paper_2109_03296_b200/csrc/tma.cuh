@@ -21,6 +21,17 @@ __device__ __forceinline__ void kb_mbar_expect_tx(uint64_t* bar, uint32_t bytes)
 __device__ __forceinline__ void kb_mbar_wait(uint64_t* bar, uint32_t parity) {
     // try_wait suspends the thread in hardware until the phase completes or the time hint (ns) runs out, so a
     // waiting warp costs a few issue slots per microsecond instead of spinning against the warps that have work
+#ifdef KB_WAIT_PLAIN
+    asm volatile(
+        "{\n\t"
+        ".reg .pred p;\n\t"
+        "KB_WAIT_%=:\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
+        "@p bra KB_DONE_%=;\n\t"
+        "bra KB_WAIT_%=;\n\t"
+        "KB_DONE_%=:\n\t"
+        "}" ::"r"(kb_smem_u32(bar)), "r"(parity) : "memory");
+#else
     asm volatile(
         "{\n\t"
         ".reg .pred p;\n\t"
@@ -30,6 +41,7 @@ __device__ __forceinline__ void kb_mbar_wait(uint64_t* bar, uint32_t parity) {
         "bra KB_WAIT_%=;\n\t"
         "KB_DONE_%=:\n\t"
         "}" ::"r"(kb_smem_u32(bar)), "r"(parity), "r"(2000u) : "memory");
+#endif
 }
 // non-blocking test of a phase (acquire): true once the phase with this parity has completed
 __device__ __forceinline__ bool kb_mbar_test(uint64_t* bar, uint32_t parity) {

@@ -113,3 +113,71 @@ def test_planner_host_logic_without_gpu(lib):
     # bad arguments are refused on the host
     with pytest.raises(kb.KbmodError):
         kb.kbmod_plan_stats(65, 64, 64, np.zeros(65), vx, vy, sp)
+
+
+def test_percentile_positions_match_the_oracle_for_user_percentiles(lib, oracle):
+    """The library's own percentile table (DevParams.rk_* / fr_*), read through the host-only kbmod_percentile_ranks,
+    against the oracle for the paper's 25 / 75 and for user percentiles, both percentile definitions: the value the
+    table picks from a sorted array must be the oracle's percentile of that array, bit for bit."""
+    rng = np.random.default_rng(9)
+    for lo, hi in ((25.0, 75.0), (10.0, 90.0), (0.0, 100.0), (33.3, 66.7), (50.0, 50.0), (5.0, 95.0)):
+        for interp in (0, 1):
+            sp = binding.SearchParams(pct_lo=lo, pct_hi=hi, pct_interp=interp)
+            for n in range(1, 65):
+                s = np.sort(rng.standard_normal(n).astype(np.float32))
+                for (k, g), q in zip(binding.kbmod_percentile_ranks(sp, n), (lo, 50.0, hi)):
+                    assert 0 <= k < n
+                    if g < 0:
+                        got = s[k]
+                        if not interp:
+                            assert k == oracle.pct_rank(q, n)
+                    else:
+                        assert interp and k + 1 < n and 0.0 <= g < 1.0
+                        got = np.float32(s[k] + np.float32(np.float32(g) * np.float32(s[k + 1] - s[k])))
+                    assert got == np.float32(oracle.pct_value(s, q, interp)), (lo, hi, interp, n, q)
+    assert [k for k, _ in binding.kbmod_percentile_ranks(binding.SearchParams(), 26)] == [6, 12, 19]
+
+
+def test_plan_without_gpu_and_row_bands_tile_the_image(lib):
+    """kbmod_plan_create is host-only work (no CUDA context needed): kernel choice, velocity groups, padded-stack
+    geometry, workspace size.  Row bands (one CCD shards over GPUs by start-pixel rows, results
+    concatenate): the bands' plans cover every start row exactly once and each needs less workspace than the whole."""
+    import paper_2109_03296_b200 as kb
+    times = synth.night_times((7, 6, 7, 6))
+    vx, vy = synth.config3_grid()
+    sp = kb.SearchParams(K=8, min_obs=13)
+    T, H, W = 26, 4096, 2048
+    full = kb.Plan(T, H, W, times, vx, vy, sp)
+    fi = full.info()
+    assert fi["algo"] == kb.ALGO_PRUNED and fi["n_groups"] == 512 and not fi["too_scattered"]
+    # motion about theta = 4.4 rad is towards -x, -y: the stack is padded on the low sides only, by the largest displacement
+    dx, dy = kb.kbmod_displacements(times, vx, vy)
+    assert fi["canvas"] == (W - dx.min() + max(dx.max(), 0), H - dy.min() + max(dy.max(), 0))
+    assert dx.max() <= 0 and dy.max() <= 0 and -dx.min() == 919 and -dy.min() == 1567   # SURVEY 7: max |d| = (919, 1567)
+    assert 0 < full.workspace_bytes() < kb.kbmod_search_workspace_bytes(T, H, W, len(vx), sp)
+    assert full.workspace_bytes() == kb.kbmod_search_workspace_bytes_for(T, H, W, times, vx, vy, sp)
+    n = 4
+    edges = [H * r // n for r in range(n + 1)]
+    covered = np.zeros(H, int)
+    for r in range(n):
+        band = kb.Plan(T, H, W, times, vx, vy, sp, rows=(edges[r], edges[r + 1]))
+        bi = band.info()
+        assert bi["algo"] == fi["algo"] and bi["n_groups"] == fi["n_groups"] and bi["canvas"] == fi["canvas"]
+        assert band.workspace_bytes() < full.workspace_bytes()
+        covered[band.rows[0]:band.rows[1]] += 1
+        # bands towards +y keep more of their trajectories on the image than bands towards -y (the motion is towards -y)
+        if r:
+            assert bi["off_image_fraction"] <= prev + 1e-12
+        prev = bi["off_image_fraction"]
+        band.destroy()
+    assert np.all(covered == 1)
+    # direct kernel when nothing can be pruned; an empty band is legal
+    assert kb.Plan(T, H, W, times, vx, vy, kb.SearchParams(min_lh=-np.inf)).info()["algo"] == kb.ALGO_DIRECT
+    assert kb.Plan(T, H, W, times, vx, vy, sp, rows=(100, 100)).workspace_bytes() > 0
+    with pytest.raises(kb.KbmodError):
+        kb.Plan(T, H, W, times, vx, vy, sp, rows=(10, H + 1))
+    with pytest.raises(kb.KbmodError):  # a canvas beyond 2^32 pixels: T = 64 with displacements in every direction
+        kb.Plan(64, 4096, 2048, np.linspace(0, 10, 64), np.array([900, -900], np.float32), np.array([900, -900], np.float32), sp)
+    full.destroy()
+    kb.kbmod_release_thread_state()   # frees the plan kbmod_search_workspace_bytes_for cached; callable without a GPU
+    kb.kbmod_release_thread_state()   # idempotent

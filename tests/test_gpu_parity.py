@@ -140,23 +140,30 @@ def test_search_empty_velocity_list(kb):
     assert torch.all(torch.isneginf(lh)) and torch.all(vel == -1) and torch.all(nobs == 0) and torch.all(flux == 0)
 
 
-def test_search_config2_medium(kb, oracle):
-    """BASELINE configs[1] at full size on the GPU (512x512, T=10, 2048 velocities, K=8, 1% mask);
-    the oracle checks 3000 random pixels, the four borders' corners and every injected mover start."""
+@pytest.mark.parametrize("min_lh", [10.0, -np.inf])
+def test_search_config2_medium_every_pixel(kb, oracle, min_lh):
+    """BASELINE configs[1] (512x512, T=10, 64 x 32 velocities over the full circle, K=8, 1% mask) as SURVEY 8c
+    prescribes: EVERY pixel, both kernels, mode (A) min_lh = 10 and mode (B) min_lh = -inf.  The full 2 pi angle
+    grid is the one configuration whose velocity groups scatter in all directions."""
     st = synth.config2_medium()
     vx, vy = synth.config2_grid()
     d = _prep(kb, st)
-    rng = np.random.default_rng(7)
-    px = rng.integers(0, 512, 3000).astype(np.int32)
-    py = rng.integers(0, 512, 3000).astype(np.int32)
-    mx = np.array([int(m["x0"]) for m in st.movers] + [0, 511, 0, 511], np.int32)
-    my = np.array([int(m["y0"]) for m in st.movers] + [0, 0, 511, 511], np.int32)
-    px, py = np.concatenate([px, mx]), np.concatenate([py, my])
-    sp = kb.SearchParams(K=8, min_obs=5, min_lh=-np.inf, algo=kb.ALGO_DIRECT)
-    r = _search_and_compare(kb, oracle, d, st.times, vx, vy, sp, pixels=(px, py))
-    assert r["n_entries"] == len(px) * 8
-    sp = kb.SearchParams(K=8, min_obs=5, min_lh=10.0, algo=kb.ALGO_DIRECT)
-    _search_and_compare(kb, oracle, d, st.times, vx, vy, sp, pixels=(px, py))
+    psiphi = d.cpu().numpy()
+    T, H, W = st.img.shape
+    yy, xx = np.mgrid[0:H, 0:W]
+    px, py = xx.reshape(-1).astype(np.int32), yy.reshape(-1).astype(np.int32)
+    op = oracle.Params(K=8, min_obs=5, min_lh=min_lh)
+    ora = oracle.search_pixels(psiphi, st.times, vx, vy, px, py, op)      # 5.4e9 evaluations
+    for algo in (kb.ALGO_DIRECT, kb.ALGO_PRUNED, kb.ALGO_AUTO):
+        sp = kb.SearchParams(K=8, min_obs=5, min_lh=min_lh, algo=algo)
+        g = [o.cpu().numpy().reshape(H * W, -1) for o in kb.kbmod_search(d, st.times, vx, vy, sp)]
+        r = parity.compare_topk(oracle, psiphi, st.times, vx, vy, op, px, py, g, ora)
+        assert r["n_pix"] == H * W and r["n_exact_pix"] > 0.999 * H * W, r
+        used = kb.kbmod_search_stats(kb.kbmod_search.last_workspace)[3]
+        assert used == (kb.ALGO_DIRECT if algo == kb.ALGO_DIRECT or (algo == kb.ALGO_AUTO and not np.isfinite(min_lh))
+                        else kb.ALGO_PRUNED)
+        if not np.isfinite(min_lh):
+            assert r["n_entries"] == H * W * 8      # every pixel returns K results
 
 
 # ------------------------------------------------------------------------------------------- lightcurves
@@ -282,7 +289,7 @@ def test_search_pruned_random(kb, oracle, seed, T, H, W, K, sig, fon, min_lh, mi
     r = _search_and_compare(kb, oracle, d, st.times, vx, vy, sp)
     assert r["n_entries"] > 0
     ws = kb.kbmod_search.last_workspace
-    ev, nominal, launches, algo = kb.kbmod_search_stats(ws)
+    ev, nominal, launches, algo, _ = kb.kbmod_search_stats(ws)
     assert algo == kb.ALGO_PRUNED and nominal == H * W * nv and 0 < ev <= nominal
 
 
@@ -306,39 +313,151 @@ def test_search_pruned_equals_direct_decam_shaped(kb):
     for name, algo in (("direct", kb.ALGO_DIRECT), ("pruned", kb.ALGO_PRUNED)):
         sp = kb.SearchParams(K=8, min_obs=13, min_lh=10.0, algo=algo)
         outs[name] = [o.clone() for o in kb.kbmod_search(d, st.times, vx, vy, sp)]
-    ev, nominal, _, algo = kb.kbmod_search_stats(kb.kbmod_search.last_workspace)
+    ev, nominal, _, algo, _ = kb.kbmod_search_stats(kb.kbmod_search.last_workspace)
     assert algo == kb.ALGO_PRUNED and ev < 0.05 * nominal, (ev, nominal)
     for a, b in zip(outs["direct"], outs["pruned"]):
         assert torch.equal(a, b)
     assert int((outs["pruned"][2] >= 0).sum()) > 100  # the movers are found
 
 
-def test_search_config3_full_size_sampled(kb, oracle):
-    """BASELINE configs[2] at full size in the launch configuration bench.py times (AUTO -> pruned,
-    min_lh = 10, K = 8): oracle on random pixels, windows on injected movers, and the borders."""
+@pytest.fixture(scope="module")
+def c3(kb):
+    """BASELINE configs[2] (2048x4096x26) and its psi/phi stack on the GPU, shared by the full-size tests."""
     st = synth.config3_decam()
-    vx, vy = synth.config3_grid()
     d = _prep(kb, st)
+    return st, d, d.cpu().numpy()
+
+
+def protocol_pixels(st, rng, n_windows=64, n_mask_adjacent=1000, n_border=2000, mover_window=2, n_random=0):
+    """The pixel sample SURVEY 8c prescribes for the full-size configurations: all pixels of `n_windows` random 32x32
+    windows, windows on EVERY injected mover start, `n_mask_adjacent` pixels next to a statically masked pixel (bad
+    columns, disc edges), the four borders."""
+    T, H, W = st.img.shape
+    px, py = [], []
+    wy, wx = np.mgrid[0:32, 0:32]
+    for _ in range(n_windows):
+        x0, y0 = int(rng.integers(0, W - 32)), int(rng.integers(0, H - 32))
+        px.append(x0 + wx.reshape(-1)); py.append(y0 + wy.reshape(-1))
+    k = mover_window
+    my, mx = np.mgrid[-k:k + 1, -k:k + 1]
+    for m in st.movers:
+        px.append(np.clip(int(m["x0"]) + mx.reshape(-1), 0, W - 1))
+        py.append(np.clip(int(m["y0"]) + my.reshape(-1), 0, H - 1))
+    static = (st.mask != 0).all(axis=0)                      # masked in every epoch: discs and bad columns
+    grown = static.copy()
+    grown[1:, :] |= static[:-1, :]; grown[:-1, :] |= static[1:, :]
+    grown[:, 1:] |= static[:, :-1]; grown[:, :-1] |= static[:, 1:]
+    ay, ax = np.nonzero(grown & ~static)
+    pick = rng.choice(len(ay), min(n_mask_adjacent, len(ay)), replace=False)
+    px.append(ax[pick]); py.append(ay[pick])
+    bx, by = rng.integers(0, W, n_border), rng.integers(0, H, n_border)
+    px += [bx[:n_border // 2], np.zeros(n_border // 2, int), np.full(n_border // 2, W - 1), bx[n_border // 2:]]
+    py += [np.zeros(n_border // 2, int), by[:n_border // 2], by[n_border // 2:], np.full(n_border - n_border // 2, H - 1)]
+    px.append(np.array([0, W - 1, 0, W - 1])); py.append(np.array([0, 0, H - 1, H - 1]))
+    if n_random:
+        px.append(rng.integers(0, W, n_random)); py.append(rng.integers(0, H, n_random))
+    return np.concatenate(px).astype(np.int32), np.concatenate(py).astype(np.int32)
+
+
+def test_search_config3_full_size_protocol_mode_a(kb, oracle, c3):
+    """BASELINE configs[2] at full size in the launch configuration bench.py times (AUTO -> pruned, min_lh = 10,
+    K = 8), on the sample SURVEY 8c prescribes: 64 random 32x32 windows, 5x5 windows on all 200 mover starts, 1000
+    mask-adjacent pixels, the four borders, and pixels where the search returned something: > 10^5 start pixels x
+    all 8192 velocities in the oracle."""
+    st, d, psiphi = c3
+    vx, vy = synth.config3_grid()
     T, H, W = st.img.shape
     rng = np.random.default_rng(3)
-    px = [rng.integers(0, W, 6000), np.array([0, W - 1, 0, W - 1, 5, W - 6]), rng.integers(0, W, 500), np.zeros(250), np.full(250, W - 1)]
-    py = [rng.integers(0, H, 6000), np.array([0, 0, H - 1, H - 1, 7, H - 8]), np.concatenate([np.zeros(250), np.full(250, H - 1)]),
-          rng.integers(0, H, 250), rng.integers(0, H, 250)]
-    for m in st.movers[:60]:  # 5x5 windows on mover starts: where results actually are
-        wy, wx = np.mgrid[-2:3, -2:3]
-        px.append(np.clip(int(m["x0"]) + wx.reshape(-1), 0, W - 1))
-        py.append(np.clip(int(m["y0"]) + wy.reshape(-1), 0, H - 1))
-    # and 6000 pixels where the search returned something (the pixel LIST may come from anywhere; every expected
-    # value is the oracle's)
+    px, py = protocol_pixels(st, rng, n_random=20000)
     sp = kb.SearchParams(K=8, min_obs=13, min_lh=10.0, algo=kb.ALGO_AUTO)
-    has_y, has_x = np.nonzero(kb.kbmod_search(d, st.times, vx, vy, sp)[2][..., 0].cpu().numpy() >= 0)
+    out = kb.kbmod_search(d, st.times, vx, vy, sp)
+    ev, nominal, _, algo, _ = kb.kbmod_search_stats(kb.kbmod_search.last_workspace)
+    assert algo == kb.ALGO_PRUNED and nominal == H * W * len(vx) and ev < 0.05 * nominal
+    g = [o.cpu().numpy() for o in out]
+    # ... and 6000 pixels where the search returned something (the pixel LIST may come from anywhere; every expected
+    # value is the oracle's)
+    has_y, has_x = np.nonzero(g[2][..., 0] >= 0)
     pick = rng.choice(len(has_y), min(6000, len(has_y)), replace=False)
-    px.append(has_x[pick]); py.append(has_y[pick])
-    px, py = np.concatenate(px).astype(np.int32), np.concatenate(py).astype(np.int32)
+    px, py = np.concatenate([px, has_x[pick].astype(np.int32)]), np.concatenate([py, has_y[pick].astype(np.int32)])
+    assert len(px) >= 100_000
+    op = parity.oracle_params(oracle, sp)
+    ora = oracle.search_pixels(psiphi, st.times, vx, vy, px, py, op)
+    r = parity.compare_topk(oracle, psiphi, st.times, vx, vy, op, px, py, [a[py, px] for a in g], ora)
+    assert r["n_entries"] > 20000 and r["n_exact_pix"] > 0.999 * len(px), r
+    # recovery (PAPER.md L177 window: 5 px, 5 px/day): the best result near a bright injected mover is the mover
+    found = 0
+    bright = [m for m in st.movers if m["flux"] > 1500]
+    for m in bright:
+        x, y = int(m["x0"]), int(m["y0"])
+        v = g[2][max(y - 2, 0):y + 3, max(x - 2, 0):x + 3, 0]
+        l = g[0][max(y - 2, 0):y + 3, max(x - 2, 0):x + 3, 0]
+        if (v >= 0).any():
+            vb = v.reshape(-1)[np.argmax(np.where(v >= 0, l, -np.inf))]
+            found += int(abs(vx[vb] - m["vx"]) <= 5 and abs(vy[vb] - m["vy"]) <= 5)
+    # (the injected velocities are random, not grid points: a mover between grid velocities drifts off its nearest
+    # trajectory by a few pixels over three days; the paper itself recovers 22 of 26 known objects, L177)
+    assert found >= 0.6 * len(bright), (found, len(bright))
+
+
+def test_search_config3_full_size_mode_b_direct(kb, oracle, c3):
+    """SURVEY 8d mode (B): min_lh = -inf, every pixel returns K results, every trajectory gets the full filter --
+    the direct kernel at full size (2048x4096x26 x 8192 velocities) on > 10^4 sampled pixels incl. borders, mover
+    starts and mask-adjacent pixels."""
+    st, d, psiphi = c3
+    vx, vy = synth.config3_grid()
+    T, H, W = st.img.shape
+    px, py = protocol_pixels(st, np.random.default_rng(33), n_windows=4, n_mask_adjacent=500, n_border=1000, mover_window=1,
+                             n_random=3000)
+    assert len(px) >= 10_000
+    sp = kb.SearchParams(K=8, min_obs=13, min_lh=-np.inf, algo=kb.ALGO_AUTO)
     r = _search_and_compare(kb, oracle, d, st.times, vx, vy, sp, pixels=(px, py))
-    ev, nominal, _, algo = kb.kbmod_search_stats(kb.kbmod_search.last_workspace)
-    assert algo == kb.ALGO_PRUNED and nominal == H * W * len(vx)
-    assert r["n_entries"] > 20000, r
+    ev, nominal, _, algo, _ = kb.kbmod_search_stats(kb.kbmod_search.last_workspace)
+    assert algo == kb.ALGO_DIRECT and ev == nominal == H * W * len(vx)
+    assert r["n_exact_pix"] > 0.99 * len(px), r
+
+
+def test_search_paper_grid_full_size_sampled(kb, oracle, c3):
+    """The paper's own operating point (512 speed x 256 angle steps = 131072 velocities; L133: of order
+    10^12 trajectories per 2Kx4K stack) on the configs[2] stack: oracle on > 2000 sampled pixels x all velocities."""
+    st, d, psiphi = c3
+    vx, vy = synth.paper_grid()
+    assert len(vx) == 131072
+    T, H, W = st.img.shape
+    px, py = protocol_pixels(st, np.random.default_rng(34), n_windows=1, n_mask_adjacent=200, n_border=200, mover_window=0,
+                             n_random=500)
+    assert len(px) >= 2000
+    sp = kb.SearchParams(K=8, min_obs=13, min_lh=10.0, algo=kb.ALGO_AUTO)
+    r = _search_and_compare(kb, oracle, d, st.times, vx, vy, sp, pixels=(px, py))
+    ev, nominal, _, algo, _ = kb.kbmod_search_stats(kb.kbmod_search.last_workspace)
+    assert algo == kb.ALGO_PRUNED and nominal == H * W * 131072
+    assert r["n_exact_pix"] > 0.99 * len(px) and r["n_entries"] > 100, r
+
+
+def test_pipeline_host_batch_against_the_oracle_full_size(kb, oracle, c3):
+    """The call bench.py's e2e figure times, at full size: the HOST result arrays of kbmod_pipeline_host_batch (two
+    stacks: both arena halves) against the oracle on sampled pixels."""
+    import torch
+    st, d, psiphi = c3
+    vx, vy = synth.config3_grid()
+    T, H, W = st.img.shape
+    sp = kb.SearchParams(K=8, min_obs=13, min_lh=10.0)
+    pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
+    h_in = (pin(st.img), pin(st.var), pin(st.mask))
+    outs = [tuple(torch.empty((H, W, 8), dtype=dt).pin_memory() for dt in (torch.float32, torch.float32, torch.int32, torch.int32))
+            for _ in range(2)]
+    arena = torch.empty(2 * kb.kbmod_pipeline_host_arena_bytes_for(T, H, W, st.times, vx, vy, sp), dtype=torch.uint8, device="cuda")
+    kb.kbmod_pipeline_host_batch([h_in, h_in], st.psf, st.times, vx, vy, sp, outs, arena)
+    del arena
+    for a, b in zip(outs[0], outs[1]):
+        assert torch.equal(a, b)
+    px, py = protocol_pixels(st, np.random.default_rng(35), n_windows=2, n_mask_adjacent=300, n_border=400, mover_window=2,
+                             n_random=1000)
+    g = [o.numpy()[py, px] for o in outs[1]]
+    op = parity.oracle_params(oracle, sp)
+    # (the pipeline's own psi/phi stack is the same kernel's output as `d`: the prep parity tests cover it)
+    ora = oracle.search_pixels(psiphi, st.times, vx, vy, px, py, op)
+    r = parity.compare_topk(oracle, psiphi, st.times, vx, vy, op, px, py, g, ora)
+    assert r["n_entries"] > 1000 and r["n_exact_pix"] > 0.99 * len(px), r
 
 
 # ------------------------------------------------------------------------------------------- round-1 additions
@@ -432,23 +551,20 @@ def test_config5_full_size_coadd_and_refilter(kb, oracle):
 
 def test_search_config4_full_size_sampled(kb, oracle):
     """BASELINE configs[3] at full size (2048x4096x50, 256 x 128 velocities, K = 16, min_obs = 25) through the
-    AUTO -> pruned path at the paper's threshold: oracle on random pixels, the corners, and 3x3 windows on
-    injected mover starts (their fluxes are sub-threshold by construction: what is checked is parity)."""
+    AUTO -> pruned path at the paper's threshold: oracle on > 2x10^4 pixels (random windows, the borders,
+    mask-adjacent pixels and 3x3 windows on all 1000 injected mover starts; their fluxes are sub-threshold by
+    construction: what is checked is parity)."""
     st = synth.config4_heavy()
     vx, vy = synth.config4_grid()
     d = _prep(kb, st)
     T, H, W = st.img.shape
-    rng = np.random.default_rng(4)
-    px = [rng.integers(0, W, 1200), np.array([0, W - 1, 0, W - 1])]
-    py = [rng.integers(0, H, 1200), np.array([0, 0, H - 1, H - 1])]
-    for m in st.movers[:40]:
-        wy, wx = np.mgrid[-1:2, -1:2]
-        px.append(np.clip(int(m["x0"]) + wx.reshape(-1), 0, W - 1))
-        py.append(np.clip(int(m["y0"]) + wy.reshape(-1), 0, H - 1))
-    px, py = np.concatenate(px).astype(np.int32), np.concatenate(py).astype(np.int32)
+    # SURVEY 8c sample: 32x32 windows, 3x3 windows on all 1000 mover starts, mask-adjacent pixels, borders: > 2x10^4
+    px, py = protocol_pixels(st, np.random.default_rng(4), n_windows=8, n_mask_adjacent=500, n_border=1000, mover_window=1,
+                             n_random=1500)
+    assert len(px) >= 20_000
     sp = kb.SearchParams(K=16, min_obs=25, min_lh=10.0, algo=kb.ALGO_AUTO)
     r = _search_and_compare(kb, oracle, d, st.times, vx, vy, sp, pixels=(px, py))
-    ev, nominal, _, algo = kb.kbmod_search_stats(kb.kbmod_search.last_workspace)
+    ev, nominal, _, algo, _ = kb.kbmod_search_stats(kb.kbmod_search.last_workspace)
     assert algo == kb.ALGO_PRUNED and nominal == H * W * len(vx) and ev < 0.2 * nominal
     assert r["n_pix"] == len(px)
 
@@ -465,7 +581,7 @@ def test_search_pruned_degenerate_shapes(kb, oracle, T, H, W, nv, K):
     sp = kb.SearchParams(min_lh=0.5, min_obs=1, K=K, algo=kb.ALGO_PRUNED)
     r = _search_and_compare(kb, oracle, d, st.times, vx, vy, sp)
     assert r["n_pix"] == H * W
-    _, nominal, _, algo = kb.kbmod_search_stats(kb.kbmod_search.last_workspace)
+    _, nominal, _, algo, _ = kb.kbmod_search_stats(kb.kbmod_search.last_workspace)
     assert algo == kb.ALGO_PRUNED and nominal == H * W * nv
 
 
