@@ -5,6 +5,7 @@
 #include <stdarg.h>
 #include <string.h>
 
+#include <algorithm>
 #include <vector>
 
 #include "common.cuh"
@@ -194,7 +195,7 @@ struct kbmod_plan {
     // host blob of the device tables and where each table sits in it
     unsigned char* blob = nullptr;
     bool blob_pinned = false;
-    size_t blob_bytes = 0, b_off = 0, b_gvel = 0, b_gtbl = 0, b_maskx = 0, b_masky = 0, b_gfoot = 0;
+    size_t blob_bytes = 0, b_off = 0, b_order = 0, b_gvel = 0, b_gtbl = 0, b_maskx = 0, b_masky = 0, b_gfoot = 0;
     // workspace layout (all offsets 256-byte aligned)
     size_t w_stats = 0, w_tables = 0, w_keys = 0, w_s4 = 0, w_scratch = 0, scratch_bytes = 0, w_total = 0;
     cudaEvent_t uploaded = nullptr;  // recorded after the last upload from the blob: the blob may be freed after it
@@ -299,9 +300,30 @@ extern "C" int kbmod_plan_create(int T, int H, int W, const double* h_times, con
     pl->algo = algo;
     if (!pl->has_pruned) pl->pr = PrunedPlan();
 
+    // the order in which the direct kernel walks the velocities: neighbours in the list are neighbours in
+    // displacement space (bands of a few rows of the displacement at the epoch farthest from times[0], swept in x in
+    // alternating directions), so consecutive velocities of a warp touch overlapping cache lines.  Results do not
+    // depend on it (the top-K keys carry the velocity index).
+    std::vector<int32_t> order(n_vel);
+    {
+        int t_far = 0;
+        double best = -1.0;
+        for (int t = 0; t < T; ++t)
+            if (fabs(h_times[t] - h_times[0]) > best) { best = fabs(h_times[t] - h_times[0]); t_far = t; }
+        const int band = 6;
+        for (int v = 0; v < n_vel; ++v) order[v] = v;
+        auto key = [&](int v) {
+            const long long dx = hdx[(size_t)v * T + t_far], dy = hdy[(size_t)v * T + t_far];
+            const long long b = (dy >= 0 ? dy : dy - (band - 1)) / band;
+            return std::make_pair(b, (b & 1) ? -dx : dx);
+        };
+        std::stable_sort(order.begin(), order.end(), [&](int a, int b) { return key(a) < key(b); });
+    }
+
     // ---- the blob
     size_t o = 0;
     pl->b_off = o;   o = align256(o + off.size() * 4);
+    pl->b_order = o; o = align256(o + order.size() * 4);
     pl->b_gvel = o;  o = align256(o + pl->pr.gvel.size() * 4);
     pl->b_gtbl = o;  o = align256(o + pl->pr.gtbl.size());
     pl->b_maskx = o; o = align256(o + pl->pr.maskx.size() * 8);
@@ -320,6 +342,7 @@ extern "C" int kbmod_plan_create(int T, int H, int W, const double* h_times, con
     }
     memset(pl->blob, 0, pl->blob_bytes);
     if (!off.empty()) memcpy(pl->blob + pl->b_off, off.data(), off.size() * 4);
+    if (!order.empty()) memcpy(pl->blob + pl->b_order, order.data(), order.size() * 4);
     if (pl->has_pruned) {
         memcpy(pl->blob + pl->b_gvel, pl->pr.gvel.data(), pl->pr.gvel.size() * 4);
         memcpy(pl->blob + pl->b_gtbl, pl->pr.gtbl.data(), pl->pr.gtbl.size());
@@ -397,7 +420,8 @@ extern "C" int kbmod_plan_search(kbmod_plan* pl, const float* d_psiphi, float* d
     int launches = 2;  // s4_build + finalize
     if (pl->algo == KBMOD_ALGO_DIRECT) {
         kb_phase_mark(KB_PHASE_PLANES, st);
-        rc = kb_launch_search_direct(pl->TP, d_S4, pl->G, d_off, pl->W, pl->row_begin, pl->row_end, pl->n_vel, pl->P, d_keys, st);
+        rc = kb_launch_search_direct(pl->TP, d_S4, pl->G, d_off, (const int*)(ws + pl->w_tables + pl->b_order), pl->W,
+                                     pl->row_begin, pl->row_end, pl->n_vel, pl->P, d_keys, st);
         if (rc) return rc;
         if (n_rows > 0) ++launches;
         kb_phase_mark(KB_PHASE_BOUND, st);  // the direct kernel is gather + filter + top-K in one: reported as phase 1
@@ -488,7 +512,7 @@ extern "C" size_t kbmod_search_workspace_bytes(int T, int H, int W, int n_vel, c
     // tables: offsets + the pruned plan's tables at their maximum group count
     const size_t ngm = std::min((size_t)n_vel, 2 * (((size_t)n_vel + 15) / 16) + 16);
     const size_t tiles_x = (W + 63) / 64, tiles_y = (H + 31) / 32;
-    size_t tb = align256((size_t)n_vel * kb_tp4(TP) * 4) + align256(ngm * 16 * 4) + align256(ngm * (size_t)T * (16 * 4 + 32)) +
+    size_t tb = align256((size_t)n_vel * kb_tp4(TP) * 4) + align256((size_t)n_vel * 4) + align256(ngm * 16 * 4) + align256(ngm * (size_t)T * (16 * 4 + 32)) +
                 align256(ngm * tiles_x * 8) + align256(ngm * tiles_y * 8) + align256(ngm * 4);
     o = align256(o + std::max<size_t>(tb, 256));
     o = align256(o + (size_t)H * W * K * 8);

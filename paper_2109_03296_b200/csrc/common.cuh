@@ -320,8 +320,9 @@ int kb_launch_unfiltered_lh(int TP, const int32_t* d_vel_idx, const void* d_S4, 
                             int row_begin, int n_rows, int K, int n_vel, float* d_lh_raw, cudaStream_t st);
 int kb_write_stats(unsigned long long* d_stats, unsigned long long nominal, unsigned long long launches,
                    unsigned long long algo, unsigned long long evaluated_all, cudaStream_t st);
-int kb_launch_search_direct(int TP, const void* d_S4, const S4Geom& G, const int* d_off, int W, int row_begin,
-                            int row_end, int n_vel, const DevParams& P, unsigned long long* d_keys, cudaStream_t st);
+int kb_launch_search_direct(int TP, const void* d_S4, const S4Geom& G, const int* d_off, const int* d_order, int W,
+                            int row_begin, int row_end, int n_vel, const DevParams& P, unsigned long long* d_keys,
+                            cudaStream_t st);
 
 // ---------------------------------------------------------------------------------------------
 // launchers (one per .cu file); all return a KBMOD_* status
