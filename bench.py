@@ -300,10 +300,11 @@ def run_ours(args):
         seg["coadd"].append(e[2].elapsed_time(e[3]))
     stats = kb.kbmod_search_stats(ws)  # [evaluated, nominal, launches, algo]
     smem_gbs = {b: kb.kbmod_measure_smem_gbs(b) for b in (4, 16)}  # after the timed region
+    issue = {n: kb.kbmod_measure_issue_rate(i) for i, n in enumerate(("FMNMX", "IADD3", "FADD", "FMNMX+IADD3_exchange"))}
     plan_info = kb.Plan(T, H, W, st.times, vx, vy, sp).info()           # host-only: what the planner staged / skipped
     R = dict(torch=torch, dist=dist, kb=kb, rank=rank, world=world, dev=dev, st=st, vx=vx, vy=vy, pd=pd, sp=sp,
              desc=desc, evals=evals, total_ms=total_ms, seg=seg, stats=stats, clocks=clocks, peaks=peaks, phases=phases,
-             n_cand=n_cand, out=out, smem_gbs=smem_gbs, plan_info=plan_info, psiphi=psiphi, ws=ws, extras={})
+             n_cand=n_cand, out=out, smem_gbs=smem_gbs, issue=issue, plan_info=plan_info, psiphi=psiphi, ws=ws, extras={})
     # ---- more timed records on the same box, after the headline region (rank 0 of a 1-GPU run, default workload)
     if rank == 0 and world == 1 and args.workload == "c3" and not args.no_extras and args.algo == "auto" and args.min_lh == 10.0:
         R["extras"]["mode_b"] = time_search(R, "configs[2], mode (B): min_lh = -inf, every trajectory filtered (SURVEY 8d)", st, psiphi,
@@ -528,6 +529,7 @@ def report(R, args):
                          d2h_bytes_per_step=d2h, ms_per_step=e2e_max, steps=e2e_steps,
                          matches_resident_run=same, api="kbmod_pipeline_host_batch (prep + search per stack; pinned host buffers; copies overlap the neighbouring searches)"),
                 gpu_launches=args.steps * (T + int(launches) + 1), clocks=R["clocks"], peaks_source=peaks["source"],
+                issue_rates_warp_instr_per_clk_per_sm=R["issue"],
                 planner=dict(n_groups=pi["n_groups"], staged_bytes_per_eval=pi["staged_bytes_per_eval"],
                              canvas=pi["canvas"], workspace_gb=pi["workspace_bytes"] / 1e9),
                 **R["extras"])

@@ -319,6 +319,13 @@ int kbmod_pipeline_host_batch(int n_stacks, const float* const* h_img, const flo
  * SMs x 128 B/clk x SM clock. */
 int kbmod_measure_smem_gbs(int bytes_per_lane, void* d_scratch4, double* h_gbs, void* stream);
 
+/* Measurement helper: issue rate, in warp-instructions per SM clock per SM, of op = 0 FMNMX, 1 IADD3 (two register
+ * operands), 2 FADD, 3 an alternative compare-exchange (FMNMX + three-register IADD3 recovering the maximum from the
+ * bit patterns, plus one FADD that keeps the benchmark's chain alive).  On sm_100a FMNMX issues at 2 per clock per SM,
+ * IADD3 and FADD at 4; the alternative exchange is no faster than two FMNMX.
+ * Synchronises; d_scratch4 = 4 bytes of caller-owned device memory. */
+int kbmod_measure_issue_rate(int op, void* d_scratch4, double* h_rate, void* stream);
+
 const char* kbmod_last_error(void); /* thread-local, never NULL */
 int kbmod_version(void);            /* 10000*major + 100*minor + patch */
 

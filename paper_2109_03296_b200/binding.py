@@ -51,6 +51,7 @@ SIGNATURES = {
     "kbmod_pipeline_host": (_I, [_P, _P, _P, _I, _I, _I, _P, _I, _I, _P, _P, _P, _I, _P, _P, _P, _P, _P, _P, _Z, _P]),
     "kbmod_pipeline_host_batch": (_I, [_I, _P, _P, _P, _I, _I, _I, _P, _I, _I, _P, _P, _P, _I, _P, _P, _P, _P, _P, _P, _Z, _P]),
     "kbmod_measure_smem_gbs": (_I, [_I, _P, _P, _P]),
+    "kbmod_measure_issue_rate": (_I, [_I, _P, _P, _P]),
     "kbmod_last_error": (C.c_char_p, []),
     "kbmod_version": (_I, []),
 }
@@ -547,6 +548,15 @@ def kbmod_measure_smem_gbs(bytes_per_lane: int = 4, stream=None) -> float:
     out = C.c_double(0.0)
     scratch = torch.zeros(4, dtype=torch.uint8, device="cuda")
     _check(lib().kbmod_measure_smem_gbs(bytes_per_lane, _dev(scratch), C.byref(out), _stream(stream)))
+    return float(out.value)
+
+
+def kbmod_measure_issue_rate(op: int, stream=None) -> float:
+    """Warp-instructions per clock per SM of op = 0 FMNMX, 1 IADD3, 2 FADD, 3 the kernels' compare-exchange."""
+    import torch
+    out = C.c_double(0.0)
+    scratch = torch.zeros(4, dtype=torch.uint8, device="cuda")
+    _check(lib().kbmod_measure_issue_rate(op, _dev(scratch), C.byref(out), _stream(stream)))
     return float(out.value)
 
 

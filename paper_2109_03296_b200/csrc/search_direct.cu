@@ -8,8 +8,7 @@
 // pruned kernel must agree with bit for bit.
 //
 // Instructions per trajectory at T = 26, about 560 (round 1: 1600): 7 offset loads + 26 x (IMAD.WIDE + LDG.128 + IADD)
-// gather, 147 x (FMNMX + IADD3) sort (the half-rate ALU pipe takes the FMNMX, the full-rate integer add recovers the
-// maximum), 26 STS + 3 LDS rank lookup, 26 x 5 clip-and-sum.  With that the kernel is no longer issue-bound: ncu
+// gather, 147 x 2 FMNMX sort (half-rate ALU pipe), 26 STS + 3 LDS rank lookup, 26 x 5 clip-and-sum.  With that the kernel is no longer issue-bound: ncu
 // shows the L1 data path at 80 % and L2 at 68 % of their peaks (profiles/r2_search_direct_kernel_full.md).
 #include <algorithm>
 

@@ -73,3 +73,93 @@ extern "C" int kbmod_measure_smem_gbs(int bytes_per_lane, void* d_scratch4, doub
     *h_gbs = best;
     return KBMOD_OK;
 }
+
+// ---------------------------------------------------------------------------------------------
+// Issue rate of a few opcodes (warp-instructions per clock per SM), measured the same way: 8 independent chains per
+// thread, 32 warps per SM, nothing else in the loop.  What it is for: on sm_100a FMNMX (like LOP3, IMAD, IMNMX) issues
+// on the half-rate ALU pipe, IADD3 (two register operands) and FADD at the full rate.  An exchange built from one FMNMX
+// and a three-register IADD3 (maximum = a + b - min on the bit patterns) was tried for that reason and runs at 0.83
+// exchanges per clock per SM against 0.99 for two FMNMX: op 3 keeps the measurement.
+namespace {
+
+constexpr int IR_CHAINS = 8, IR_ITERS = 4096;
+
+template <int OP>
+__global__ void __launch_bounds__(1024) issue_rate_kernel(int iters, float a0, unsigned int* __restrict__ sink) {
+    float x[IR_CHAINS], y[IR_CHAINS];
+    int ix[IR_CHAINS];
+#pragma unroll
+    for (int i = 0; i < IR_CHAINS; ++i) {
+        x[i] = a0 + threadIdx.x * 1e-3f + i;
+        y[i] = 2.0f * a0 - i;
+        ix[i] = threadIdx.x + i;
+    }
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int i = 0; i < IR_CHAINS; ++i) {
+            if (OP == 0) {  // two FMNMX (min, max on different chains so that ptxas cannot fuse them into FMNMX3)
+                asm volatile("min.f32 %0, %0, %1;" : "+f"(x[i]) : "f"(y[(i + 1) % IR_CHAINS]));
+                asm volatile("max.f32 %0, %0, %1;" : "+f"(y[i]) : "f"(x[(i + 3) % IR_CHAINS]));
+            }
+            if (OP == 1) {  // two integer adds
+                asm volatile("add.s32 %0, %0, %1;" : "+r"(ix[i]) : "r"(ix[(i + 1) % IR_CHAINS]));
+                asm volatile("add.s32 %0, %0, %1;" : "+r"(ix[(i + 2) % IR_CHAINS]) : "r"(it));
+            }
+            if (OP == 2) {  // two FADD
+                asm volatile("add.f32 %0, %0, %1;" : "+f"(x[i]) : "f"(y[(i + 1) % IR_CHAINS]));
+                asm volatile("add.f32 %0, %0, %1;" : "+f"(y[i]) : "f"(x[(i + 3) % IR_CHAINS]));
+            }
+            if (OP == 3) {  // the alternative compare-exchange: FMNMX + (a + b - min) on the bit patterns
+                const float lo = fminf(x[i], y[i]);
+                y[i] = __int_as_float(__float_as_int(x[i]) + __float_as_int(y[i]) - __float_as_int(lo));
+                x[i] = lo + a0;  // keeps the chain alive (one FADD)
+            }
+        }
+    }
+    float s = 0.0f;
+    int si = 0;
+#pragma unroll
+    for (int i = 0; i < IR_CHAINS; ++i) {
+        s += x[i] + y[i];
+        si += ix[i];
+    }
+    if (s + (float)si == a0 * 7.25f) sink[0] = (unsigned int)si;
+}
+
+}  // namespace
+
+// op: 0 = FMNMX, 1 = IADD3, 2 = FADD, 3 = the alternative compare-exchange (FMNMX + three-register IADD3 + FADD).  *h_rate = warp-instructions of the
+// loop body per SM clock (max SM clock) per SM: 2 per chain step for op 0-2, 3 for op 3.
+extern "C" int kbmod_measure_issue_rate(int op, void* d_scratch4, double* h_rate, void* stream) {
+    KB_REQUIRE(h_rate && d_scratch4, KBMOD_ERR_INVALID_ARG, "NULL argument");
+    KB_REQUIRE(op >= 0 && op <= 3, KBMOD_ERR_INVALID_ARG, "op = %d must be 0..3", op);
+    cudaStream_t st = (cudaStream_t)stream;
+    int dev = 0, n_sm = 0, khz = 0;
+    KB_CUDA(cudaGetDevice(&dev));
+    KB_CUDA(cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev));
+    KB_CUDA(cudaDeviceGetAttribute(&khz, cudaDevAttrClockRate, dev));
+    cudaEvent_t e0, e1;
+    KB_CUDA(cudaEventCreate(&e0));
+    KB_CUDA(cudaEventCreate(&e1));
+    unsigned int* sink = (unsigned int*)d_scratch4;
+    double best = 0.0;
+    for (int rep = 0; rep < 4; ++rep) {
+        KB_CUDA(cudaEventRecord(e0, st));
+        if (op == 0) issue_rate_kernel<0><<<n_sm * 2, 1024, 0, st>>>(IR_ITERS, 1.0f, sink);
+        if (op == 1) issue_rate_kernel<1><<<n_sm * 2, 1024, 0, st>>>(IR_ITERS, 1.0f, sink);
+        if (op == 2) issue_rate_kernel<2><<<n_sm * 2, 1024, 0, st>>>(IR_ITERS, 1.0f, sink);
+        if (op == 3) issue_rate_kernel<3><<<n_sm * 2, 1024, 0, st>>>(IR_ITERS, 1.0f, sink);
+        KB_CUDA(cudaEventRecord(e1, st));
+        KB_CUDA(cudaEventSynchronize(e1));
+        float ms = 0.0f;
+        KB_CUDA(cudaEventElapsedTime(&ms, e0, e1));
+        const double winst = (double)n_sm * 2 * 32 * (double)IR_ITERS * IR_CHAINS * (op == 3 ? 3 : 2);
+        const double clk = (double)ms * 1e-3 * (double)khz * 1e3;
+        if (rep > 0) best = fmax(best, winst / clk / n_sm);
+    }
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    KB_CUDA(cudaGetLastError());
+    *h_rate = best;
+    return KBMOD_OK;
+}
