@@ -27,6 +27,7 @@ constexpr int SD_THREADS = SD_BX * SD_BY;
 // overlapping lines; measured on configs[2], mode (B): 1 / 2 / 3 / 4 blocks per SM take 6.25 / 3.65 / 3.03 / 2.91 s
 // (latency hiding beats the L1 reuse fewer warps would gain), against 3.05-3.24 s in list order.
 constexpr int SD_BLOCKS_PER_SM = KB_SD_BLOCKS;
+constexpr int SD_SBW = 8, SD_SBH = 64;  // super-block of tiles: 8 x 32 = 256 pixels wide, 64 x 4 = 256 rows tall
 
 template <int TP>
 __global__ void __launch_bounds__(SD_THREADS)
@@ -41,8 +42,17 @@ search_direct_kernel(const float4* __restrict__ S4, const __grid_constant__ S4Ge
     const int K = P.K;
     constexpr int TP4 = (TP + 3) & ~3;
     const int tiles_x = (W + SD_BX - 1) / SD_BX, tiles_y = (row_end - row_begin + SD_BY - 1) / SD_BY;
-    for (int tile = blockIdx.x; tile < tiles_x * tiles_y; tile += gridDim.x) {
-        const int ty = tile / tiles_x, tx = tile - ty * tiles_x;
+    // tiles are numbered in compact super-blocks of SD_SBW x SD_SBH tiles (256 x 256 pixels, about one grid's worth), not
+    // along whole image rows: the blocks running at one time then cover a square patch, whose displaced copies (blocks
+    // drift apart by tens of velocities) still fit L2; in row-major order the same drift spread a 2048-pixel-wide strip
+    // over several hundred MB and the kernel read 12.6 TB from DRAM per search.
+    const int sb_per_row = (tiles_x + SD_SBW - 1) / SD_SBW;
+    const int n_sb = sb_per_row * ((tiles_y + SD_SBH - 1) / SD_SBH);
+    for (int slot = blockIdx.x; slot < n_sb * SD_SBW * SD_SBH; slot += gridDim.x) {
+        const int sb = slot / (SD_SBW * SD_SBH), in = slot - sb * (SD_SBW * SD_SBH);
+        const int sby = sb / sb_per_row, sbx = sb - sby * sb_per_row;
+        const int ty = sby * SD_SBH + in / SD_SBW, tx = sbx * SD_SBW + in % SD_SBW;
+        if (tx >= tiles_x || ty >= tiles_y) continue;  // block-uniform
         const int x0 = tx * SD_BX + threadIdx.x;
         const int y0 = row_begin + ty * SD_BY + threadIdx.y;
         const bool active = x0 < W && y0 < row_end;
