@@ -10,7 +10,7 @@ independent CCD stack per rank (replicas: 2580 independent per-CCD se
 no data-path collective, "scaling": "weak".
 
   python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload c3|c2|c1|c4]
-                  [--min-lh X] [--algo auto|direct|pruned]
+                  [--min-lh X] [--algo auto|direct|pruned] [--shard replicas|rows] [--no-extras]
 `--impl reference` times the oracle (oracle/, plain C, double) on the host cores on a bounded sample
 of the same workload; it is the only leg besides `cpu_baseline` that executes anything under oracle/.
 """
@@ -215,7 +215,7 @@ def run_reference(args):
 #                    SURVEY 8(d) counted 8 B per evaluation (psi and phi as float32): reported beside it.
 # dram__bytes_read.sum + dram__bytes_write.sum per step of the dominant kernel from the committed ncu --set full
 # capture (profiles/); None = not captured for this kernel
-TRAFFIC = {"bound_phase_kernel": 11.6e9, "search_direct_kernel": 1.78e12}  # bytes per step: profiles/r2_launches.md, r2_search_direct_kernel_full.md
+TRAFFIC = {"bound_phase_kernel": 11.6e9, "search_direct_kernel": 11.7e12}  # bytes per step: profiles/r2_launches.md, r2_search_direct_kernel_full.md
 CE_COUNT = {4: 5, 5: 9, 8: 19, 10: 32, 12: 42, 16: 63, 20: 103, 24: 132, 26: 147, 28: 162, 32: 191, 40: 305,
             48: 384, 50: 403, 56: 464, 64: 543}
 N_SM = 148
@@ -241,7 +241,10 @@ def run_ours(args):
     peaks = load_peaks()
     dev = torch.device("cuda", local)
 
-    st, vx, vy, pd, desc = make_workload(args.workload, seed_shift=100 * rank)  # one CCD stack per rank
+    shard_rows = args.shard == "rows" and world > 1
+    # replicas (default): one CCD stack per rank.  --shard rows: ONE stack, every rank holds all of it and searches its
+    # band of start rows; the bands' results concatenate, no collective
+    st, vx, vy, pd, desc = make_workload(args.workload, seed_shift=0 if shard_rows else 100 * rank)
     T, H, W = st.img.shape
     algo = dict(auto=kb.ALGO_AUTO, direct=kb.ALGO_DIRECT, pruned=kb.ALGO_PRUNED)[args.algo]
     sp = kb.SearchParams(K=pd["K"], min_obs=pd["min_obs"], min_lh=args.min_lh, algo=algo)
@@ -251,9 +254,14 @@ def run_ours(args):
     # inputs resident in HBM before the timed region
     img, var, mask = (torch.from_numpy(a).to(dev) for a in (st.img, st.var, st.mask))
     psiphi = torch.empty((T, H, W, 2), dtype=torch.float32, device=dev)
-    out = tuple(torch.empty((H, W, sp.K), dtype=dt, device=dev)
+    rows = row_band(rank, world, H) if shard_rows else None
+    n_rows = H if rows is None else rows[1] - rows[0]
+    out = tuple(torch.empty((n_rows, W, sp.K), dtype=dt, device=dev)
                 for dt in (torch.float32, torch.float32, torch.int32, torch.int32))
-    ws = torch.empty(max(256, kb.kbmod_search_workspace_bytes_for(T, H, W, st.times, vx, vy, sp)), dtype=torch.uint8, device=dev)
+    ws = torch.empty(max(256, kb.kbmod_search_workspace_bytes_for(T, H, W, st.times, vx, vy, sp, rows=rows)), dtype=torch.uint8,
+                     device=dev)
+    if shard_rows:
+        evals = float(H) * W * n_vel * T / world  # per rank; whole_job_value multiplies by world
     n_cand = min(100_000, H * W)  # (a6) candidate list: configs[4]'s recipe
     cx0, cy0, cvx, cvy = (torch.from_numpy(a).to(dev) for a in synth.config5_trajectories(4 + rank, H, W, n_cand))
 
@@ -266,7 +274,7 @@ def run_ours(args):
         e[0].record()
         kb.kbmod_prepare_psi_phi(img, var, mask, st.psf, out=psiphi)
         e[1].record()
-        kb.kbmod_search(psiphi, st.times, vx, vy, sp, out=out, workspace=ws)
+        kb.kbmod_search(psiphi, st.times, vx, vy, sp, out=out, workspace=ws, rows=rows)
         e[2].record()
         kb.kbmod_coadd_stamps_filtered(img, mask, st.times, cx0, cy0, cvx, cvy, 10)  # (a6) + the moment filter (L141)
         e[3].record()
@@ -301,10 +309,10 @@ def run_ours(args):
     stats = kb.kbmod_search_stats(ws)  # [evaluated, nominal, launches, algo]
     smem_gbs = {b: kb.kbmod_measure_smem_gbs(b) for b in (4, 16)}  # after the timed region
     issue = {n: kb.kbmod_measure_issue_rate(i) for i, n in enumerate(("FMNMX", "IADD3", "FADD", "FMNMX+IADD3_exchange"))}
-    plan_info = kb.Plan(T, H, W, st.times, vx, vy, sp).info()           # host-only: what the planner staged / skipped
+    plan_info = kb.Plan(T, H, W, st.times, vx, vy, sp, rows=rows).info()  # host-only: what the planner staged / skipped
     R = dict(torch=torch, dist=dist, kb=kb, rank=rank, world=world, dev=dev, st=st, vx=vx, vy=vy, pd=pd, sp=sp,
              desc=desc, evals=evals, total_ms=total_ms, seg=seg, stats=stats, clocks=clocks, peaks=peaks, phases=phases,
-             n_cand=n_cand, out=out, smem_gbs=smem_gbs, issue=issue, plan_info=plan_info, psiphi=psiphi, ws=ws, extras={})
+             n_cand=n_cand, out=out, shard_rows=shard_rows, rows=rows, smem_gbs=smem_gbs, issue=issue, plan_info=plan_info, psiphi=psiphi, ws=ws, extras={})
     # ---- more timed records on the same box, after the headline region (rank 0 of a 1-GPU run, default workload)
     if rank == 0 and world == 1 and args.workload == "c3" and not args.no_extras and args.algo == "auto" and args.min_lh == 10.0:
         R["extras"]["mode_b"] = time_search(R, "configs[2], mode (B): min_lh = -inf, every trajectory filtered (SURVEY 8d)", st, psiphi,
@@ -316,6 +324,7 @@ def run_ours(args):
         del img, var, mask, psiphi, ws
         R["psiphi"] = R["ws"] = None
         torch.cuda.empty_cache()
+        R["extras"]["configs2_without_star_residuals"] = time_clean(R)
         R["extras"]["configs3_heavy"] = time_heavy(R)
     return R
 
@@ -355,6 +364,8 @@ def time_search(R, what, st, psiphi, vx, vy, pd, min_lh, steps, warmup):
         rec["roofline"] = dict(bound="issue", kernel="search_direct_kernel", achieved=winst / (kern_ms * 1e-3) / 1e12,
                                peak=peak / 1e12, unit="Twarp-instr/s", frac=winst / (kern_ms * 1e-3) / peak,
                                warp_instr_per_trajectory=DIRECT_WARP_INSTR_PER_TRAJ[tp], kernel_ms=kern_ms,
+                               traffic=TRAFFIC["search_direct_kernel"] if T == 26 and len(vx) == 8192 else None,
+                               note="issue slots are not what binds this kernel: the L1 / L2 / DRAM path is (profiles/)",
                                source="smsp__inst_executed per trajectory from profiles/r2_search_direct_kernel_full.md")
     del ws, out
     return rec
@@ -386,6 +397,23 @@ def time_postfilter(R):
     return out
 
 
+def time_clean(R):
+    """How much the headline depends on the synthetic artefacts: the configs[2] recipe WITHOUT the 500 star residuals
+    (cosmic rays, masks and movers kept).  The bound phase does the same work on any data; the survivors, and with
+    them the exact phase, are what the artefacts drive."""
+    torch, kb = R["torch"], R["kb"]
+    st = synth.decam_stack(2, (7, 6, 7, 6), n_stars=0, name="config3_no_stars")
+    vx, vy = synth.config3_grid()
+    img, var, mask = (torch.from_numpy(a).to(R["dev"]) for a in (st.img, st.var, st.mask))
+    psiphi = kb.kbmod_prepare_psi_phi(img, var, mask, st.psf)
+    del img, var, mask
+    rec = time_search(R, "configs[2] recipe without the star residuals, min_lh = 10", st, psiphi, vx, vy, dict(K=8, min_obs=13), 10.0,
+                      steps=2, warmup=1)
+    del psiphi
+    torch.cuda.empty_cache()
+    return rec
+
+
 def time_heavy(R):
     """BASELINE configs[3] (2048x4096x50, 256 x 128 velocities, K = 16): prep + search, one warm-up and one timed pass."""
     torch, kb = R["torch"], R["kb"]
@@ -415,6 +443,11 @@ def max_over_ranks(ms_local: float, dist, device, world: int) -> float:
     if world > 1:
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
     return float(t.item())
+
+
+def row_band(rank: int, world: int, H: int):
+    """Start rows [begin, end) of `rank` when one stack is sharded over `world` ranks by row bands."""
+    return H * rank // world, H * (rank + 1) // world
 
 
 def whole_job_value(evals_per_rank: float, world: int, ms_per_step: float) -> float:
@@ -456,7 +489,7 @@ def report(R, args):
     # max over ranks of the device time of the timed region
     total_ms = max_over_ranks(R["total_ms"], dist, R["dev"], world)
     e2e_steps = max(2, min(args.steps, 4))
-    e2e_ms, h2d, d2h, same = run_e2e(R, e2e_steps)
+    e2e_ms, h2d, d2h, same = run_e2e(R, e2e_steps) if not R["shard_rows"] else (float("nan"), 0, 0, False)
     e2e_max = max_over_ranks(e2e_ms, dist, R["dev"], world)
     if rank != 0:
         return
@@ -513,13 +546,16 @@ def report(R, args):
         r, cores, sample, _ = smp.step(12.0)
         cpu = dict(value=r, unit=UNIT, cores=cores, kind="oracle", sample=sample, value_one_core=smp.one_core(), cpu=cpu_model())
     line = dict(metric=METRIC, value=value, unit=UNIT, n_gpus=world, steps=args.steps, warmup=args.warmup,
-                ms_per_step=ms_per_step, higher_is_better=True, scaling="weak", vs_baseline=None, dtype="f32",
+                ms_per_step=ms_per_step, higher_is_better=True, scaling="strong" if R["shard_rows"] else "weak", vs_baseline=None,
+                dtype="f32",
                 data="synthetic",
                 config=dict(workload=R["desc"], min_lh=args.min_lh, min_obs=sp.min_obs, sigma_g="on",
                             algo={1: "direct", 2: "pruned"}.get(algo_used, "?"), coadd_candidates=R["n_cand"],
                             l2=("inputs larger than L2 (psi/phi stack %.2f GB)" % (T * H * W * 8 / 1e9)) if T * H * W * 8 > 2.6e8 else
                                "inputs SMALLER than L2 and no flush: a parity-test configuration, not a cold-cache measurement",
-                            multi_gpu="one independent CCD stack per rank, no collective" if world > 1 else "single GPU",
+                            multi_gpu=("one CCD stack sharded by start-row bands, whole stack on every rank, results concatenate, "
+                                       "no collective" if R["shard_rows"] else
+                                       "one independent CCD stack per rank, no collective") if world > 1 else "single GPU",
                             host_plan="velocity grouping / staging geometry cached after the first (warm-up) step: same grid and times"),
                 segments_ms={k: float(np.mean(v)) for k, v in R["seg"].items()},
                 evaluated_fraction=evaluated / max(1, nominal), trajectories_reaching_min_lh=reached,
@@ -545,6 +581,8 @@ def main():
     ap.add_argument("--workload", default="c3", choices=["c1", "c2", "c3", "c4", "paper"])
     ap.add_argument("--min-lh", type=float, default=10.0, dest="min_lh")
     ap.add_argument("--algo", default="auto", choices=["auto", "direct", "pruned"])
+    ap.add_argument("--shard", default="replicas", choices=["replicas", "rows"],
+                    help="N > 1: independent CCD stacks per rank (default) or one stack sharded by start-row bands")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-extras", action="store_true", help="skip the mode-B / paper-grid / configs[3] / post-filter records")
     args = ap.parse_args()

@@ -48,6 +48,20 @@ def test_two_rank_gloo_replicas(tmp_path):
     assert recs[0]["checksum"] != recs[1]["checksum"]                   # one independent stack per rank
 
 
+def test_row_bands_partition_the_image():
+    """--shard rows: the bands of the ranks tile [0, H) exactly, for any world size."""
+    sys.path.insert(0, ROOT)
+    import bench
+    for H in (1, 7, 64, 4096, 4097):
+        for world in (1, 2, 3, 4, 8):
+            bands = [bench.row_band(r, world, H) for r in range(world)]
+            assert bands[0][0] == 0 and bands[-1][1] == H
+            assert all(a[1] == b[0] for a, b in zip(bands[:-1], bands[1:]))
+            assert max(b[1] - b[0] for b in bands) - min(b[1] - b[0] for b in bands) <= 1
+    vx = bench.whole_job_value(100.0, 4, 1000.0)
+    assert vx == 400.0   # per-rank evaluations x ranks / seconds
+
+
 def test_reference_arm_runs_on_rank0_only():
     env = dict(os.environ, RANK="1", WORLD_SIZE="2")
     out = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--workload", "c1",
