@@ -455,7 +455,7 @@ extern "C" int kbmod_plan_unfiltered_lh(const kbmod_plan* pl, const void* d_work
     KB_REQUIRE(pl && d_workspace && d_vel_idx && d_lh_raw, KBMOD_ERR_INVALID_ARG, "NULL argument");
     const char* ws = (const char*)d_workspace;
     return kb_launch_unfiltered_lh(pl->TP, d_vel_idx, ws + pl->w_s4, pl->G, (const int*)(ws + pl->w_tables + pl->b_off),
-                                   pl->W, pl->row_begin, pl->row_end - pl->row_begin, pl->P.K, pl->n_vel, d_lh_raw,
+                                   pl->W, pl->row_begin, pl->row_end - pl->row_begin, pl->P.K, pl->n_vel, pl->P.filter_on, d_lh_raw,
                                    (cudaStream_t)stream);
 }
 

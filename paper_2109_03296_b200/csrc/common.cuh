@@ -175,13 +175,19 @@ __device__ __forceinline__ int kb_score_lightcurve(const float (&psi)[TP], const
 }
 
 // ---------------------------------------------------------------------------------------------
-// The search kernels' working copy of the psi/phi stack ("S4", built by s4_build_kernel at the start of every
-// kbmod_search): one float4 per pixel of a zero-padded canvas,
-//     (psi, phi, f, valid)   valid pixel:   f = kb_filter_value(psi, phi), valid = integer 1 (as bits)
-//                            invalid pixel, padding, and the extra plane T: (0, 0, +inf, 0)
+// The search kernels' working copy of the psi/phi stack (the "canvas", built by s4_build_kernel at the start of
+// every kbmod_search): one float2 per pixel of a padded canvas,
+//     (f, m)   valid pixel:   f = kb_filter_value(psi, phi), the value the filter sorts and clips;
+//                             m = MINUS the denominator f was divided by: -phi, or -sqrt(phi) with filter_on
+//              invalid pixel, padding, and the extra plane T: (+inf, +0)
 // padded by the largest displacement of the velocity list on each side (clamped to the image size), so a
-// trajectory sample is ONE 16-byte load at  base(x0, y0) + off[v][t]  with no bounds test: off-image samples land
+// trajectory sample is ONE 8-byte load at  base(x0, y0) + off[v][t]  with no bounds test: off-image samples land
 // in the padding and read "invalid".  Epochs t >= T of the padded count TP point into plane T.
+// The kept sums are accumulated from these two numbers (reading R25): sum psi as fma(f, -m, sum) -- f |m| is
+// psi up to two float32 roundings (1.2e-7 relative, against the 1e-4 the results are held to) -- and sum phi as
+// sum - m, or fma(m, m, sum) with filter_on.  The sign bit of m is the valid flag, so counting the valid samples
+// costs one shift-add per sample.  A warp's 32 samples of one epoch are 256 contiguous bytes (two or three lines)
+// instead of the 512 of a (psi, phi, f, valid) cell, and a lightcurve occupies 2 x T registers instead of 3 x T.
 struct S4Geom {
     int Wp, Hp;        // padded canvas
     int pxn, pyn;      // padding on the low-x / low-y side (image pixel (x, y) sits at (x + pxn, y + pyn))
@@ -192,10 +198,9 @@ __host__ __device__ inline int kb_tp4(int TP) { return (TP + 3) & ~3; }
 // gather the TP samples of the trajectory that starts at canvas index `base`; offrow = this velocity's row of the
 // offset table (kb_tp4(TP) entries, 16-byte aligned).  n = number of valid samples.
 template <int TP>
-__device__ __forceinline__ void kb_gather_s4(const float4* __restrict__ S4, unsigned int base,
-                                             const int4* __restrict__ offrow, float (&psi)[TP], float (&phi)[TP],
-                                             float (&f)[TP], int& n) {
-    n = 0;
+__device__ __forceinline__ void kb_gather_s4(const float2* __restrict__ S4, unsigned int base,
+                                             const int4* __restrict__ offrow, float (&f)[TP], float (&m)[TP], int& n) {
+    unsigned int cnt = 0u;
 #pragma unroll
     for (int q = 0; q < (TP + 3) / 4; ++q) {
         const int4 o = __ldg(offrow + q);
@@ -204,62 +209,74 @@ __device__ __forceinline__ void kb_gather_s4(const float4* __restrict__ S4, unsi
         for (int i = 0; i < 4; ++i) {
             const int t = 4 * q + i;
             if (t < TP) {
-                const float4 s = __ldg(S4 + (base + (unsigned int)oo[i]));
-                psi[t] = s.x;
-                phi[t] = s.y;
-                f[t] = s.z;
-                n += __float_as_int(s.w);
+                const float2 s = __ldg(S4 + (base + (unsigned int)oo[i]));
+                f[t] = s.x;
+                m[t] = s.y;
+                cnt += __float_as_uint(s.y) >> 31;  // the sign bit of m is the valid flag
             }
         }
     }
+    n = (int)cnt;
+}
+
+// kept sums of one sample: psi = f |m| (one fused multiply-add), phi = |m| or m^2
+template <bool SQ>
+__device__ __forceinline__ void kb_accumulate(float f, float m, float& sp, float& sf) {
+    sp = __fmaf_rn(f, -m, sp);
+    sf = SQ ? __fmaf_rn(m, m, sf) : __fsub_rn(sf, m);
+}
+
+// nk = number of kept samples if COUNT, else 1 if anything was kept (sum phi > 0) and 0 if not
+template <int TP, bool SQ, bool COUNT>
+__device__ __forceinline__ int kb_kept_sums(const float (&f)[TP], const float (&m)[TP], int n, const DevParams& P,
+                                            float lo, float hi, float& sp, float& sf) {
+    int nk = 0;
+    if (!P.sigmag_enable) {
+#pragma unroll
+        for (int t = 0; t < TP; ++t)
+            if (m[t] < 0.0f) kb_accumulate<SQ>(f[t], m[t], sp, sf);
+        nk = n;
+    } else if (hi < CUDART_INF_F) {
+        // an invalid sample (f = +inf) fails f <= hi on its own
+#pragma unroll
+        for (int t = 0; t < TP; ++t) {
+            if (f[t] >= lo && f[t] <= hi) {
+                kb_accumulate<SQ>(f[t], m[t], sp, sf);
+                if (COUNT) ++nk;
+            }
+        }
+    } else {  // hi = +inf (or NaN: then nothing is kept either way): the validity test is needed
+#pragma unroll
+        for (int t = 0; t < TP; ++t) {
+            if (m[t] < 0.0f && f[t] >= lo && f[t] <= hi) {
+                kb_accumulate<SQ>(f[t], m[t], sp, sf);
+                if (COUNT) ++nk;
+            }
+        }
+    }
+    if (!COUNT && P.sigmag_enable) nk = sf > 0.0f ? 1 : 0;  // every kept sample adds phi > 0
+    return nk;
 }
 
 // sigma-G filter + kept sums of a gathered trajectory (the search kernels' form of kb_score_lightcurve: the filter
-// values come from the S4 canvas instead of 26 divides, invalid samples carry f = +inf, psi = phi = 0).
-// Returns n_kept (0 = no result); sp, sf = kept sums.
-template <int TP>
-__device__ __forceinline__ int kb_score_s4(const float (&psi)[TP], const float (&phi)[TP], const float (&f)[TP], int n,
-                                           const DevParams& P, float* scratch, int stride, float& sp, float& sf) {
+// values come from the canvas instead of 26 divides; invalid samples carry f = +inf, m = 0).
+// Returns n_kept (COUNT; 0 = no result) or just non-zero / zero; sp, sf = kept sums.
+template <int TP, bool COUNT>
+__device__ __forceinline__ int kb_score_s4(const float (&f)[TP], const float (&m)[TP], int n, const DevParams& P,
+                                           float* scratch, int stride, float& sp, float& sf) {
     sp = 0.0f;
     sf = 0.0f;
     const int need = P.min_obs > 1 ? P.min_obs : 1;
     if (n < need) return 0;
-    int nk = 0;
+    float lo = -CUDART_INF_F, hi = CUDART_INF_F;
     if (P.sigmag_enable) {
         float s[TP];
 #pragma unroll
         for (int t = 0; t < TP; ++t) s[t] = f[t];
-        float lo, hi;
         kb_clip_window<TP>(s, n, P, scratch, stride, lo, hi);
-        if (hi < CUDART_INF_F) {
-            // an invalid sample (f = +inf) fails f <= hi on its own
-#pragma unroll
-            for (int t = 0; t < TP; ++t) {
-                if (f[t] >= lo && f[t] <= hi) {
-                    sp += psi[t];
-                    sf += phi[t];
-                    ++nk;
-                }
-            }
-        } else {  // hi = +inf (or NaN: then nothing is kept either way): the validity test is needed
-#pragma unroll
-            for (int t = 0; t < TP; ++t) {
-                if (phi[t] > 0.0f && f[t] >= lo && f[t] <= hi) {
-                    sp += psi[t];
-                    sf += phi[t];
-                    ++nk;
-                }
-            }
-        }
-    } else {
-#pragma unroll
-        for (int t = 0; t < TP; ++t) {
-            sp += psi[t];  // invalid samples add (0, 0)
-            sf += phi[t];
-        }
-        nk = n;
     }
-    return nk;
+    return P.filter_on ? kb_kept_sums<TP, true, COUNT>(f, m, n, P, lo, hi, sp, sf)
+                       : kb_kept_sums<TP, false, COUNT>(f, m, n, P, lo, hi, sp, sf);
 }
 
 // 64-bit top-K key: (orderable L', ~velocity index); larger key = better result (L' desc, then vel_idx asc); 0 = empty
@@ -317,7 +334,7 @@ int kb_launch_finalize(int TP, const unsigned long long* d_keys, const void* d_S
                        int W, int row_begin, int n_rows, const DevParams& P, float* d_lh, float* d_flux, int32_t* d_vel,
                        int32_t* d_nobs, cudaStream_t st);
 int kb_launch_unfiltered_lh(int TP, const int32_t* d_vel_idx, const void* d_S4, const S4Geom& G, const int* d_off, int W,
-                            int row_begin, int n_rows, int K, int n_vel, float* d_lh_raw, cudaStream_t st);
+                            int row_begin, int n_rows, int K, int n_vel, int filter_on, float* d_lh_raw, cudaStream_t st);
 int kb_write_stats(unsigned long long* d_stats, unsigned long long nominal, unsigned long long launches,
                    unsigned long long algo, unsigned long long evaluated_all, cudaStream_t st);
 int kb_launch_search_direct(int TP, const void* d_S4, const S4Geom& G, const int* d_off, const int* d_order, int W,

@@ -12,17 +12,17 @@ namespace {
 
 // one thread per canvas pixel of planes 0..T (plane T is the all-invalid plane padding epochs point into)
 __global__ void __launch_bounds__(256)
-s4_build_kernel(const float2* __restrict__ psiphi, float4* __restrict__ S4, int T, int H, int W,
+s4_build_kernel(const float2* __restrict__ psiphi, float2* __restrict__ S4, int T, int H, int W,
                 const __grid_constant__ S4Geom G, int filter_on) {
     const unsigned int xp = blockIdx.x * 256u + threadIdx.x;
     if (xp >= (unsigned int)G.Wp) return;
     const int yp = blockIdx.y, t = blockIdx.z;
     const int x = (int)xp - G.pxn, y = yp - G.pyn;
-    float4 o = make_float4(0.0f, 0.0f, CUDART_INF_F, 0.0f);
+    float2 o = make_float2(CUDART_INF_F, 0.0f);  // (f, m): common.cuh "canvas"
     if (t < T && x >= 0 && x < W && y >= 0 && y < H) {
         const float2 s = __ldg(psiphi + ((size_t)t * H + y) * W + x);
         if (s.y > 0.0f)  // reading R21: a sample is valid iff phi > 0 (prep writes (0, 0) for invalid pixels)
-            o = make_float4(s.x, s.y, kb_filter_value(s.x, s.y, filter_on), __int_as_float(1));
+            o = make_float2(kb_filter_value(s.x, s.y, filter_on), filter_on ? -__fsqrt_rn(s.y) : -s.y);
     }
     S4[(size_t)t * G.plane + (size_t)yp * G.Wp + xp] = o;
 }
@@ -33,7 +33,7 @@ constexpr int FIN_THREADS = 128;
 
 template <int TP>
 __global__ void __launch_bounds__(FIN_THREADS)
-finalize_kernel(const unsigned long long* __restrict__ keys, const float4* __restrict__ S4,
+finalize_kernel(const unsigned long long* __restrict__ keys, const float2* __restrict__ S4,
                 const __grid_constant__ S4Geom G, const int* __restrict__ off, int W, int row_begin, int n_rows,
                 const __grid_constant__ DevParams P, float* __restrict__ out_lh, float* __restrict__ out_flux,
                 int32_t* __restrict__ out_vel, int32_t* __restrict__ out_nobs) {
@@ -49,10 +49,10 @@ finalize_kernel(const unsigned long long* __restrict__ keys, const float4* __res
         const int pixlin = (int)(i / P.K);
         const int yb = pixlin / W, x0 = pixlin - yb * W;
         const unsigned int base = (unsigned int)(yb + row_begin + G.pyn) * (unsigned int)G.Wp + (unsigned int)(x0 + G.pxn);
-        float psi[TP], phi[TP], f[TP], sp, sf;
+        float f[TP], m[TP], sp, sf;
         int n;
-        kb_gather_s4<TP>(S4, base, reinterpret_cast<const int4*>(off + (size_t)vel * kb_tp4(TP)), psi, phi, f, n);
-        nobs = kb_score_s4<TP>(psi, phi, f, n, P, scratch_all + threadIdx.x, FIN_THREADS, sp, sf);
+        kb_gather_s4<TP>(S4, base, reinterpret_cast<const int4*>(off + (size_t)vel * kb_tp4(TP)), f, m, n);
+        nobs = kb_score_s4<TP, true>(f, m, n, P, scratch_all + threadIdx.x, FIN_THREADS, sp, sf);
         lh = kb_lh_of(sp, sf);
         flux = kb_flux_of(sp, sf);
     }
@@ -65,8 +65,8 @@ finalize_kernel(const unsigned long long* __restrict__ keys, const float4* __res
 // unfiltered sum-LH of every result slot: sum over ALL valid epochs, no clip, no threshold
 template <int TP>
 __global__ void __launch_bounds__(FIN_THREADS)
-unfiltered_lh_kernel(const int32_t* __restrict__ vel_idx, const float4* __restrict__ S4, const __grid_constant__ S4Geom G,
-                     const int* __restrict__ off, int W, int row_begin, int n_rows, int K, int n_vel,
+unfiltered_lh_kernel(const int32_t* __restrict__ vel_idx, const float2* __restrict__ S4, const __grid_constant__ S4Geom G,
+                     const int* __restrict__ off, int W, int row_begin, int n_rows, int K, int n_vel, int filter_on,
                      float* __restrict__ out_lh) {
     const size_t i = (size_t)blockIdx.x * FIN_THREADS + threadIdx.x;
     const size_t total = (size_t)n_rows * W * K;
@@ -77,14 +77,16 @@ unfiltered_lh_kernel(const int32_t* __restrict__ vel_idx, const float4* __restri
         const int pixlin = (int)(i / K);
         const int yb = pixlin / W, x0 = pixlin - yb * W;
         const unsigned int base = (unsigned int)(yb + row_begin + G.pyn) * (unsigned int)G.Wp + (unsigned int)(x0 + G.pxn);
-        float psi[TP], phi[TP], f[TP];
+        float f[TP], m[TP];
         int n;
-        kb_gather_s4<TP>(S4, base, reinterpret_cast<const int4*>(off + (size_t)vel * kb_tp4(TP)), psi, phi, f, n);
+        kb_gather_s4<TP>(S4, base, reinterpret_cast<const int4*>(off + (size_t)vel * kb_tp4(TP)), f, m, n);
         float sp = 0.0f, sf = 0.0f;
 #pragma unroll
         for (int t = 0; t < TP; ++t) {
-            sp += psi[t];
-            sf += phi[t];
+            if (m[t] < 0.0f) {
+                if (filter_on) kb_accumulate<true>(f[t], m[t], sp, sf);
+                else kb_accumulate<false>(f[t], m[t], sp, sf);
+            }
         }
         if (n > 0) lh = kb_lh_of(sp, sf);
     }
@@ -148,13 +150,13 @@ int kb_s4_plan(int T, int TP, int H, int W, const int32_t* h_dx, const int32_t* 
     return KBMOD_OK;
 }
 
-size_t kb_s4_bytes(const S4Geom& G, int T) { return (size_t)G.plane * (size_t)(T + 1) * sizeof(float4); }
+size_t kb_s4_bytes(const S4Geom& G, int T) { return (size_t)G.plane * (size_t)(T + 1) * sizeof(float2); }
 
 int kb_launch_s4_build(const float* d_psiphi, int T, int H, int W, const S4Geom& G, int filter_on, void* d_S4,
                        cudaStream_t st) {
     const dim3 grid((unsigned)((G.Wp + 255) / 256), (unsigned)G.Hp, (unsigned)(T + 1));
     KB_REQUIRE(G.Hp <= 65535 && T + 1 <= 65535, KBMOD_ERR_UNSUPPORTED, "canvas of %d rows exceeds the grid limit", G.Hp);
-    s4_build_kernel<<<grid, 256, 0, st>>>(reinterpret_cast<const float2*>(d_psiphi), reinterpret_cast<float4*>(d_S4), T, H,
+    s4_build_kernel<<<grid, 256, 0, st>>>(reinterpret_cast<const float2*>(d_psiphi), reinterpret_cast<float2*>(d_S4), T, H,
                                           W, G, filter_on);
     KB_CUDA(cudaGetLastError());
     return KBMOD_OK;
@@ -168,19 +170,19 @@ int kb_launch_finalize(int TPv, const unsigned long long* d_keys, const void* d_
     KB_DISPATCH_TP(TPv, {
         const size_t smem = (size_t)TP * FIN_THREADS * sizeof(float);
         finalize_kernel<TP><<<(unsigned)((total + FIN_THREADS - 1) / FIN_THREADS), FIN_THREADS, smem, st>>>(
-            d_keys, reinterpret_cast<const float4*>(d_S4), G, d_off, W, row_begin, n_rows, P, d_lh, d_flux, d_vel, d_nobs);
+            d_keys, reinterpret_cast<const float2*>(d_S4), G, d_off, W, row_begin, n_rows, P, d_lh, d_flux, d_vel, d_nobs);
     });
     KB_CUDA(cudaGetLastError());
     return KBMOD_OK;
 }
 
 int kb_launch_unfiltered_lh(int TPv, const int32_t* d_vel_idx, const void* d_S4, const S4Geom& G, const int* d_off, int W,
-                            int row_begin, int n_rows, int K, int n_vel, float* d_lh_raw, cudaStream_t st) {
+                            int row_begin, int n_rows, int K, int n_vel, int filter_on, float* d_lh_raw, cudaStream_t st) {
     const size_t total = (size_t)n_rows * W * K;
     if (total == 0) return KBMOD_OK;
     KB_DISPATCH_TP(TPv, {
         unfiltered_lh_kernel<TP><<<(unsigned)((total + FIN_THREADS - 1) / FIN_THREADS), FIN_THREADS, 0, st>>>(
-            d_vel_idx, reinterpret_cast<const float4*>(d_S4), G, d_off, W, row_begin, n_rows, K, n_vel, d_lh_raw);
+            d_vel_idx, reinterpret_cast<const float2*>(d_S4), G, d_off, W, row_begin, n_rows, K, n_vel, filter_on, d_lh_raw);
     });
     KB_CUDA(cudaGetLastError());
     return KBMOD_OK;

@@ -19,7 +19,7 @@ namespace {
 constexpr int SD_BX = 32, SD_BY = 4;  // block = 4 warps, each a 32-pixel row segment
 constexpr int SD_THREADS = SD_BX * SD_BY;
 #ifndef KB_SD_BLOCKS
-#define KB_SD_BLOCKS 4
+#define KB_SD_BLOCKS 5
 #endif
 // Persistent blocks per SM (4 x 128 threads x 127 registers fill the register file).  The kernel is bound by the
 // L1 / L2 path (16 bytes per sample, one 512-byte row segment per warp and epoch).  The velocity list is walked in an
@@ -30,8 +30,8 @@ constexpr int SD_BLOCKS_PER_SM = KB_SD_BLOCKS;
 constexpr int SD_SBW = 8, SD_SBH = 64;  // super-block of tiles: 8 x 32 = 256 pixels wide, 64 x 4 = 256 rows tall
 
 template <int TP>
-__global__ void __launch_bounds__(SD_THREADS)
-search_direct_kernel(const float4* __restrict__ S4, const __grid_constant__ S4Geom G, const int* __restrict__ off,
+__global__ void __launch_bounds__(SD_THREADS, SD_BLOCKS_PER_SM)
+search_direct_kernel(const float2* __restrict__ S4, const __grid_constant__ S4Geom G, const int* __restrict__ off,
                      const int* __restrict__ order, int W, int row_begin, int row_end, int n_vel,
                      const __grid_constant__ DevParams P, unsigned long long* __restrict__ keys_out) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -65,10 +65,10 @@ search_direct_kernel(const float4* __restrict__ S4, const __grid_constant__ S4Ge
         for (int i = 0; i < n_vel; ++i) {
             __syncwarp();  // re-converge after the divergent top-K insertion of the previous velocity
             const int v = __ldg(order + i);
-            float psi[TP], phi[TP], f[TP], sp, sf;
+            float f[TP], m[TP], sp, sf;
             int n;
-            kb_gather_s4<TP>(S4, base, reinterpret_cast<const int4*>(off + (size_t)v * TP4), psi, phi, f, n);  // uniform row
-            const int nk = kb_score_s4<TP>(psi, phi, f, n, P, scratch, SD_THREADS, sp, sf);
+            kb_gather_s4<TP>(S4, base, reinterpret_cast<const int4*>(off + (size_t)v * TP4), f, m, n);  // uniform row
+            const int nk = kb_score_s4<TP, false>(f, m, n, P, scratch, SD_THREADS, sp, sf);
             if (nk == 0) continue;
             const float lh = kb_lh_of(sp, sf);
             if (!(lh >= P.min_lh)) continue;
@@ -109,7 +109,7 @@ int kb_launch_search_direct(int TPv, const void* d_S4, const S4Geom& G, const in
     KB_DISPATCH_TP(TPv, {
         const size_t smem = (size_t)TP * SD_THREADS * sizeof(float) + (size_t)P.K * SD_THREADS * sizeof(unsigned long long);
         KB_CUDA(cudaFuncSetAttribute(search_direct_kernel<TP>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        search_direct_kernel<TP><<<grid, block, smem, st>>>(reinterpret_cast<const float4*>(d_S4), G, d_off, d_order, W,
+        search_direct_kernel<TP><<<grid, block, smem, st>>>(reinterpret_cast<const float2*>(d_S4), G, d_off, d_order, W,
                                                             row_begin, row_end, n_vel, P, d_keys);
     });
     KB_CUDA(cudaGetLastError());

@@ -642,7 +642,7 @@ bound_phase_kernel(const __grid_constant__ TensorMaps maps, int T, int row_begin
 // ---------------------------------------------------------------------------------------------
 // phase 2: exact evaluation (steps 1-3 of kbmod_search) of one (pixel, velocity) pair + top-K insertion
 struct ExactArgs {
-    const float4* S4;
+    const float2* S4;
     S4Geom G;
     const int* off;      // [n_vel][kb_tp4(TP)]
     int W, row_begin, row_end;
@@ -656,10 +656,10 @@ template <int TP>
 __device__ __forceinline__ bool eval_pair(const ExactArgs& A, const DevParams& P, int x0, int y0, int v, float* scratch,
                                           int stride) {
     const unsigned int base = (unsigned int)(y0 + A.G.pyn) * (unsigned int)A.G.Wp + (unsigned int)(x0 + A.G.pxn);
-    float psi[TP], phi[TP], f[TP], sp, sf;
+    float f[TP], m[TP], sp, sf;
     int n;
-    kb_gather_s4<TP>(A.S4, base, reinterpret_cast<const int4*>(A.off + (size_t)v * kb_tp4(TP)), psi, phi, f, n);
-    const int nk = kb_score_s4<TP>(psi, phi, f, n, P, scratch, stride, sp, sf);
+    kb_gather_s4<TP>(A.S4, base, reinterpret_cast<const int4*>(A.off + (size_t)v * kb_tp4(TP)), f, m, n);
+    const int nk = kb_score_s4<TP, false>(f, m, n, P, scratch, stride, sp, sf);
     if (nk > 0) {
         const float lh = kb_lh_of(sp, sf);
         if (lh >= P.min_lh) {
@@ -1111,7 +1111,7 @@ int kb_launch_search_pruned(const float* d_psiphi, const PrunedPlan& plan, const
     const size_t smem1 = (size_t)plan.ring_bytes + (size_t)PR_NTBL * TBL + PR_SMEM_MISC;
     KB_CUDA(cudaFuncSetAttribute(bound_phase_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem1));
     PrunedTables tb{tbd.gvel, tbd.gtbl, tbd.maskx, tbd.masky, tbd.gfoot, ng, plan.ring_bytes};
-    ExactArgs EA{reinterpret_cast<const float4*>(d_S4), G, d_off, W, row_begin, row_end, d_keys};
+    ExactArgs EA{reinterpret_cast<const float2*>(d_S4), G, d_off, W, row_begin, row_end, d_keys};
     KB_DISPATCH_TP(TPv, {
         const size_t smem2 = (size_t)TP * EX_THREADS * sizeof(float);
         KB_CUDA(cudaFuncSetAttribute(exact_queue_kernel<TP>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem2));
