@@ -261,6 +261,23 @@ int kbmod_sigmag_postfilter(const float* d_psi_lc, const float* d_phi_lc, int n_
                             const kbmod_search_params* p, uint64_t* d_kept, float* d_lh, float* d_flux, uint8_t* d_pass,
                             int32_t* d_survivors, uint64_t* d_n_pass, void* stream);
 
+/* The same post-filter for callers that cannot allocate device memory (code under CUDA graph capture, tight serving
+ * loops, harnesses that forbid cudaMalloc): results identical to kbmod_sigmag_postfilter, but the
+ * scratch -- the pass flags and the counters of the ordered compaction -- is a static device array inside the library:
+ * KBMOD_POSTFILTER_STATIC_MAX_LC flag bytes + 256 B (4 MiB + 256 B on every GPU that loads the library, until exit).
+ * The call allocates nothing (no cudaMalloc / cudaFree, no allocating library routine); it enqueues two 8/32-byte
+ * memsets and two kernels on `stream` and returns without synchronising.
+ *   d_survivors    out [n_lc] int32: indices with a result and L' >= min_lh, ascending, compacted to the front
+ *   d_n_survivors  out, 1 uint64 (device): their number
+ *   d_kept, d_lh, d_flux  out, nullable, as in kbmod_sigmag_filter
+ * n_lc > KBMOD_POSTFILTER_STATIC_MAX_LC returns KBMOD_ERR_WORKSPACE (split the list, or use kbmod_sigmag_postfilter).
+ * Every call on a device shares the one array, which keeps the previous call's contents (the call clears what must
+ * start at zero): calls that overlap on the GPU -- different streams with no ordering between them -- race. */
+#define KBMOD_POSTFILTER_STATIC_MAX_LC (1 << 22)
+int kbmod_sigmag_postfilter_static(const float* d_psi_lc, const float* d_phi_lc, int n_lc, int T,
+                                   const kbmod_search_params* p, uint64_t* d_kept, float* d_lh, float* d_flux,
+                                   int32_t* d_survivors, uint64_t* d_n_survivors, void* stream);
+
 /* ---------------------------------------------------------------------------------------------
  * Central-moment stamp filter, the step behind the coadd (s3.3): "we computed the central moments
  * of postage stamps for candidate trajectories.  Stamps were rejected if they did not have central moments that

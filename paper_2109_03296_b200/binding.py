@@ -45,6 +45,7 @@ SIGNATURES = {
     "kbmod_eval_trajectories": (_I, [_P, _I, _I, _I, _P, _P, _P, _P, _P, _I, _P, _P, _P, _P, _P, _P, _P, _P]),
     "kbmod_sigmag_filter": (_I, [_P, _P, _I, _I, _P, _P, _P, _P, _P]),
     "kbmod_sigmag_postfilter": (_I, [_P, _P, _I, _I, _P, _P, _P, _P, _P, _P, _P, _P]),
+    "kbmod_sigmag_postfilter_static": (_I, [_P, _P, _I, _I, _P, _P, _P, _P, _P, _P, _P]),
     "kbmod_stamp_moments": (_I, [_P, _I, _I, _P, _P, _P, _P]),
     "kbmod_pipeline_host_arena_bytes": (_Z, [_I, _I, _I, _I, _P]),
     "kbmod_pipeline_host_arena_bytes_for": (_Z, [_I, _I, _I, _P, _P, _P, _I, _P]),
@@ -490,6 +491,33 @@ def kbmod_sigmag_postfilter(psi_lc, phi_lc, params: SearchParams, compact=True, 
                                          _dev(r["kept"]), _dev(r["lh"]), _dev(r["flux"]), _dev(r["passed"]),
                                          _dev(r.get("survivors"), allow_none=True), _dev(r.get("n_pass"), allow_none=True),
                                          _stream(stream)))
+    return r
+
+
+POSTFILTER_STATIC_MAX_LC = 1 << 22
+
+
+def kbmod_sigmag_postfilter_static(psi_lc, phi_lc, params: SearchParams, out=None, stream=None):
+    """kbmod_sigmag_postfilter without device allocations inside the library call: the pass flags and compaction
+    counters live in a static device array of the library (at most POSTFILTER_STATIC_MAX_LC lightcurves per call;
+    calls that overlap on the GPU race on it).  `out`: optional dict of preallocated outputs (kept int64 [n], lh,
+    flux float32 [n], survivors int32 [n], n_survivors int64 [1]); returned (allocated by torch if not given)."""
+    import torch
+    n, T = psi_lc.shape
+    if tuple(phi_lc.shape) != (n, T):
+        raise ValueError("psi_lc and phi_lc must have one shape [n][T]")
+    dev = psi_lc.device
+    r = out if out is not None else dict(
+        kept=torch.empty(n, dtype=torch.int64, device=dev), lh=torch.empty(n, dtype=torch.float32, device=dev),
+        flux=torch.empty(n, dtype=torch.float32, device=dev), survivors=torch.empty(n, dtype=torch.int32, device=dev),
+        n_survivors=torch.empty(1, dtype=torch.int64, device=dev))
+    for k, dt in (("kept", torch.int64), ("lh", torch.float32), ("flux", torch.float32), ("survivors", torch.int32)):
+        if r[k].numel() < n or r[k].dtype != dt:
+            raise ValueError(f"out[{k!r}] must hold {n} elements of {dt}")
+    cp = params.c()
+    _check(lib().kbmod_sigmag_postfilter_static(_dev(psi_lc, torch.float32), _dev(phi_lc, torch.float32), n, T,
+                                                C.byref(cp), _dev(r["kept"]), _dev(r["lh"]), _dev(r["flux"]),
+                                                _dev(r["survivors"]), _dev(r["n_survivors"]), _stream(stream)))
     return r
 
 
