@@ -205,9 +205,10 @@ def run_reference(args):
 
 # ----------------------------------------------------------------------------------------- GPU arm
 # Algorithmic work per unit for the roofline.
-#   direct kernel  : bound "alu" -- every trajectory runs the compare-exchange network; the algorithmic
-#                    lane-operations per trajectory are 2*CE(T) min/max + per epoch 1 gather, 1 divide,
-#                    2 window compares, 2 adds, 1 count = 2*CE(T) + 7*T; peak = 148 SMs x 128 lanes x f_max.
+#   direct kernel  : bound "alu" -- every trajectory runs the compare-exchange network; FMNMX, FSETP, LOP3 and SHF
+#                    issue on the half-rate ALU pipe (2 warp-instructions per clock per SM, measured live by
+#                    kbmod_measure_issue_rate): achieved = ALU-pipe warp-instructions per trajectory (from the
+#                    committed ncu capture) x trajectories / live kernel time; peak = 148 SMs x 2 x f_max.
 #   pruned path    : bound "smem" -- the dominant kernel, bound_phase_kernel, gathers one packed 32-bit word
 #                    (fixed-point psi_+ | low-phi flag | valid flag) per trajectory-epoch evaluation from shared
 #                    memory: 4 B algorithmic; peak = 148 SMs x 128 B/clk x f_max.  Its duration is measured live
@@ -215,13 +216,38 @@ def run_reference(args):
 #                    SURVEY 8(d) counted 8 B per evaluation (psi and phi as float32): reported beside it.
 # dram__bytes_read.sum + dram__bytes_write.sum per step of the dominant kernel from the committed ncu --set full
 # capture (profiles/); None = not captured for this kernel
-TRAFFIC = {"bound_phase_kernel": 11.6e9, "search_direct_kernel": 11.7e12}  # bytes per step: profiles/r2_launches.md, r2_search_direct_kernel_full.md
+TRAFFIC = {"bound_phase_kernel": 11.6e9, "search_direct_kernel": 6.0e12}  # bytes per step: profiles/r2_launches.md, r2_search_direct_kernel_full.md
 CE_COUNT = {4: 5, 5: 9, 8: 19, 10: 32, 12: 42, 16: 63, 20: 103, 24: 132, 26: 147, 28: 162, 32: 191, 40: 305,
             48: 384, 50: 403, 56: 464, 64: 543}
 N_SM = 148
 # executed warp-instructions per warp-trajectory of search_direct_kernel<TP> (ncu smsp__inst_executed / (trajectories / 32),
 # profiles/r2_search_direct_kernel_full.md); other TP: scaled by the compare-exchange count
-DIRECT_WARP_INSTR_PER_TRAJ = {26: 607.0}
+DIRECT_WARP_INSTR_PER_TRAJ = {26: 585.7}
+# of which on the half-rate ALU pipe (FMNMX, FSETP, LOP3, SHF ...): sm__inst_executed_pipe_alu of the same capture,
+# 62.28 % of 2 per clock over the active cycles
+DIRECT_ALU_INSTR_PER_TRAJ = {26: 356.0}
+ALU_PIPE_PER_CLK = 2.0  # warp-instructions per clock per SM (16 lanes per scheduler); measured live beside it: issue_rates FMNMX
+
+
+def direct_roofline(T, tp, n_traj, kernel_ms, f_max, issue):
+    """The direct kernel is bound by the half-rate ALU pipe: 2 x 147 FMNMX of the sorting network + 2 FSETP per epoch
+    of the clip + the valid-bit shift-adds per trajectory (T = 26: 356 of its 586 warp-instructions)."""
+    if T <= max(DIRECT_WARP_INSTR_PER_TRAJ):
+        k = min(k for k in DIRECT_WARP_INSTR_PER_TRAJ if k >= T)
+        per, per_alu = DIRECT_WARP_INSTR_PER_TRAJ[k], DIRECT_ALU_INSTR_PER_TRAJ[k]
+    else:  # other network sizes: scaled by the compare-exchange count
+        per = 585.7 * CE_COUNT[tp] / CE_COUNT[26]
+        per_alu = 356.0 * CE_COUNT[tp] / CE_COUNT[26]
+    warp_traj = n_traj / 32.0
+    peak = N_SM * ALU_PIPE_PER_CLK * f_max
+    ach = warp_traj * per_alu / (kernel_ms * 1e-3)
+    return dict(bound="alu", kernel="search_direct_kernel", achieved=ach / 1e12, peak=peak / 1e12, unit="Twarp-instr/s",
+                frac=ach / peak, alu_pipe_warp_instr_per_trajectory=per_alu, warp_instr_per_trajectory=per,
+                issue_frac=warp_traj * per / (kernel_ms * 1e-3) / (N_SM * 4 * f_max),
+                alu_pipe_rate_measured_live=(issue or {}).get("FMNMX"),
+                peak_source="derived: 148 SMs x 2 ALU-pipe warp-instructions per clock x sm_max_mhz; the live FMNMX issue "
+                            "rate (kbmod_measure_issue_rate) is beside it",
+                source="instruction counts per trajectory from profiles/r2_search_direct_kernel_full.md")
 
 
 def run_ours(args):
@@ -355,18 +381,11 @@ def time_search(R, what, st, psiphi, vx, vy, pd, min_lh, steps, warmup):
                search_phases_ms={k: float(np.mean([p[k] for p in ph])) for k in ph[0]},
                filled_result_slots=int((out[2] >= 0).sum()))
     if algo_used == kb.ALGO_DIRECT:
-        # instruction-issue roofline of the direct kernel: executed warp-instructions per warp-trajectory from the
-        # committed ncu capture (profiles/), peak = 148 SMs x 4 warp-instructions per clock x max SM clock
-        tp = min(k for k in DIRECT_WARP_INSTR_PER_TRAJ if k >= T)
+        tp = min(k for k in CE_COUNT if k >= T)
         kern_ms = rec["search_phases_ms"]["gather"]
-        winst = float(H) * W * len(vx) / 32.0 * DIRECT_WARP_INSTR_PER_TRAJ[tp]
-        peak = N_SM * 4 * R["peaks"]["sm_max_mhz"] * 1e6
-        rec["roofline"] = dict(bound="issue", kernel="search_direct_kernel", achieved=winst / (kern_ms * 1e-3) / 1e12,
-                               peak=peak / 1e12, unit="Twarp-instr/s", frac=winst / (kern_ms * 1e-3) / peak,
-                               warp_instr_per_trajectory=DIRECT_WARP_INSTR_PER_TRAJ[tp], kernel_ms=kern_ms,
-                               traffic=TRAFFIC["search_direct_kernel"] if T == 26 and len(vx) == 8192 else None,
-                               note="issue slots are not what binds this kernel: the L1 / L2 / DRAM path is (profiles/)",
-                               source="smsp__inst_executed per trajectory from profiles/r2_search_direct_kernel_full.md")
+        rec["roofline"] = direct_roofline(T, tp, float(H) * W * len(vx), kern_ms, R["peaks"]["sm_max_mhz"] * 1e6, R.get("issue"))
+        rec["roofline"]["kernel_ms"] = kern_ms
+        rec["roofline"]["traffic"] = TRAFFIC["search_direct_kernel"] if T == 26 and len(vx) == 8192 else None
     del ws, out
     return rec
 
@@ -507,12 +526,7 @@ def report(R, args):
     kernel_ms = ph["gather"]  # the dominant kernel alone: bound_phase_kernel launches / the direct kernel
     pi = R["plan_info"]
     if algo_used == kb.ALGO_DIRECT:
-        tpd = min(k for k in DIRECT_WARP_INSTR_PER_TRAJ if k >= T) if T <= max(DIRECT_WARP_INSTR_PER_TRAJ) else None
-        per = DIRECT_WARP_INSTR_PER_TRAJ[tpd] if tpd else 640.0 * CE_COUNT[tp] / CE_COUNT[26]
-        winst = float(H) * W * n_vel / 32.0 * per
-        roof = dict(bound="issue", achieved=winst / (kernel_ms * 1e-3) / 1e12, peak=N_SM * 4 * f_max / 1e12,
-                    unit="Twarp-instr/s", kernel="search_direct_kernel", warp_instr_per_trajectory=per,
-                    peak_source="derived: 148 SMs x 4 warp-instructions per clock x sm_max_mhz (DESIGN.md)")
+        roof = direct_roofline(T, tp, float(H) * W * n_vel, kernel_ms, f_max, R.get("issue"))
     else:
         # one packed 32-bit bound word per trajectory-epoch evaluation.  `frac` counts the words the
         # kernel PHYSICALLY loads from shared memory: the nominal count less the (tile, group, epoch) regions that lie

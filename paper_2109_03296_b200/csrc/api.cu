@@ -421,7 +421,7 @@ extern "C" int kbmod_plan_search(kbmod_plan* pl, const float* d_psiphi, float* d
     if (pl->algo == KBMOD_ALGO_DIRECT) {
         kb_phase_mark(KB_PHASE_PLANES, st);
         rc = kb_launch_search_direct(pl->TP, d_S4, pl->G, d_off, (const int*)(ws + pl->w_tables + pl->b_order), pl->W,
-                                     pl->row_begin, pl->row_end, pl->n_vel, pl->P, d_keys, st);
+                                     pl->row_begin, pl->row_end, pl->n_vel, pl->P, d_keys, d_stats + 7 /* work counter */, st);
         if (rc) return rc;
         if (n_rows > 0) ++launches;
         kb_phase_mark(KB_PHASE_BOUND, st);  // the direct kernel is gather + filter + top-K in one: reported as phase 1

@@ -339,7 +339,7 @@ int kb_write_stats(unsigned long long* d_stats, unsigned long long nominal, unsi
                    unsigned long long algo, unsigned long long evaluated_all, cudaStream_t st);
 int kb_launch_search_direct(int TP, const void* d_S4, const S4Geom& G, const int* d_off, const int* d_order, int W,
                             int row_begin, int row_end, int n_vel, const DevParams& P, unsigned long long* d_keys,
-                            cudaStream_t st);
+                            unsigned long long* d_next_unit, cudaStream_t st);
 
 // ---------------------------------------------------------------------------------------------
 // launchers (one per .cu file); all return a KBMOD_* status

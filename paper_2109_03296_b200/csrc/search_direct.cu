@@ -1,15 +1,15 @@
 // (a3)-(a5) direct search: one thread per start pixel walks every velocity, gathers the T samples of the
-// trajectory from the padded S4 canvas (one 16-byte load per sample, no bounds test; a warp is 32 consecutive x0,
-// so each epoch is one 512-byte row segment through L1), runs the sigma-G filter on the register-resident
+// trajectory from the padded canvas (one 8-byte (f, m) load per sample, no bounds test; a warp is 32 consecutive x0,
+// so each epoch is one 256-byte row segment through L1), runs the sigma-G filter on the register-resident
 // lightcurve and keeps its pixel's top-K keys in shared memory.  search_common.cu's finalize_kernel turns the keys
 // into the output arrays.
 // PAPER.md:L79-L81 (s3), L93-L117 (s3.1), L127-L137 (s3.2); steps 1-4 of kbmod_search in include/kbmod_b200.h.
 // This is the evaluator for every trajectory when no threshold prunes (min_lh = -inf) and the implementation the
 // pruned kernel must agree with bit for bit.
 //
-// Instructions per trajectory at T = 26, about 560 (round 1: 1600): 7 offset loads + 26 x (IMAD.WIDE + LDG.128 + IADD)
-// gather, 147 x 2 FMNMX sort (half-rate ALU pipe), 26 STS + 3 LDS rank lookup, 26 x 5 clip-and-sum.  With that the kernel is no longer issue-bound: ncu
-// shows the L1 data path at 80 % and L2 at 68 % of their peaks (profiles/r2_search_direct_kernel_full.md).
+// Instructions per trajectory at T = 26 (round 1: 1600): 7 offset loads + 26 x (IMAD.WIDE + LDG.64 + shift-add of the
+// valid bit) gather, 147 x 2 FMNMX sort (half-rate ALU pipe), 26 STS + 3 LDS rank lookup, 26 x (2 FSETP + FFMA + FADD)
+// clip-and-sum.  The executed count and the pipe utilisations are in profiles/r2_search_direct_kernel_full.md.
 #include <algorithm>
 
 #include "common.cuh"
@@ -21,11 +21,11 @@ constexpr int SD_THREADS = SD_BX * SD_BY;
 #ifndef KB_SD_BLOCKS
 #define KB_SD_BLOCKS 5
 #endif
-// Persistent blocks per SM (4 x 128 threads x 127 registers fill the register file).  The kernel is bound by the
-// L1 / L2 path (16 bytes per sample, one 512-byte row segment per warp and epoch).  The velocity list is walked in an
-// order in which neighbours are neighbours in displacement space, so that consecutive velocities of a warp touch
-// overlapping lines; measured on configs[2], mode (B): 1 / 2 / 3 / 4 blocks per SM take 6.25 / 3.65 / 3.03 / 2.91 s
-// (latency hiding beats the L1 reuse fewer warps would gain), against 3.05-3.24 s in list order.
+// Persistent blocks per SM: a lightcurve is 2 x T registers (f, m), the kernel fits 96 registers and 5 blocks of 128
+// threads fill the register file.  The velocity list is walked in an order in which neighbours are neighbours in
+// displacement space, so that consecutive velocities of a warp touch overlapping lines.  Measured on configs[2],
+// mode (B): 4 / 5 / 6 blocks per SM take 2.33 / 2.29 / 2.32 s (6 blocks: 80 registers, spills); with the 16-byte
+// (psi, phi, f, valid) cell of the earlier design (128 registers, 4 blocks) 2.82 s; in list order +0.5 s.
 constexpr int SD_BLOCKS_PER_SM = KB_SD_BLOCKS;
 constexpr int SD_SBW = 8, SD_SBH = 64;  // super-block of tiles: 8 x 32 = 256 pixels wide, 64 x 4 = 256 rows tall
 
@@ -33,7 +33,8 @@ template <int TP>
 __global__ void __launch_bounds__(SD_THREADS, SD_BLOCKS_PER_SM)
 search_direct_kernel(const float2* __restrict__ S4, const __grid_constant__ S4Geom G, const int* __restrict__ off,
                      const int* __restrict__ order, int W, int row_begin, int row_end, int n_vel,
-                     const __grid_constant__ DevParams P, unsigned long long* __restrict__ keys_out) {
+                     const __grid_constant__ DevParams P, unsigned long long* __restrict__ keys_out,
+                     unsigned long long* __restrict__ next_unit) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     float* scratch = reinterpret_cast<float*>(smem_raw) + (threadIdx.y * SD_BX + threadIdx.x);  // [TP][threads]
     unsigned long long* list =
@@ -48,16 +49,28 @@ search_direct_kernel(const float2* __restrict__ S4, const __grid_constant__ S4Ge
     // over several hundred MB and the kernel read 12.6 TB from DRAM per search.
     const int sb_per_row = (tiles_x + SD_SBW - 1) / SD_SBW;
     const int n_sb = sb_per_row * ((tiles_y + SD_SBH - 1) / SD_SBH);
-    for (int slot = blockIdx.x; slot < n_sb * SD_SBW * SD_SBH; slot += gridDim.x) {
+    // Work units are the 32-pixel row segments of the tiles, handed out to the warps from a global counter in tile
+    // order (the warps in flight at one time work on neighbouring rows of neighbouring tiles): trajectories near the
+    // edges the velocities point away from leave the image early and cost a fraction of an interior row, so a static
+    // split leaves a fifth of the warp slots idle towards the end (measured: 2.29 s static, 2.22 s with twice as many
+    // blocks in two waves).
+    const unsigned int n_units = (unsigned int)(n_sb * SD_SBW * SD_SBH) * SD_BY;
+    for (;;) {
+        unsigned int u = 0;
+        if (threadIdx.x == 0) u = (unsigned int)atomicAdd(next_unit, 1ull);
+        u = __shfl_sync(0xFFFFFFFFu, u, 0);
+        if (u >= n_units) break;
+        const int slot = (int)(u / SD_BY), r = (int)(u % SD_BY);
         const int sb = slot / (SD_SBW * SD_SBH), in = slot - sb * (SD_SBW * SD_SBH);
         const int sby = sb / sb_per_row, sbx = sb - sby * sb_per_row;
         const int ty = sby * SD_SBH + in / SD_SBW, tx = sbx * SD_SBW + in % SD_SBW;
-        if (tx >= tiles_x || ty >= tiles_y) continue;  // block-uniform
+        if (tx >= tiles_x || ty >= tiles_y) continue;  // warp-uniform
         const int x0 = tx * SD_BX + threadIdx.x;
-        const int y0 = row_begin + ty * SD_BY + threadIdx.y;
-        const bool active = x0 < W && y0 < row_end;
+        const int y0 = row_begin + ty * SD_BY + r;
+        if (y0 >= row_end) continue;  // warp-uniform: the last tile row of the band may be partial
+        const bool active = x0 < W;
         // lanes past the edge evaluate the edge pixel again and write nothing: the warp stays whole
-        const int xc = min(x0, W - 1), yc = min(y0, row_end - 1);
+        const int xc = min(x0, W - 1), yc = y0;
         for (int k = 0; k < K; ++k) list[k * SD_THREADS] = 0ull;
         unsigned long long kth = 0ull;  // key of slot K-1: only a larger key enters the list
         const unsigned int base = (unsigned int)(yc + G.pyn) * (unsigned int)G.Wp + (unsigned int)(xc + G.pxn);
@@ -97,7 +110,7 @@ search_direct_kernel(const float2* __restrict__ S4, const __grid_constant__ S4Ge
 
 int kb_launch_search_direct(int TPv, const void* d_S4, const S4Geom& G, const int* d_off, const int* d_order, int W,
                             int row_begin, int row_end, int n_vel, const DevParams& P, unsigned long long* d_keys,
-                            cudaStream_t st) {
+                            unsigned long long* d_next_unit, cudaStream_t st) {
     const int n_rows = row_end - row_begin;
     if (n_rows <= 0) return KBMOD_OK;
     int n_sm = 148, dev = 0;
@@ -106,11 +119,12 @@ int kb_launch_search_direct(int TPv, const void* d_S4, const S4Geom& G, const in
     const dim3 block(SD_BX, SD_BY);
     const int n_tiles = ((W + SD_BX - 1) / SD_BX) * ((n_rows + SD_BY - 1) / SD_BY);
     const dim3 grid(std::min(n_tiles, n_sm * SD_BLOCKS_PER_SM));
+    KB_CUDA(cudaMemsetAsync(d_next_unit, 0, sizeof(unsigned long long), st));
     KB_DISPATCH_TP(TPv, {
         const size_t smem = (size_t)TP * SD_THREADS * sizeof(float) + (size_t)P.K * SD_THREADS * sizeof(unsigned long long);
         KB_CUDA(cudaFuncSetAttribute(search_direct_kernel<TP>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         search_direct_kernel<TP><<<grid, block, smem, st>>>(reinterpret_cast<const float2*>(d_S4), G, d_off, d_order, W,
-                                                            row_begin, row_end, n_vel, P, d_keys);
+                                                            row_begin, row_end, n_vel, P, d_keys, d_next_unit);
     });
     KB_CUDA(cudaGetLastError());
     return KBMOD_OK;

@@ -23,8 +23,8 @@
 //                        trajectory-epoch evaluation, one conflict-free LDS.32 and one integer add.  full/empty
 //                        mbarriers per in-flight region; no CTA-wide barrier anywhere in the loop.  (pixel,
 //                        velocity) pairs whose bound reaches min_lh are appended to a global queue.
-//   exact_queue_kernel   the queued pairs get the same evaluation as the direct kernel (16-byte gathers from the
-//                        padded S4 canvas, register sorting network); results enter the per-pixel top-K through a
+//   exact_queue_kernel   the queued pairs get the same evaluation as the direct kernel (8-byte gathers from the
+//                        padded canvas, register sorting network); results enter the per-pixel top-K through a
 //                        cascade of 64-bit atomicMax on (orderable L', ~vel_idx) keys.
 //   exact_overflow_kernel  (tile, group, warp) items that did not fit the queue, all pairs evaluated.
 // search_common.cu's finalize_kernel turns the keys into the four output arrays.
