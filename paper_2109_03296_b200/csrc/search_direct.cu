@@ -52,8 +52,8 @@ search_direct_kernel(const float2* __restrict__ S4, const __grid_constant__ S4Ge
     // Work units are the 32-pixel row segments of the tiles, handed out to the warps from a global counter in tile
     // order (the warps in flight at one time work on neighbouring rows of neighbouring tiles): trajectories near the
     // edges the velocities point away from leave the image early and cost a fraction of an interior row, so a static
-    // split leaves a fifth of the warp slots idle towards the end (measured: 2.29 s static, 2.22 s with twice as many
-    // blocks in two waves).
+    // split leaves a fifth of the warp slots idle towards the end (measured on configs[2], mode (B): 2.23 s static,
+    // 2.22 s with twice as many blocks in two waves, 1.78 s this way).
     const unsigned int n_units = (unsigned int)(n_sb * SD_SBW * SD_SBH) * SD_BY;
     for (;;) {
         unsigned int u = 0;

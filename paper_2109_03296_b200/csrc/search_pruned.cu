@@ -113,6 +113,10 @@ struct BoundParams {
 constexpr int SC_UNIT = 0, SC_INV_UNIT = 1, SC_CAP = 2, SC_FLOOR = 4, SC_THR = SC_FLOOR + KBMOD_MAX_T,
               SC_FLOATS = SC_THR + KBMOD_MAX_T + 1;
 
+// threshold table of the bound test: indexed by the low 2 cbits bits of an accumulator (n_low << cbits | n_valid), holds
+// the smallest accumulator value that passes; behind the scale table in the scratch
+constexpr size_t TT_BYTES = 4u << (2 * 7);                    // KBMOD_MAX_T = 64 -> cbits = 7
+
 struct Queue {
     uint2* entries;                  // (pixel index y0*W+x0, velocity index); v = 0xFFFFFFFF: hole
     unsigned long long* count;       // entries appended (may exceed cap: the excess overflowed)
@@ -137,7 +141,8 @@ struct Queue {
 constexpr int SC_BINS = 40, SC_SAMPLES = 16384;
 __global__ void __launch_bounds__(1024)
 bound_scale_kernel(const float2* __restrict__ psiphi, int T, int H, int W, float min_lh,
-                                   const __grid_constant__ BoundParams BP, float* __restrict__ scale) {
+                                   const __grid_constant__ BoundParams BP, int need, float* __restrict__ scale,
+                                   unsigned int* __restrict__ thrtab) {
     __shared__ float ssum[32];
     __shared__ int scnt[32];
     __shared__ int hist[SC_BINS + 1];
@@ -242,6 +247,23 @@ bound_scale_kernel(const float2* __restrict__ psiphi, int T, int H, int W, float
         for (int k = 0; k <= KBMOD_MAX_T; ++k) scale[SC_THR + k] = thr_units * ratio[k] * (1.0f - 1e-4f);
         scale[SC_THR] = 0.0f;  // no epoch is known to have phi >= its floor: no bound, always pass
     }
+    __syncthreads();
+    // The bound test as one table lookup.  An accumulator is  sum << 2c | n_low << c | n;  entry [n_low << c | n] is
+    // the smallest accumulator that passes: ceil(thr[max(m(n) - n_low, 0)]) << 2c (the float test
+    // (float)sum >= thr is sum >= ceil(thr) for an integer sum), 0 = always (no bound), ~0 = never (n < need).
+    const unsigned int cmask = (1u << BP.cbits) - 1u;
+    for (unsigned int idx = threadIdx.x; idx < (1u << (2 * BP.cbits)); idx += blockDim.x) {
+        const int n = (int)(idx & cmask), n_low = (int)(idx >> BP.cbits);
+        unsigned int e;
+        if (n < need || n > T) e = 0xFFFFFFFFu;
+        else if (BP.pass_all) e = 0u;
+        else {
+            const int m_eff = max((int)BP.mkept[n] - n_low, 0);
+            const float th = scale[SC_THR + m_eff];
+            e = th <= 0.0f ? 0u : ((unsigned int)ceilf(th)) << (2 * BP.cbits);
+        }
+        thrtab[idx] = e;
+    }
 }
 
 __global__ void bound_plane_kernel(const float2* __restrict__ psiphi, unsigned int* __restrict__ B, int H, int W, int Wp,
@@ -297,7 +319,7 @@ __global__ void __launch_bounds__(PR_THREADS, 1)
 bound_phase_kernel(const __grid_constant__ TensorMaps maps, int T, int row_begin, int row_end, int W, int tile_begin,
                    int tile_end, int g_begin, int g_end,
                    const __grid_constant__ PrunedTables tb, const __grid_constant__ BoundParams BP, int min_obs,
-                   const float* __restrict__ scale, const __grid_constant__ Queue Qu) {
+                   const unsigned int* __restrict__ thrtab, const __grid_constant__ Queue Qu) {
     extern __shared__ __align__(1024) unsigned char smem[];
     const int TBL = tbl_bytes(T);
     unsigned char* tblbase = smem + tb.ring_bytes;
@@ -566,37 +588,20 @@ bound_phase_kernel(const __grid_constant__ TensorMaps maps, int T, int row_begin
             const uint32_t vmask = __ldg(reinterpret_cast<const uint32_t*>(tb.gtbl + (size_t)g * TBL + (size_t)T * PR_G * 4 +
                                                                             offsetof(GroupEpoch, vmask)));
             int my_cnt = 0;
-            const unsigned int cmask = (1u << BP.cbits) - 1u;
-            const float* thr = scale + SC_THR;
+            // the bound test: one table lookup per (pixel, velocity), indexed by the accumulator's two count fields
+            // (bound_scale_kernel; n < min_obs never passes)
+            const unsigned int idx_mask = (1u << (2 * BP.cbits)) - 1u;
 #pragma unroll
             for (int h = 0; h < PR_PIX; ++h) {
                 const bool in_img = (px0 + 32 * (h & 1)) < W && (py0 + 16 * (h >> 1)) < row_end;
                 m[h] = 0u;
-                // quick test of the pixel's 16 velocities at once: the largest sum against the smallest threshold any of
-                // them can have (the fields of a word do not carry into each other, so the maximum of the packed words
-                // carries the maximum sum, and the OR of the low-phi counts bounds their maximum); 98 % of the pixels
-                // stop here
-                unsigned int mx = AN[h][0], orr = AN[h][0];
 #pragma unroll
-                for (int j = 1; j < PR_G; ++j) {
-                    mx = max(mx, AN[h][j]);
-                    orr |= AN[h][j];
+                for (int j = 0; j < PR_G; ++j) {
+                    const unsigned int an = AN[h][j] + ANU[h];
+                    const unsigned int need_an = __ldg(thrtab + (an & idx_mask));
+                    m[h] |= (an >= need_an ? 1u : 0u) << j;
                 }
-                const int nlow_ub = (int)((orr >> BP.cbits) & cmask) + (int)((ANU[h] >> BP.cbits) & cmask);
-                const float sum_max = (float)((mx + ANU[h]) >> (2 * BP.cbits));
-                const bool maybe = in_img && (BP.pass_all || sum_max >= __ldg(thr + max(BP.mk_min - nlow_ub, 0)));
-                if (maybe) {
-#pragma unroll
-                    for (int j = 0; j < PR_G; ++j) {
-                        const unsigned int an = AN[h][j] + ANU[h];
-                        const int n = (int)(an & cmask), n_low = (int)((an >> BP.cbits) & cmask);
-                        // at least m(n) epochs are kept, at least m(n) - n_low of them with phi >= their epoch's floor
-                        const int m_eff = max((int)BP.mkept[n] - n_low, 0);
-                        const bool pass = BP.pass_all || (float)(an >> (2 * BP.cbits)) >= __ldg(thr + m_eff);
-                        if (n >= need && pass) m[h] |= 1u << j;
-                    }
-                }
-                m[h] &= vmask;
+                m[h] = in_img ? (m[h] & vmask) : 0u;
                 my_cnt += __popc(m[h]);
             }
             const int total = __reduce_add_sync(0xFFFFFFFFu, my_cnt);
@@ -883,7 +888,8 @@ ScratchLayout scratch_layout(int T, int H, int W, int n_rows, int n_vel) {
     size_t o = 0;
     L.B = o;        o += al256((size_t)T * H * Wp * 4);
     L.qentries = o; o += al256(queue_cap(n_vel) * 8);
-    L.qcount = o;   o += 256 + al256(SC_FLOATS * sizeof(float));  // queue counter, then the scale table
+    // queue counters, then the scale table, then the threshold table of the bound test (2^(2 cbits) words, cbits <= 7)
+    L.qcount = o;   o += 256 + al256(SC_FLOATS * sizeof(float)) + TT_BYTES;
     L.overflow_words = (n_tiles_of(n_rows, W) * ngm * (PR_CONSUMERS / 32) + 31) / 32;
     L.overflow = o; o += al256(L.overflow_words * 4);
     L.total = o;
@@ -1084,6 +1090,7 @@ int kb_launch_search_pruned(const float* d_psiphi, const PrunedPlan& plan, const
     Qu.count = (unsigned long long*)(w + L.qcount);
     Qu.units = Qu.count + 1;
     float* d_scale = (float*)(w + L.qcount + 256);  // unit, cap, floors and thresholds of the fixed-point bound planes
+    unsigned int* d_thrtab = (unsigned int*)(w + L.qcount + 256 + al256(SC_FLOATS * sizeof(float)));
     Qu.cap = queue_cap(n_vel);
     Qu.overflow = (unsigned int*)(w + L.overflow);
 
@@ -1111,7 +1118,8 @@ int kb_launch_search_pruned(const float* d_psiphi, const PrunedPlan& plan, const
     int launches = 0;
     {
         const size_t n = (size_t)T * H * Wp;
-        bound_scale_kernel<<<1, 1024, 0, st>>>(reinterpret_cast<const float2*>(d_psiphi), T, H, W, P.min_lh, bp, d_scale);
+        bound_scale_kernel<<<1, 1024, 0, st>>>(reinterpret_cast<const float2*>(d_psiphi), T, H, W, P.min_lh, bp,
+                                               P.min_obs > 1 ? P.min_obs : 1, d_scale, d_thrtab);
         KB_CUDA(cudaGetLastError());
         bound_plane_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(reinterpret_cast<const float2*>(d_psiphi), d_B, H, W,
                                                                         (int)Wp, (size_t)T * H, bp.cbits, d_scale);
@@ -1137,7 +1145,7 @@ int kb_launch_search_pruned(const float* d_psiphi, const PrunedPlan& plan, const
                     const int g1 = std::min(ng, g0 + groups_per_chunk);
                     KB_CUDA(cudaMemsetAsync(Qu.count, 0, 3 * sizeof(unsigned long long), st));  // queue, unit and chunk counters
                     bound_phase_kernel<<<std::min(grid, b1 - b0), PR_THREADS, smem1, st>>>(maps, T, row_begin, row_end, W, b0, b1,
-                                                                                          g0, g1, tb, bp, P.min_obs, d_scale, Qu);
+                                                                                          g0, g1, tb, bp, P.min_obs, d_thrtab, Qu);
                     KB_CUDA(cudaGetLastError());
                     kb_phase_mark(KB_PHASE_BOUND, st);
                     exact_queue_kernel<TP><<<n_sm * EX_CTAS_PER_SM, EX_THREADS, smem2, st>>>(EA, P, Qu, d_stats);
