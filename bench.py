@@ -216,7 +216,7 @@ def run_reference(args):
 #                    SURVEY 8(d) counted 8 B per evaluation (psi and phi as float32): reported beside it.
 # dram__bytes_read.sum + dram__bytes_write.sum per step of the dominant kernel from the committed ncu --set full
 # capture (profiles/); None = not captured for this kernel
-TRAFFIC = {"bound_phase_kernel": 11.6e9, "search_direct_kernel": 6.0e12}  # bytes per step: profiles/r2_launches.md, r2_search_direct_kernel_full.md
+TRAFFIC = {"bound_phase_kernel": 11.6e9, "search_direct_kernel": 1.37e12}  # bytes per step: profiles/r2_launches.md, r2_search_direct_kernel_full.md
 CE_COUNT = {4: 5, 5: 9, 8: 19, 10: 32, 12: 42, 16: 63, 20: 103, 24: 132, 26: 147, 28: 162, 32: 191, 40: 305,
             48: 384, 50: 403, 56: 464, 64: 543}
 N_SM = 148
@@ -224,7 +224,7 @@ N_SM = 148
 # profiles/r2_search_direct_kernel_full.md); other TP: scaled by the compare-exchange count
 DIRECT_WARP_INSTR_PER_TRAJ = {26: 585.7}
 # of which on the half-rate ALU pipe (FMNMX, FSETP, LOP3, SHF ...): sm__inst_executed_pipe_alu of the same capture,
-# 62.28 % of 2 per clock over the active cycles
+# 74.4 % of 2 per clock over the active cycles
 DIRECT_ALU_INSTR_PER_TRAJ = {26: 356.0}
 ALU_PIPE_PER_CLK = 2.0  # warp-instructions per clock per SM (16 lanes per scheduler); measured live beside it: issue_rates FMNMX
 
