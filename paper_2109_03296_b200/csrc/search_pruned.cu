@@ -874,7 +874,7 @@ size_t queue_cap(int n_vel) {
         if (v > 0) return (size_t)std::max<long long>(64, v);
     }
     const double want = 1100.0 * PR_TW * PR_TH * (double)n_vel / 32.0;
-    return (size_t)std::min(268435456.0, std::max(1048576.0, want));
+    return (size_t)std::min(536870912.0, std::max(1048576.0, want));  // at most 2^29 entries = 4 GiB
 }
 size_t n_tiles_of(int n_rows, int W) { return (size_t)((W + PR_TW - 1) / PR_TW) * ((n_rows + PR_TH - 1) / PR_TH); }
 size_t al256(size_t x) { return (x + 255) & ~(size_t)255; }
@@ -1066,14 +1066,19 @@ int kb_launch_search_pruned(const float* d_psiphi, const PrunedPlan& plan, const
     KB_REQUIRE(!plan.too_scattered && (size_t)ng <= ngm, KBMOD_ERR_UNSUPPORTED,
                "pruned search: %d velocity groups needed, workspace holds %zu (velocities too scattered; use the direct kernel)",
                ng, ngm);
-    // launches cover (a batch of whole waves of tiles) x (a chunk of the groups), sized so that 1/4 of the launch's
-    // trajectories fit the survivor queue (what does not fit is evaluated wholesale by the overflow kernel)
+    // launches cover (a batch of whole waves of tiles) x (a chunk of the groups), sized so that 1/16 of the launch's
+    // trajectories fit the survivor queue: 1.5 % survive on configs[2], 2.6 % on configs[3] (unevenly over the image);
+    // what does not fit is evaluated wholesale by the overflow kernel (correct, 65 x the work for the items concerned).
+    // Measured on configs[2] with a 2^28-entry queue for 1/4, 1/16, 1/24, 1/32, 1/64: bound phase 226.7 / 222.8 /
+    // 218.4 / 221.1 / 217.0 ms (fewer launch tails, more L2 reuse of the staged planes), exact phase 82 ms except at
+    // 1/64, where the queue overflows (169 ms); at 1/24 configs[3] overflowed on some launches.  Hence a larger queue
+    // (2^29 entries) at 1/16, and batches of equal size (work units are handed out dynamically: whole waves do not matter).
     int n_sm = 148, dev = 0;
     KB_CUDA(cudaGetDevice(&dev));
     KB_CUDA(cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev));
     const int n_tiles = (int)n_tiles_of(n_rows, W);
     const int grid = std::max(1, std::min(n_sm, n_tiles));
-    const double budget = 4.0 * (double)queue_cap(n_vel);
+    const double budget = 16.0 * (double)queue_cap(n_vel);
     const double wave_nominal = (double)grid * PR_TW * PR_TH * (double)ng * PR_G;  // one wave, all groups
     const int n_chunks = std::max(1, std::min(std::max(ng, 1), (int)ceil(wave_nominal / budget)));
     const int groups_per_chunk = ((std::max(1, (ng + n_chunks - 1) / n_chunks) + PR_SUB - 1) / PR_SUB) * PR_SUB;
@@ -1127,9 +1132,11 @@ int kb_launch_search_pruned(const float* d_psiphi, const PrunedPlan& plan, const
         launches += 2;
         kb_phase_mark(KB_PHASE_PLANES, st);
     }
-    long long waves = (long long)(budget / std::max(1.0, wave_nominal / n_chunks));
-    waves = std::max<long long>(1, std::min<long long>(PR_WAVES_PER_BATCH, waves));
-    const int batch = (int)std::min<long long>((long long)n_tiles, waves * grid);
+    const double tile_nominal = (double)PR_TW * PR_TH * (double)groups_per_chunk * PR_G;  // one tile, one chunk of groups
+    long long per_launch = (long long)(budget / std::max(1.0, tile_nominal));
+    per_launch = std::max<long long>(grid, std::min<long long>((long long)PR_WAVES_PER_BATCH * grid, per_launch));
+    const long long n_batches = ((long long)n_tiles + per_launch - 1) / per_launch;
+    const int batch = (int)(((long long)n_tiles + n_batches - 1) / n_batches);
     const size_t smem1 = (size_t)plan.ring_bytes + (size_t)PR_NTBL * TBL + PR_SMEM_MISC;
     KB_CUDA(cudaFuncSetAttribute(bound_phase_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem1));
     PrunedTables tb{tbd.gvel, tbd.gtbl, tbd.maskx, tbd.masky, tbd.gfoot, ng, plan.ring_bytes};
