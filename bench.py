@@ -216,7 +216,7 @@ def run_reference(args):
 #                    SURVEY 8(d) counted 8 B per evaluation (psi and phi as float32): reported beside it.
 # dram__bytes_read.sum + dram__bytes_write.sum per step of the dominant kernel from the committed ncu --set full
 # capture (profiles/); None = not captured for this kernel
-TRAFFIC = {"bound_phase_kernel": 11.6e9, "search_direct_kernel": 1.37e12}  # bytes per step: profiles/r2_launches.md, r2_search_direct_kernel_full.md
+TRAFFIC = {"bound_phase_kernel": 15.8e9, "search_direct_kernel": 1.37e12}  # bytes per step: profiles/r2_launches.md, r2_search_direct_kernel_full.md
 CE_COUNT = {4: 5, 5: 9, 8: 19, 10: 32, 12: 42, 16: 63, 20: 103, 24: 132, 26: 147, 28: 162, 32: 191, 40: 305,
             48: 384, 50: 403, 56: 464, 64: 543}
 N_SM = 148
