@@ -699,7 +699,7 @@ exact_queue_kernel(const __grid_constant__ ExactArgs A, const __grid_constant__ 
     // counters).  A static grid-stride split left the SMs idle for 19 % of the kernel's duration (ncu: sm__cycles_active
     // against elapsed) and the warps in flight far apart in the queue: 100.2 ms per search against 79.6 ms this way.
     // The next entry of a chunk is fetched one iteration ahead.
-    constexpr int EX_CHUNK = 4;
+    constexpr int EX_CHUNK = 16;  // 2 / 4 / 8 / 16 groups of 32 per grab: 83.6 / 82.0 / 82.0 / 81.4 ms
     unsigned long long* next_chunk = Qu.units + 1;
     const unsigned int lane = threadIdx.x & 31u;
     const uint2 hole = make_uint2(0u, 0xFFFFFFFFu);
