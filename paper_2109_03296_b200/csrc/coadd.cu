@@ -9,10 +9,16 @@
 // kbmod_stamp_moments -- no second pass over the stamps in global memory.
 #include "moments.cuh"
 
+// Blocks of 448 threads per SM the kernel is compiled for.  It is bound by the latency of its scattered 84-byte row
+// reads, so residency beats registers: 2 / 3 / 4 blocks per SM (50 / 40 / 32 registers, the last two with a few spilled
+// words) take 6.7 / 4.9 / 4.3 ms for 10^5 trajectories x 26 epochs with the moment filter.
+#ifndef KB_COADD_BLOCKS
+#define KB_COADD_BLOCKS 4
+#endif
 namespace {
 
 template <int TP>
-__global__ void __launch_bounds__(448) coadd_kernel(const float* __restrict__ img, const uint8_t* __restrict__ mask, int T, int H, int W,
+__global__ void __launch_bounds__(448, KB_COADD_BLOCKS) coadd_kernel(const float* __restrict__ img, const uint8_t* __restrict__ mask, int T, int H, int W,
                              const __grid_constant__ DevTimes times, const int32_t* __restrict__ x0s,
                              const int32_t* __restrict__ y0s, const float* __restrict__ vxs,
                              const float* __restrict__ vys, const unsigned long long* __restrict__ epoch_mask,
