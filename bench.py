@@ -507,7 +507,9 @@ def report(R, args):
     rank, world = R["rank"], R["world"]
     # max over ranks of the device time of the timed region
     total_ms = max_over_ranks(R["total_ms"], dist, R["dev"], world)
-    e2e_steps = max(2, min(args.steps, 10))  # stacks of one kbmod_pipeline_host_batch call (a pointing group has 60, L39)
+    # stacks of one kbmod_pipeline_host_batch call (a pointing group has 60 CCD stacks, L39): the first input copy and the
+    # last result copy of a call cannot overlap a search (about 55 ms of fill and drain per call at 55 GB/s)
+    e2e_steps = max(10, min(args.steps, 20))
     # (the end-to-end leg is the replica path's: one whole stack per call; a row-band run reports the resident figure only)
     e2e_ms, h2d, d2h, same = run_e2e(R, e2e_steps) if not R["shard_rows"] else (0.0, 0, 0, False)
     e2e_max = max_over_ranks(e2e_ms, dist, R["dev"], world)

@@ -389,8 +389,27 @@ extern "C" int kbmod_plan_info(const kbmod_plan* pl, double* h_out) {
     return KBMOD_OK;
 }
 
+// the plan's tables -> the workspace (one asynchronous copy from the pinned blob; no host synchronisation)
+static int plan_upload_tables(kbmod_plan* pl, void* d_workspace, cudaStream_t st) {
+    if (!pl->uploaded) KB_CUDA(cudaEventCreateWithFlags(&pl->uploaded, cudaEventDisableTiming));
+    KB_CUDA(cudaMemcpyAsync((char*)d_workspace + pl->w_tables, pl->blob, pl->blob_bytes, cudaMemcpyHostToDevice, st));
+    KB_CUDA(cudaEventRecord(pl->uploaded, st));
+    return KBMOD_OK;
+}
+
+static int plan_search_impl(kbmod_plan* pl, const float* d_psiphi, float* d_lh, float* d_flux, int32_t* d_vel_idx,
+                            int32_t* d_n_obs, void* d_workspace, size_t workspace_bytes, void* stream, bool upload_tables);
+
 extern "C" int kbmod_plan_search(kbmod_plan* pl, const float* d_psiphi, float* d_lh, float* d_flux, int32_t* d_vel_idx,
                                  int32_t* d_n_obs, void* d_workspace, size_t workspace_bytes, void* stream) {
+    return plan_search_impl(pl, d_psiphi, d_lh, d_flux, d_vel_idx, d_n_obs, d_workspace, workspace_bytes, stream, true);
+}
+
+// upload_tables = false: the caller has put the plan's tables into this workspace already and nothing has written
+// there since (kbmod_pipeline_host_batch does, once per arena half: a table upload behind every search would queue
+// on the host-to-device copy engine after the next stack's 2 GB of inputs and hold the search up for their 35 ms)
+static int plan_search_impl(kbmod_plan* pl, const float* d_psiphi, float* d_lh, float* d_flux, int32_t* d_vel_idx,
+                            int32_t* d_n_obs, void* d_workspace, size_t workspace_bytes, void* stream, bool upload_tables) {
     KB_REQUIRE(pl && d_psiphi, KBMOD_ERR_INVALID_ARG, "NULL argument");
     if (pl->row_end == pl->row_begin) return KBMOD_OK;  // an empty band: nothing to search, nothing to write
     KB_REQUIRE(d_lh && d_flux && d_vel_idx && d_n_obs, KBMOD_ERR_INVALID_ARG, "NULL argument");
@@ -408,9 +427,10 @@ extern "C" int kbmod_plan_search(kbmod_plan* pl, const float* d_psiphi, float* d
 
     // stats + tables: one copy from the plan's blob (pinned: asynchronous, no host synchronisation); the 64 stats
     // bytes ride in front of the tables
-    if (!pl->uploaded) KB_CUDA(cudaEventCreateWithFlags(&pl->uploaded, cudaEventDisableTiming));
-    KB_CUDA(cudaMemcpyAsync(ws + pl->w_tables, pl->blob, pl->blob_bytes, cudaMemcpyHostToDevice, st));
-    KB_CUDA(cudaEventRecord(pl->uploaded, st));
+    if (upload_tables) {
+        const int rcu = plan_upload_tables(pl, d_workspace, st);
+        if (rcu) return rcu;
+    }
     unsigned long long stats[8] = {0, plane * (unsigned long long)pl->n_vel, 2, (unsigned long long)pl->algo, 0, 0, 0, 0};
     if (pl->algo == KBMOD_ALGO_DIRECT) stats[0] = stats[1];
     KB_CUDA(cudaMemsetAsync(d_stats, 0, 8 * sizeof(unsigned long long), st));
@@ -784,6 +804,11 @@ static int batch_body(int n_stacks, const float* const* h_img, const float* cons
                       void* d_arena, cudaStream_t st) {
     const size_t px = (size_t)T * H * W, res = (size_t)H * W * pl->P.K;
     // everything enqueued on `stream` before this call happens-before the first copy
+    // the plan's tables go into the workspace of each arena half once, before the first input copy is queued
+    for (int b = 0; b < (n_stacks > 1 ? 2 : 1); ++b) {
+        const int rcu = plan_upload_tables(pl, (char*)d_arena + (size_t)b * a.total + a.off_ws, st);
+        if (rcu) return rcu;
+    }
     KB_CUDA(cudaEventRecord(g_bs.comp_done[1], st));
     KB_CUDA(cudaStreamWaitEvent(g_bs.s_in, g_bs.comp_done[1], 0));
     for (int i = 0; i < n_stacks; ++i) {
@@ -803,8 +828,8 @@ static int batch_body(int n_stacks, const float* const* h_img, const float* cons
                                        hm ? (const uint8_t*)(A + a.off_mask) : nullptr, T, H, W, h_psf, n_psf, k,
                                        (float*)(A + a.off_psiphi), st);
         if (rc) return rc;
-        rc = kbmod_plan_search(pl, (const float*)(A + a.off_psiphi), (float*)(A + a.off_lh), (float*)(A + a.off_flux),
-                               (int32_t*)(A + a.off_vel), (int32_t*)(A + a.off_nobs), A + a.off_ws, a.ws_bytes, st);
+        rc = plan_search_impl(pl, (const float*)(A + a.off_psiphi), (float*)(A + a.off_lh), (float*)(A + a.off_flux),
+                              (int32_t*)(A + a.off_vel), (int32_t*)(A + a.off_nobs), A + a.off_ws, a.ws_bytes, st, false);
         if (rc) return rc;
         KB_CUDA(cudaEventRecord(g_bs.comp_done[b], st));
         KB_CUDA(cudaStreamWaitEvent(g_bs.s_out, g_bs.comp_done[b], 0));
