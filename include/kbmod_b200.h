@@ -174,6 +174,9 @@ int kbmod_search_unfiltered_lh(const void* d_workspace, const int32_t* d_vel_idx
  * pointing group, on any number of streams, share ONE plan; each search needs its own workspace of
  * kbmod_plan_workspace_bytes().  kbmod_plan_search enqueues: one table upload, the padded-stack build, the
  * search kernels, the key -> output pass; it never synchronises and never touches pageable host memory.
+ * The table upload (a few MB, host to device from pinned memory) is ordered by the device's copy engine: behind a large
+ * host-to-device copy that is in flight on another stream it waits for that copy, and the search with it.
+ * kbmod_pipeline_host_batch, which has such copies in flight by design, uploads the tables once per call instead.
  *   row_begin, row_end   the band of start rows this plan searches (0, H for the whole image)
  * kbmod_plan_info fills h_out[10]: kernel used (KBMOD_ALGO_DIRECT / PRUNED), velocity groups, bytes staged into shared
  * memory per trajectory-epoch evaluation, share of (tile, group, epoch) region loads that lie off the image, padded
