@@ -27,10 +27,16 @@ constexpr int SD_THREADS = SD_BX * SD_BY;
 // mode (B): 4 / 5 / 6 blocks per SM take 2.33 / 2.29 / 2.32 s (6 blocks: 80 registers, spills); with the 16-byte
 // (psi, phi, f, valid) cell of the earlier design (128 registers, 4 blocks) 2.82 s; in list order +0.5 s.
 constexpr int SD_BLOCKS_PER_SM = KB_SD_BLOCKS;
+// ... for lightcurves of up to 28 epochs.  Longer ones need more registers (2 x T values + the sort's copy; at 96
+// registers T = 50 spills 488 bytes per thread): 3 blocks per SM (170 registers).  Measured on configs[3], mode (B),
+// T = 50: 5 / 4 / 3 / 2 blocks per SM take 31.5 / 18.8 / 16.4 / 19.1 s.
+template <int TP> struct SdCfg {
+    static constexpr int blocks = TP <= 28 ? SD_BLOCKS_PER_SM : 3;
+};
 constexpr int SD_SBW = 8, SD_SBH = 64;  // super-block of tiles: 8 x 32 = 256 pixels wide, 64 x 4 = 256 rows tall
 
 template <int TP>
-__global__ void __launch_bounds__(SD_THREADS, SD_BLOCKS_PER_SM)
+__global__ void __launch_bounds__(SD_THREADS, SdCfg<TP>::blocks)
 search_direct_kernel(const float2* __restrict__ S4, const __grid_constant__ S4Geom G, const int* __restrict__ off,
                      const int* __restrict__ order, int W, int row_begin, int row_end, int n_vel,
                      const __grid_constant__ DevParams P, unsigned long long* __restrict__ keys_out,
@@ -118,9 +124,9 @@ int kb_launch_search_direct(int TPv, const void* d_S4, const S4Geom& G, const in
     KB_CUDA(cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev));
     const dim3 block(SD_BX, SD_BY);
     const int n_tiles = ((W + SD_BX - 1) / SD_BX) * ((n_rows + SD_BY - 1) / SD_BY);
-    const dim3 grid(std::min(n_tiles, n_sm * SD_BLOCKS_PER_SM));
     KB_CUDA(cudaMemsetAsync(d_next_unit, 0, sizeof(unsigned long long), st));
     KB_DISPATCH_TP(TPv, {
+        const dim3 grid(std::min(n_tiles, n_sm * SdCfg<TP>::blocks));
         const size_t smem = (size_t)TP * SD_THREADS * sizeof(float) + (size_t)P.K * SD_THREADS * sizeof(unsigned long long);
         KB_CUDA(cudaFuncSetAttribute(search_direct_kernel<TP>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         search_direct_kernel<TP><<<grid, block, smem, st>>>(reinterpret_cast<const float2*>(d_S4), G, d_off, d_order, W,

@@ -683,12 +683,26 @@ constexpr int EX_THREADS = KB_EX_THREADS;
 #define KB_EX_CTAS 2
 #endif
 constexpr int EX_CTAS_PER_SM = KB_EX_CTAS;
+#ifndef KB_EX_BIG_T
+#define KB_EX_BIG_T 32
+#endif
+#ifndef KB_EX_BIG_THREADS
+#define KB_EX_BIG_THREADS 256
+#endif
+// lightcurves longer than KB_EX_BIG_T epochs do not fit 128 registers (T = 50: 228 bytes spilled per thread): one CTA
+// of 256 threads per SM and up to 255 registers instead.  The phase is not occupancy-bound, the spills
+// cost: configs[3]'s exact phase 1147 -> 1062 ms (384 threads at 168 registers: 1068; 512 at 128, spilling: 1166)
+template <int TP> struct ExCfg {
+    static constexpr bool big = TP > KB_EX_BIG_T;
+    static constexpr int ctas = big ? 1 : EX_CTAS_PER_SM;
+    static constexpr int threads = big ? KB_EX_BIG_THREADS : EX_THREADS;
+};
 
 template <int TP>
-__global__ void __launch_bounds__(EX_THREADS, EX_CTAS_PER_SM)
+__global__ void __launch_bounds__(ExCfg<TP>::threads, ExCfg<TP>::ctas)
 exact_queue_kernel(const __grid_constant__ ExactArgs A, const __grid_constant__ DevParams P,
                    const __grid_constant__ Queue Qu, unsigned long long* __restrict__ stats) {
-    extern __shared__ float scratch_all[];  // [TP][EX_THREADS]
+    extern __shared__ float scratch_all[];  // [TP][threads]
     const unsigned long long cnt = *Qu.count;
     const unsigned long long n = cnt < Qu.cap ? cnt : Qu.cap;
     unsigned long long done = 0, passed = 0;
@@ -717,7 +731,7 @@ exact_queue_kernel(const __grid_constant__ ExactArgs A, const __grid_constant__ 
             e_next = (k + 1 < EX_CHUNK && i_next < n) ? __ldg(Qu.entries + i_next) : hole;
             if (e.y != 0xFFFFFFFFu) {
                 const int y0 = (int)(e.x / (unsigned)A.W), x0 = (int)(e.x - (unsigned)y0 * (unsigned)A.W);
-                passed += eval_pair<TP>(A, P, x0, y0, (int)e.y, scratch_all + threadIdx.x, EX_THREADS) ? 1ull : 0ull;
+                passed += eval_pair<TP>(A, P, x0, y0, (int)e.y, scratch_all + threadIdx.x, ExCfg<TP>::threads) ? 1ull : 0ull;
                 ++done;
             }
             __syncwarp();
@@ -1143,7 +1157,8 @@ int kb_launch_search_pruned(const float* d_psiphi, const PrunedPlan& plan, const
     ExactArgs EA{reinterpret_cast<const float2*>(d_S4), G, d_off, W, row_begin, row_end, d_keys};
     KB_DISPATCH_TP(TPv, {
         const size_t smem2 = (size_t)TP * EX_THREADS * sizeof(float);
-        KB_CUDA(cudaFuncSetAttribute(exact_queue_kernel<TP>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem2));
+        const size_t smem2q = (size_t)TP * ExCfg<TP>::threads * sizeof(float);
+        KB_CUDA(cudaFuncSetAttribute(exact_queue_kernel<TP>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem2q));
         KB_CUDA(cudaFuncSetAttribute(exact_overflow_kernel<TP>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem2));
         if (ng > 0) {
             for (int b0 = 0; b0 < n_tiles; b0 += batch) {
@@ -1155,7 +1170,7 @@ int kb_launch_search_pruned(const float* d_psiphi, const PrunedPlan& plan, const
                                                                                           g0, g1, tb, bp, P.min_obs, d_thrtab, Qu);
                     KB_CUDA(cudaGetLastError());
                     kb_phase_mark(KB_PHASE_BOUND, st);
-                    exact_queue_kernel<TP><<<n_sm * EX_CTAS_PER_SM, EX_THREADS, smem2, st>>>(EA, P, Qu, d_stats);
+                    exact_queue_kernel<TP><<<n_sm * ExCfg<TP>::ctas, ExCfg<TP>::threads, smem2q, st>>>(EA, P, Qu, d_stats);
                     KB_CUDA(cudaGetLastError());
                     kb_phase_mark(KB_PHASE_EXACT, st);
                     launches += 2;
